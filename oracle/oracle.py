@@ -1,0 +1,215 @@
+"""ctypes face of oracle/cwo_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+may import this module.  It imports nothing from paper_1107_5578_b200 and the package
+imports nothing from here.  All arithmetic lives in cwo_oracle.c (double precision);
+this file only marshals numpy arrays.
+
+Citations: P:Lnnn = /root/reference/PAPER.md line nnn.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cwo_oracle.c")
+_SO = os.path.join(_HERE, "libcwo_oracle.so")
+
+METHOD_FRESNEL = 0   # config c5 (BASELINE.json configs[4])
+METHOD_ASM = 1       # the paper's own Listing 8
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -fopenmp the oracle into oracle/libcwo_oracle.so (rebuilds when the source is newer)."""
+    if (not force and os.path.exists(_SO)
+            and os.path.getmtime(_SO) >= os.path.getmtime(_SRC)):
+        return _SO
+    tmp = _SO + ".tmp%d" % os.getpid()
+    cmd = ["gcc", "-std=c99", "-O2", "-fopenmp", "-fno-fast-math", "-ffp-contract=off",
+           "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _SO)
+    return _SO
+
+
+_lib = None
+_c128 = np.ctypeslib.ndpointer(dtype=np.complex128, flags="C_CONTIGUOUS")
+_f64 = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_i32 = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+_I, _D = ctypes.c_int, ctypes.c_double
+
+
+def lib():
+    global _lib
+    if _lib is not None:
+        return _lib
+    L = ctypes.CDLL(build())
+    L.cwo_oracle_set_threads.argtypes = [_I]
+    L.cwo_oracle_get_threads.restype = _I
+    L.cwo_oracle_max_threads.restype = _I
+    L.cwo_oracle_dft1d.argtypes = [_I, _c128, _c128, _I]
+    L.cwo_oracle_fft1d.argtypes = [_I, _c128, _c128, _I]
+    L.cwo_oracle_fft2d.argtypes = [_I, _I, _c128, _I]
+    L.cwo_oracle_dft2d.argtypes = [_I, _I, _c128, _c128, _I]
+    L.cwo_oracle_asm_transfer.argtypes = [_I, _I, _D, _D, _D, _D, _c128]
+    L.cwo_oracle_asm.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_asm_naive.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_stack.argtypes = [_I, _I, _D, _D, _D, _f64, _I, _c128, _c128]
+    L.cwo_oracle_fresnel_points.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _I, _i32, _i32, _c128]
+    L.cwo_oracle_fresnel_direct.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_fresnel_conv.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_rs_direct.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_gs_init.argtypes = [_I, _I, _I, _D, _D, _D, _D, _f64, _f64, _c128]
+    L.cwo_oracle_gs_iter.argtypes = [_I, _I, _I, _D, _D, _D, _D, _f64, _f64, _c128, ctypes.c_void_p]
+    L.cwo_oracle_gs.argtypes = [_I, _I, _I, _D, _D, _D, _D, _I, _f64, _f64, _f64]
+    L.cwo_oracle_gs_error.argtypes = [_I, _I, _I, _D, _D, _D, _D, _f64, _f64, _c128]
+    L.cwo_oracle_gs_error.restype = _D
+    _lib = L
+    return L
+
+
+def set_threads(t: int) -> None:
+    lib().cwo_oracle_set_threads(int(t))
+
+
+def max_threads() -> int:
+    return int(lib().cwo_oracle_max_threads())
+
+
+def _z(a) -> np.ndarray:
+    """Widen (complex64-rounded) input to a fresh contiguous complex128 array."""
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _d(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise ValueError("oracle %s failed with code %d" % (what, rc))
+
+
+def dft1d(x, sign=-1):
+    x = _z(x); out = np.empty_like(x)
+    lib().cwo_oracle_dft1d(x.size, x, out, sign)
+    return out
+
+
+def fft1d(x, sign=-1):
+    x = _z(x); out = np.empty_like(x)
+    _check(lib().cwo_oracle_fft1d(x.size, x, out, sign), "fft1d")
+    return out
+
+
+def fft2d(a, sign=-1):
+    a = _z(a).copy()
+    ny, nx = a.shape
+    _check(lib().cwo_oracle_fft2d(ny, nx, a, sign), "fft2d")
+    return a
+
+
+def dft2d(a, sign=-1):
+    a = _z(a); out = np.empty_like(a)
+    ny, nx = a.shape
+    lib().cwo_oracle_dft2d(ny, nx, a, out, sign)
+    return out
+
+
+def asm_transfer(ny, nx, px, py, lam, z):
+    H = np.empty((ny, nx), np.complex128)
+    lib().cwo_oracle_asm_transfer(ny, nx, px, py, lam, z, H)
+    return H
+
+
+def asm(u1, px, py, lam, z, naive=False):
+    """Angular spectrum method, Eq.(15)-(17) P:L194-211."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    if naive:
+        lib().cwo_oracle_asm_naive(ny, nx, px, py, lam, z, u1, u2)
+    else:
+        _check(lib().cwo_oracle_asm(ny, nx, px, py, lam, z, u1, u2), "asm")
+    return u2
+
+
+def stack(u1, px, py, lam, zs):
+    """Diffract3D: out[k] = asm(u1, zs[k])."""
+    u1 = _z(u1); zs = _d(zs)
+    ny, nx = u1.shape
+    out = np.empty((zs.size, ny, nx), np.complex128)
+    _check(lib().cwo_oracle_stack(ny, nx, px, py, lam, zs, zs.size, u1, out), "stack")
+    return out
+
+
+def fresnel_conv(u1, px, py, lam, z):
+    """Literal Eq.(5) pipeline with the 2N expansion."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    _check(lib().cwo_oracle_fresnel_conv(ny, nx, px, py, lam, z, u1, u2), "fresnel_conv")
+    return u2
+
+
+def fresnel_direct(u1, px, py, lam, z):
+    """Direct O(N^4) linear convolution = Eq.(1) discretised."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    lib().cwo_oracle_fresnel_direct(ny, nx, px, py, lam, z, u1, u2)
+    return u2
+
+
+def fresnel_points(u1, px, py, lam, z, ms, ns):
+    """Direct-sum value of u2[ns[i], ms[i]] for a handful of samples (array indices)."""
+    u1 = _z(u1)
+    ny, nx = u1.shape
+    ms = np.ascontiguousarray(ms, np.int32); ns = np.ascontiguousarray(ns, np.int32)
+    out = np.empty(ms.size, np.complex128)
+    lib().cwo_oracle_fresnel_points(ny, nx, px, py, lam, z, u1, ms.size, ms, ns, out)
+    return out
+
+
+def rs_direct(u1, px, py, lam, z):
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    lib().cwo_oracle_rs_direct(ny, nx, px, py, lam, z, u1, u2)
+    return u2
+
+
+def gs_init(method, amp_dst, phi0, px, py, lam, z):
+    amp_dst = _d(amp_dst); phi0 = _d(phi0)
+    ny, nx = amp_dst.shape
+    p = np.empty((ny, nx), np.complex128)
+    _check(lib().cwo_oracle_gs_init(method, ny, nx, px, py, lam, z, amp_dst, phi0, p), "gs_init")
+    return p
+
+
+def gs_iter(method, amp_src, amp_dst, p, px, py, lam, z, want_G=False):
+    """One loop pass (Listing 8 lines 8-17).  Returns the new p (and G of this pass)."""
+    amp_src = _d(amp_src); amp_dst = _d(amp_dst); p = _z(p).copy()
+    ny, nx = p.shape
+    G = np.empty_like(p) if want_G else None
+    gp = G.ctypes.data_as(ctypes.c_void_p) if want_G else None
+    _check(lib().cwo_oracle_gs_iter(method, ny, nx, px, py, lam, z, amp_src, amp_dst, p, gp), "gs_iter")
+    return (p, G) if want_G else p
+
+
+def gs(method, amp_src, amp_dst, phi0, px, py, lam, z, iters):
+    amp_src = _d(amp_src); amp_dst = _d(amp_dst); ph = _d(phi0).copy()
+    ny, nx = ph.shape
+    _check(lib().cwo_oracle_gs(method, ny, nx, px, py, lam, z, iters, amp_src, amp_dst, ph), "gs")
+    return ph
+
+
+def gs_error(method, amp_src, amp_dst, p, px, py, lam, z):
+    amp_src = _d(amp_src); amp_dst = _d(amp_dst); p = _z(p)
+    ny, nx = p.shape
+    return float(lib().cwo_oracle_gs_error(method, ny, nx, px, py, lam, z, amp_src, amp_dst, p))
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))
