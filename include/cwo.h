@@ -1,0 +1,122 @@
+/*
+ * cwo.h -- C ABI of libcwo.so: FFT-based scalar light propagation on one NVIDIA B200 (sm_100a).
+ *
+ * The calls follow the paper's statement of the problem (arxiv/paper_1107_5578, "CWO++"):
+ * a source plane u1, a destination plane u2, a propagation distance z, a wavelength and the
+ * sampling pitches.  P:Lnnn = line nnn of the paper text.
+ *
+ * Common rules
+ *   Layout     Every field is a DEVICE pointer, row-major [Ny][Nx], x fastest, dense (row stride
+ *              Nx), 16-byte aligned.  Complex fields are interleaved (re, im) float pairs
+ *              (8*Nx*Ny bytes); real fields are float (4*Nx*Ny bytes).
+ *   Ownership  The caller owns every buffer, including the workspace.  A plan owns only small
+ *              lookup tables (<= ~1.3 MiB) that it allocates with cudaMalloc at plan time or on the first call
+ *              that needs them.  No call allocates or frees caller-visible memory.
+ *   Asynchrony Every propagation call only enqueues kernels on the plan's stream and returns;
+ *              results are valid once the caller has synchronised that stream.  No hidden
+ *              host<->device copies of field data.  Host arrays (zs) are read before return.
+ *   Aliasing   u2 == u1 (exact in-place, as the paper's c.Diffract) is allowed.
+ *              Partial overlap, or overlap with the workspace, is the caller's error.
+ *   Errors     int return, CWO_OK == 0, negative on failure.  Nothing is enqueued when a call
+ *              returns CWO_EINVAL / CWO_EWORKSPACE / CWO_EUNSUPPORTED.  No exceptions, no
+ *              global state; use one plan per host thread at a time.
+ *   Sizes      Nx, Ny powers of two.  cwo_asm / cwo_propagate_stack: 32..16384 per axis.
+ *              cwo_fresnel_conv (transforms of 2Nx x 2Ny): 16..8192 per axis.  cwo_gs: the
+ *              range of its propagator.
+ *   Sign       z < 0 is back-propagation for both methods.
+ *   FFT        forward kernel exp(-i 2 pi jk/n), inverse exp(+i 2 pi jk/n) scaled 1/(Mx*My)
+ *              (the paper is silent; with this choice cwo_asm at z = 0 is the identity).
+ */
+#ifndef CWO_H_
+#define CWO_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cwo_plan_s* cwo_plan_t;
+typedef struct { float re, im; } cwo_c64;      /* == float2 == torch.complex64 element */
+
+enum {
+    CWO_OK = 0,
+    CWO_EINVAL = -1,        /* bad argument: null/unaligned pointer, unsupported size, lambda/pitch <= 0,
+                               non-finite z, z == 0 for Fresnel, n <= 0, iters < 0 */
+    CWO_EWORKSPACE = -2,    /* workspace missing or smaller than cwo_plan_workspace_bytes() */
+    CWO_EUNSUPPORTED = -3,  /* current device is not compute capability 10.x */
+    CWO_ECUDA = -4          /* CUDA runtime failure; code via cwo_last_cuda_error() */
+};
+
+enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4 };
+
+enum {
+    CWO_OPT_GS_METHOD = 1   /* value: CWO_GS_FRESNEL (default; BASELINE config 5) or CWO_GS_ASM
+                               (the paper's Listing 8) */
+};
+enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
+
+/* Plane parameters (SetPitch / SetWaveLength / Create).  pitch_x = pitch_y = pitch
+ * [m], lambda [m].  Frequency sampling is 1/(M*pitch) with M the transform size.
+ * Builds the FFT twiddle tables on the current CUDA device (tiny kernels on the null stream,
+ * synchronised before return). */
+int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t* plan_out);
+int cwo_plan_destroy(cwo_plan_t plan);
+
+/* Stream (a cudaStream_t passed as void*) that all later calls enqueue on.  Default: null stream. */
+int cwo_plan_set_stream(cwo_plan_t plan, void* cuda_stream);
+
+/* The paper allows px != py (SetPitch(px, py)). */
+int cwo_plan_set_pitch_xy(cwo_plan_t plan, double px, double py);
+
+int cwo_plan_set_option(cwo_plan_t plan, int key, int value);
+
+/* Workspace a call needs, in bytes (n = number of planes for CWO_OP_STACK, ignored otherwise):
+ *   ASM      8*Nx*Ny            (the row-transformed field in column-tile order)
+ *   FRESNEL  16*Nx*Ny           (Ny rows x 2Nx columns; the 2Nx x 2Ny padded array is never stored)
+ *   STACK    16*Nx*Ny           (spectrum + one plane in flight)
+ *   GS       propagator's workspace + 8*Nx*Ny (the constrained field between propagations)
+ * Returns 0 for an unknown op. */
+size_t cwo_plan_workspace_bytes(cwo_plan_t plan, int op, int n);
+
+/* Device memory the calls may scribble on; 256-byte aligned; must outlive the calls using it. */
+int cwo_plan_set_workspace(cwo_plan_t plan, void* dev_ptr, size_t bytes);
+
+/* Angular spectrum method, Eq.(15)-(17):
+ *   u2 = IFFT2[ FFT2[u1] * H ],  H(k,l) = exp(i 2 pi z sqrt(1/lambda^2 - fx(k)^2 - fy(l)^2)),
+ *   H = 0 where the radicand is negative (evanescent), fx(k) = k_signed/(Nx*px).
+ * Unpadded Nx x Ny circular transform.  z = 0 is the identity. */
+int cwo_asm(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
+
+/* Fresnel diffraction, convolution form, Eq.(1)-(6) with the 2Nx x 2Ny expansion of
+ * P:L235:  u2 = exp(i 2 pi z/lambda)/(i lambda z) * px*py * crop( IFFT2[ FFT2[pad u1] * FFT2[h_F] ] ),
+ * h_F(m,n) = exp(i pi ((m px)^2 + (n py)^2)/(lambda z)) sampled at taps -N..N-1 per axis; i.e. the
+ * exact linear convolution of u1 with the sampled impulse response.  z == 0 -> CWO_EINVAL. */
+int cwo_fresnel_conv(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
+
+/* 3-D diffraction as a stack of 2-D diffractions (Diffract3D): out[k] = cwo_asm(u1, zs[k]),
+ * k = 0..n-1, the forward FFT of u1 computed once.  zs: HOST array of n doubles.  out: device,
+ * [n][Ny][Nx] complex; must not overlap u1. */
+int cwo_propagate_stack(cwo_plan_t plan, const cwo_c64* u1, const double* zs, int n, cwo_c64* out);
+
+/* Gerchberg-Saxton loop (section 7.2, Listing 8) between a source (hologram)
+ * plane with amplitude amp_src and a destination (image) plane with amplitude amp_dst, z apart:
+ *   G = amp_dst * exp(i phase_out);  p = phasor(P(-z)[G]);
+ *   repeat iters times:  q = phasor(P(+z)[amp_src * p]);  p = phasor(P(-z)[amp_dst * q]);
+ *   phase_out = atan2(Im p, Re p)  in [-pi, pi];   phasor(u) = u/|u|, 1 where u == 0.
+ * P = cwo_fresnel_conv or cwo_asm per CWO_OPT_GS_METHOD.  phase_out is in/out (the library has no
+ * random generator; the paper's SetRandPhase seed is unspecified).  iters == 0 yields the
+ * kinoform of section 7.1.  amp_src, amp_dst, phase_out: float [Ny][Nx], device. */
+int cwo_gs(cwo_plan_t plan, const float* amp_src, const float* amp_dst, double z, int iters,
+           float* phase_out);
+
+const char* cwo_strerror(int code);
+int cwo_last_cuda_error(cwo_plan_t plan);
+
+/* Number of kernels the library has launched through this plan so far (bench accounting). */
+long long cwo_plan_launch_count(cwo_plan_t plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CWO_H_ */

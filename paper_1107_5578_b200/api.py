@@ -1,0 +1,173 @@
+"""Thin Python binding of libcwo.so (include/cwo.h): argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels; torch is used for device memory and
+streams.  There is no CPU fallback: if libcwo.so cannot be loaded this module raises.
+
+    plan = cwo_plan(Nx, Ny, pitch, lam)
+    cwo_asm(plan, u1, u2, z)                     # u1, u2: torch.complex64 CUDA tensors [Ny, Nx]
+    cwo_fresnel_conv(plan, u1, u2, z)
+    cwo_propagate_stack(plan, u1, zs, out)       # out: [n, Ny, Nx]
+    cwo_gs(plan, amp_src, amp_dst, z, iters, phase)   # phase: float32 in/out
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libcwo.so")
+
+CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA = 0, -1, -2, -3, -4
+CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS = 1, 2, 3, 4
+CWO_OPT_GS_METHOD = 1
+CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
+
+EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",
+           "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_asm", "cwo_fresnel_conv",
+           "cwo_propagate_stack", "cwo_gs", "cwo_strerror", "cwo_last_cuda_error", "cwo_plan_launch_count"]
+
+_lib = None
+
+
+class CwoError(RuntimeError):
+    def __init__(self, code: int, what: str, cuda: int = 0):
+        self.code = code
+        msg = "%s: %s" % (what, lib().cwo_strerror(code).decode())
+        if code == CWO_ECUDA:
+            msg += " (cudaError %d)" % cuda
+        super().__init__(msg)
+
+
+def lib() -> ctypes.CDLL:
+    """Load libcwo.so (built in-tree by paper_1107_5578_b200/build.py).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError("libcwo.so is missing (%s): run `python -m paper_1107_5578_b200.build`; "
+                          "there is no CPU fallback" % _LIB_PATH)
+    L = ctypes.CDLL(_LIB_PATH)
+    vp, I, D, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    L.cwo_plan.argtypes = [I, I, D, D, ctypes.POINTER(vp)]
+    L.cwo_plan_destroy.argtypes = [vp]
+    L.cwo_plan_set_stream.argtypes = [vp, vp]
+    L.cwo_plan_set_pitch_xy.argtypes = [vp, D, D]
+    L.cwo_plan_set_option.argtypes = [vp, I, I]
+    L.cwo_plan_workspace_bytes.argtypes = [vp, I, I]
+    L.cwo_plan_workspace_bytes.restype = sz
+    L.cwo_plan_set_workspace.argtypes = [vp, vp, sz]
+    L.cwo_asm.argtypes = [vp, vp, vp, D]
+    L.cwo_fresnel_conv.argtypes = [vp, vp, vp, D]
+    L.cwo_propagate_stack.argtypes = [vp, vp, ctypes.POINTER(D), I, vp]
+    L.cwo_gs.argtypes = [vp, vp, vp, D, I, vp]
+    L.cwo_strerror.argtypes = [I]
+    L.cwo_strerror.restype = ctypes.c_char_p
+    L.cwo_last_cuda_error.argtypes = [vp]
+    L.cwo_plan_launch_count.argtypes = [vp]
+    L.cwo_plan_launch_count.restype = ctypes.c_longlong
+    _lib = L
+    return L
+
+
+class Plan:
+    """Owns a cwo_plan_t and (optionally) a torch-allocated workspace handed to the library."""
+
+    def __init__(self, Nx: int, Ny: int, pitch: float, lam: float):
+        self.Nx, self.Ny = int(Nx), int(Ny)
+        self._h = ctypes.c_void_p()
+        self._ws = None
+        rc = lib().cwo_plan(self.Nx, self.Ny, float(pitch), float(lam), ctypes.byref(self._h))
+        if rc != CWO_OK:
+            raise CwoError(rc, "cwo_plan")
+
+    def _check(self, rc: int, what: str) -> None:
+        if rc != CWO_OK:
+            raise CwoError(rc, what, lib().cwo_last_cuda_error(self._h))
+
+    def set_pitch_xy(self, px: float, py: float) -> None:
+        self._check(lib().cwo_plan_set_pitch_xy(self._h, float(px), float(py)), "cwo_plan_set_pitch_xy")
+
+    def set_option(self, key: int, value: int) -> None:
+        self._check(lib().cwo_plan_set_option(self._h, int(key), int(value)), "cwo_plan_set_option")
+
+    def workspace_bytes(self, op: int, n: int = 0) -> int:
+        return int(lib().cwo_plan_workspace_bytes(self._h, int(op), int(n)))
+
+    def set_workspace(self, t: "torch.Tensor | None") -> None:
+        self._ws = t
+        if t is None:
+            self._check(lib().cwo_plan_set_workspace(self._h, None, 0), "cwo_plan_set_workspace")
+        else:
+            self._check(lib().cwo_plan_set_workspace(self._h, t.data_ptr(), t.numel() * t.element_size()),
+                        "cwo_plan_set_workspace")
+
+    def ensure_workspace(self, op: int, n: int = 0) -> None:
+        need = self.workspace_bytes(op, n)
+        have = 0 if self._ws is None else self._ws.numel()
+        if have < need:
+            self.set_workspace(torch.empty(need, dtype=torch.uint8, device="cuda"))
+
+    def bind_stream(self) -> None:
+        self._check(lib().cwo_plan_set_stream(self._h, torch.cuda.current_stream().cuda_stream), "cwo_plan_set_stream")
+
+    @property
+    def launch_count(self) -> int:
+        return int(lib().cwo_plan_launch_count(self._h))
+
+    def close(self) -> None:
+        if self._h:
+            lib().cwo_plan_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _field(t: torch.Tensor, dtype, shape, name: str) -> int:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()
+            and tuple(t.shape) == tuple(shape)):
+        raise TypeError("%s must be a contiguous CUDA %s tensor of shape %s" % (name, dtype, tuple(shape)))
+    return t.data_ptr()
+
+
+def cwo_plan(Nx: int, Ny: int, pitch: float, lam: float) -> Plan:
+    return Plan(Nx, Ny, pitch, lam)
+
+
+def cwo_asm(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
+    s = (plan.Ny, plan.Nx)
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.complex64, s, "u2")
+    plan.ensure_workspace(CWO_OP_ASM); plan.bind_stream()
+    plan._check(lib().cwo_asm(plan._h, a, b, float(z)), "cwo_asm")
+
+
+def cwo_fresnel_conv(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
+    s = (plan.Ny, plan.Nx)
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.complex64, s, "u2")
+    plan.ensure_workspace(CWO_OP_FRESNEL); plan.bind_stream()
+    plan._check(lib().cwo_fresnel_conv(plan._h, a, b, float(z)), "cwo_fresnel_conv")
+
+
+def cwo_propagate_stack(plan: Plan, u1: torch.Tensor, zs: Sequence[float], out: torch.Tensor) -> None:
+    n = len(zs)
+    a = _field(u1, torch.complex64, (plan.Ny, plan.Nx), "u1")
+    b = _field(out, torch.complex64, (n, plan.Ny, plan.Nx), "out")
+    arr = (ctypes.c_double * n)(*[float(z) for z in zs])
+    plan.ensure_workspace(CWO_OP_STACK, n); plan.bind_stream()
+    plan._check(lib().cwo_propagate_stack(plan._h, a, arr, n, b), "cwo_propagate_stack")
+
+
+def cwo_gs(plan: Plan, amp_src: torch.Tensor, amp_dst: torch.Tensor, z: float, iters: int,
+           phase: torch.Tensor) -> None:
+    s = (plan.Ny, plan.Nx)
+    a = _field(amp_src, torch.float32, s, "amp_src")
+    b = _field(amp_dst, torch.float32, s, "amp_dst")
+    c = _field(phase, torch.float32, s, "phase")
+    plan.ensure_workspace(CWO_OP_GS); plan.bind_stream()
+    plan._check(lib().cwo_gs(plan._h, a, b, float(z), int(iters), c), "cwo_gs")

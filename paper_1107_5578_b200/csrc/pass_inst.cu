@@ -1,0 +1,15 @@
+// pass_inst.cu -- instantiates the pass kernels for ONE transform length; compiled once per
+// CWO_LOGN in [5, 14] (see build.py) so the ten lengths build in parallel.
+#include "pass_kernel.cuh"
+
+#ifndef CWO_LOGN
+#error "compile with -DCWO_LOGN=<5..14>"
+#endif
+
+namespace cwo {
+#define CWO_CAT2(a, b) a##b
+#define CWO_CAT(a, b) CWO_CAT2(a, b)
+cudaError_t CWO_CAT(launch_pass_, CWO_LOGN)(int kind, int n_tiles, cudaStream_t s, const PassParams& p) {
+    return launch_pass_impl<CWO_LOGN>(kind, n_tiles, s, p);
+}
+}  // namespace cwo

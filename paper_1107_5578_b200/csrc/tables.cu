@@ -1,0 +1,80 @@
+// tables.cu -- small double-precision table builders.
+//   * FFT twiddles exp(-i 2 pi m/n), evaluated in fp64 and rounded once to fp32.
+//   * Fresnel: the spectrum C[k] of the sampled 1-D chirp (impulse response of Eq.(3)/(6), P:L113,
+//     P:L132, taps d = -N..N-1 stored wrapped at d mod 2N), by a single-CTA fp64 Stockham FFT in
+//     global scratch.  FFT2[h_F](k,l) = Cx[k]*Cy[l] exactly because h_F is separable, so the
+//     2N x 2N impulse response and its FFT (the paper's FresnelConvProp + FFT) are never formed.
+#include "cwo_internal.h"
+
+namespace cwo {
+
+__global__ void twiddle_kernel(float2* tw, int n) {
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n) return;
+    double s, c;
+    sincospi(-2.0 * (double)m / (double)n, &s, &c);
+    tw[m] = make_float2((float)c, (float)s);
+}
+
+__global__ void twiddle64_kernel(double2* tw, int n) {
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= n / 2) return;
+    double s, c;
+    sincospi(-2.0 * (double)m / (double)n, &s, &c);
+    tw[m] = make_double2(c, s);
+}
+
+cudaError_t build_twiddles(float2* tw, int n, cudaStream_t s) {
+    twiddle_kernel<<<(n + 255) / 256, 256, 0, s>>>(tw, n);
+    return cudaGetLastError();
+}
+cudaError_t build_twiddles_f64(double2* tw, int n, cudaStream_t s) {
+    twiddle64_kernel<<<(n / 2 + 255) / 256, 256, 0, s>>>(tw, n);
+    return cudaGetLastError();
+}
+
+__device__ __forceinline__ double2 zmul(double2 a, double2 b) {
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+
+// One CTA per axis.  x[i] = exp(i 2 pi a d^2), d = i < M/2 ? i : i - M, a = pitch^2/(2 lambda z) in
+// cycles; radix-2 Stockham stages ping-pong between the two halves of scratch; out = coef * X.
+__global__ void __launch_bounds__(1024) chirp_fft_kernel(ChirpAxis ax0, ChirpAxis ax1) {
+    const ChirpAxis& ax = (blockIdx.x == 0) ? ax0 : ax1;
+    const int M = 1 << ax.logm, H = M >> 1;
+    double2* a = ax.scratch;
+    double2* b = ax.scratch + M;
+    for (int i = threadIdx.x; i < M; i += blockDim.x) {
+        double d = (double)((i < H) ? i : i - M);
+        double c = ax.a_cycles * d * d;      // |c| <= ~3e3 cycles: fp64 keeps ~1e-13 cycles
+        c -= rint(c);
+        double s, co;
+        sincospi(2.0 * c, &s, &co);
+        a[i] = make_double2(co, s);
+    }
+    __syncthreads();
+    for (int lns = 0; lns < ax.logm; ++lns) {
+        const int ns = 1 << lns;
+        for (int j = threadIdx.x; j < H; j += blockDim.x) {
+            int k = j & (ns - 1);
+            double2 w = ax.tw64[k << (ax.logm - 1 - lns)];
+            double2 x0 = a[j], x1 = zmul(a[j + H], w);
+            int j0 = ((j >> lns) << (lns + 1)) + k;
+            b[j0] = make_double2(x0.x + x1.x, x0.y + x1.y);
+            b[j0 + ns] = make_double2(x0.x - x1.x, x0.y - x1.y);
+        }
+        __syncthreads();
+        double2* t = a; a = b; b = t;
+    }
+    for (int i = threadIdx.x; i < M; i += blockDim.x) {
+        double2 r = zmul(a[i], ax.coef);
+        ax.out[i] = make_float2((float)r.x, (float)r.y);
+    }
+}
+
+cudaError_t build_chirp_spectrum(const ChirpAxis& ax0, const ChirpAxis* ax1, cudaStream_t s) {
+    chirp_fft_kernel<<<ax1 ? 2 : 1, 1024, 0, s>>>(ax0, ax1 ? *ax1 : ax0);
+    return cudaGetLastError();
+}
+
+}  // namespace cwo

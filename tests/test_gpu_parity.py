@@ -1,0 +1,328 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle, element by element.
+
+Bar (BASELINE.json north_star): relative L2 <= 2e-5 and max abs error <= 1e-4 * peak |u2_oracle|,
+fp32 against double on the same seeded complex64 inputs.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from paper_1107_5578_b200 import workloads as W   # noqa: E402
+
+REL_L2, MAX_ABS = 2e-5, 1e-4
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1107_5578_b200 import api as a
+    a.lib()
+    return a
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _assert_parity(got, ref, what=""):
+    got = np.asarray(got).astype(np.complex128); ref = np.asarray(ref)
+    rel = np.linalg.norm((got - ref).ravel()) / np.linalg.norm(ref.ravel())
+    mx = np.max(np.abs(got - ref)) / np.max(np.abs(ref))
+    assert rel <= REL_L2 and mx <= MAX_ABS, "%s rel-L2 %.3e max/peak %.3e" % (what, rel, mx)
+    return rel, mx
+
+
+def _rand(shape, seed):
+    r = np.random.default_rng(seed)
+    return (r.standard_normal(shape) + 1j * r.standard_normal(shape)).astype(np.complex64)
+
+
+def _gpu_asm(api, u1, px, py, lam, z, inplace=False):
+    ny, nx = u1.shape
+    plan = api.cwo_plan(nx, ny, px, lam)
+    if px != py:
+        plan.set_pitch_xy(px, py)
+    d1 = _dev(u1)
+    d2 = d1 if inplace else torch.empty_like(d1)
+    api.cwo_asm(plan, d1, d2, z)
+    torch.cuda.synchronize()
+    return d2.cpu().numpy()
+
+
+def _gpu_fresnel(api, u1, px, py, lam, z, inplace=False):
+    ny, nx = u1.shape
+    plan = api.cwo_plan(nx, ny, px, lam)
+    if px != py:
+        plan.set_pitch_xy(px, py)
+    d1 = _dev(u1)
+    d2 = d1 if inplace else torch.empty_like(d1)
+    api.cwo_fresnel_conv(plan, d1, d2, z)
+    torch.cuda.synchronize()
+    return d2.cpu().numpy()
+
+
+# ---------------------------------------------------------------- ASM -----------------------------------------
+
+@pytest.mark.parametrize("n", [32, 64, 128, 256, 512, 1024, 2048])
+def test_asm_square_sizes(api, oracle, n):
+    cfg = W.CONFIGS["c3"].scaled(n)
+    u1 = W.make_field(cfg)
+    for z in (0.01, -0.037):
+        _assert_parity(_gpu_asm(api, u1, cfg.pitch, cfg.pitch, cfg.lam, z), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, z),
+                       "asm %d z=%g" % (n, z))
+
+
+@pytest.mark.parametrize("shape", [(32, 1024), (2048, 64), (256, 4096), (8192, 32), (32, 16384), (16384, 32)])
+def test_asm_non_square_and_unequal_pitch(api, oracle, shape):
+    u1 = _rand(shape, 3)
+    px, py, lam, z = 3e-6, 5e-6, 633e-9, 0.004
+    _assert_parity(_gpu_asm(api, u1, px, py, lam, z), oracle.asm(u1, px, py, lam, z), "asm %s" % (shape,))
+
+
+def test_asm_c1_full(api, oracle):
+    cfg = W.CONFIGS["c1"]
+    u1 = W.make_field(cfg)
+    _assert_parity(_gpu_asm(api, u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0]),
+                   oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0]), "c1")
+
+
+def test_asm_c3_full_all_distances(api, oracle):
+    cfg = W.CONFIGS["c3"]
+    u1 = W.make_field(cfg)
+    plan = api.cwo_plan(cfg.N, cfg.N, cfg.pitch, cfg.lam)
+    d1 = _dev(u1); d2 = torch.empty_like(d1)
+    for z in cfg.zs:
+        api.cwo_asm(plan, d1, d2, z)
+        torch.cuda.synchronize()
+        _assert_parity(d2.cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, z), "c3 z=%g" % z)
+
+
+def test_asm_8192(api, oracle):
+    u1 = W.make_field(W.CONFIGS["c3"].scaled(8192))
+    _assert_parity(_gpu_asm(api, u1, 4e-6, 4e-6, 633e-9, 0.1), oracle.asm(u1, 4e-6, 4e-6, 633e-9, 0.1), "asm 8192")
+
+
+def test_asm_z0_identity_inplace_and_roundtrip(api):
+    u1 = _rand((512, 512), 5)
+    out = _gpu_asm(api, u1, 4e-6, 4e-6, 633e-9, 0.0, inplace=True)
+    _assert_parity(out, u1.astype(np.complex128), "z=0")
+    fwd = _gpu_asm(api, u1, 4e-6, 4e-6, 633e-9, 0.02)
+    back = _gpu_asm(api, fwd, 4e-6, 4e-6, 633e-9, -0.02)
+    _assert_parity(back, u1.astype(np.complex128), "round trip")
+    assert abs(np.linalg.norm(fwd.astype(np.complex128)) / np.linalg.norm(u1.astype(np.complex128)) - 1) < 1e-5
+
+
+def test_asm_evanescent_classification(api, oracle):
+    # pitch < lambda/sqrt(2): a large share of the bins is evanescent; one misclassified bin costs ~1/N
+    n, d, lam = 64, 0.3e-6, 633e-9
+    u1 = _rand((n, n), 7)
+    for z in (5e-6, -5e-6):
+        _assert_parity(_gpu_asm(api, u1, d, d, lam, z), oracle.asm(u1, d, d, lam, z), "evanescent z=%g" % z)
+    jy, jx = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+    pw = np.exp(2j * np.pi * (25 * jx + 20 * jy) / n).astype(np.complex64)      # f0 > 1/lambda
+    assert np.max(np.abs(_gpu_asm(api, pw, d, d, lam, 5e-6))) < 1e-4
+
+
+# ---------------------------------------------------------------- Fresnel ---------------------------------------
+
+@pytest.mark.parametrize("n", [16, 32, 64, 128, 256, 512])
+def test_fresnel_square_sizes(api, oracle, n):
+    cfg = W.CONFIGS["c2"].scaled(n)
+    u1 = _rand((n, n), n)
+    z = cfg.zs[0] * n / 1024                      # keeps N pitch^2/(lambda z) as in c2
+    for zz in (z, -z):
+        _assert_parity(_gpu_fresnel(api, u1, cfg.pitch, cfg.pitch, cfg.lam, zz),
+                       oracle.fresnel_conv(u1, cfg.pitch, cfg.pitch, cfg.lam, zz), "fresnel %d z=%g" % (n, zz))
+
+
+@pytest.mark.parametrize("shape", [(16, 512), (1024, 32), (64, 2048)])
+def test_fresnel_non_square_and_unequal_pitch(api, oracle, shape):
+    u1 = _rand(shape, 11)
+    px, py, lam, z = 6e-6, 9e-6, 532e-9, 0.01
+    _assert_parity(_gpu_fresnel(api, u1, px, py, lam, z), oracle.fresnel_conv(u1, px, py, lam, z), "fresnel %s" % (shape,))
+
+
+def test_fresnel_c2_full_and_inplace(api, oracle):
+    cfg = W.CONFIGS["c2"]
+    u1 = W.make_field(cfg)
+    ref = oracle.fresnel_conv(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0])
+    _assert_parity(_gpu_fresnel(api, u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0]), ref, "c2")
+    _assert_parity(_gpu_fresnel(api, u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0], inplace=True), ref, "c2 in place")
+
+
+def test_fresnel_2048_and_4096(api, oracle):
+    for n in (2048, 4096):
+        u1 = W.make_field(W.CONFIGS["c2"].scaled(n))
+        got = _gpu_fresnel(api, u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024)
+        if n == 2048:
+            _assert_parity(got, oracle.fresnel_conv(u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024), "fresnel 2048")
+        else:       # sampled outputs: direct sum of Eq.(1) per point
+            r = np.random.default_rng(1)
+            ms = r.integers(0, n, 24); ns = r.integers(0, n, 24)
+            ref = oracle.fresnel_points(u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024, ms, ns)
+            peak = np.abs(ref).max()
+            err = np.abs(got[ns, ms] - ref)
+            assert np.linalg.norm(err) / np.linalg.norm(ref) <= REL_L2 and err.max() <= MAX_ABS * peak
+
+
+def test_fresnel_c5_size_sampled(api, oracle):
+    # 8192^2 -> virtual 16384^2: spot-check against the direct sum (the oracle's plain definition)
+    cfg = W.CONFIGS["c5"]
+    n = cfg.N
+    r = np.random.default_rng(2)
+    u1 = W.random_phasor(cfg)
+    got = _gpu_fresnel(api, u1, cfg.pitch, cfg.pitch, cfg.lam, -cfg.zs[0])
+    ms = np.concatenate([[0, n - 1, 0, n - 1], r.integers(0, n, 8)])
+    ns = np.concatenate([[0, n - 1, n - 1, 0], r.integers(0, n, 8)])
+    ref = oracle.fresnel_points(u1, cfg.pitch, cfg.pitch, cfg.lam, -cfg.zs[0], ms, ns)
+    err = np.abs(got[ns, ms] - ref)
+    assert np.linalg.norm(err) / np.linalg.norm(ref) <= REL_L2, (err, np.abs(ref))
+
+
+# ---------------------------------------------------------------- stack ---------------------------------------
+
+def test_stack_small_full(api, oracle):
+    cfg = W.CONFIGS["c4"].scaled(256)
+    u1 = W.make_field(cfg)
+    zs = [0.001, 0.002, 0.0035, -0.001, 0.064]
+    plan = api.cwo_plan(cfg.N, cfg.N, cfg.pitch, cfg.lam)
+    out = torch.empty((len(zs), cfg.N, cfg.N), dtype=torch.complex64, device="cuda")
+    api.cwo_propagate_stack(plan, _dev(u1), zs, out)
+    torch.cuda.synchronize()
+    ref = oracle.stack(u1, cfg.pitch, cfg.pitch, cfg.lam, zs)
+    for k in range(len(zs)):
+        _assert_parity(out[k].cpu().numpy(), ref[k], "stack plane %d" % k)
+
+
+def test_stack_c4_full_size_sampled_planes(api, oracle):
+    cfg = W.CONFIGS["c4"]
+    u1 = W.make_field(cfg)
+    plan = api.cwo_plan(cfg.N, cfg.N, cfg.pitch, cfg.lam)
+    out = torch.empty((len(cfg.zs), cfg.N, cfg.N), dtype=torch.complex64, device="cuda")
+    api.cwo_propagate_stack(plan, _dev(u1), cfg.zs, out)
+    torch.cuda.synchronize()
+    for k in (0, 17, 63):
+        _assert_parity(out[k].cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[k]), "c4 plane %d" % k)
+    # every plane carries the input's energy (unitary H, no evanescent bins)
+    e = torch.linalg.vector_norm(out.reshape(len(cfg.zs), -1), dim=1).cpu().numpy()
+    assert np.allclose(e, np.linalg.norm(u1.astype(np.complex128)), rtol=1e-5)
+
+
+# ---------------------------------------------------------------- GS ------------------------------------------
+
+def _gs_gpu(api, method, amp_src, amp_dst, phi, pitch, lam, z, iters):
+    n = amp_src.shape[0]
+    plan = api.cwo_plan(n, n, pitch, lam)
+    plan.set_option(api.CWO_OPT_GS_METHOD, method)
+    ph = _dev(phi.astype(np.float32))
+    api.cwo_gs(plan, _dev(amp_src), _dev(amp_dst), z, iters, ph)
+    torch.cuda.synchronize()
+    return ph.cpu().numpy()
+
+
+def _phasor_rel_l2(theta_gpu, p_ref):
+    return np.linalg.norm(np.exp(1j * theta_gpu.astype(np.float64)) - p_ref) / np.linalg.norm(p_ref)
+
+
+@pytest.mark.parametrize("method", [0, 1])
+@pytest.mark.parametrize("n", [128, 512])
+def test_gs_kinoform_and_restart_parity(api, oracle, method, n):
+    cfg = W.CONFIGS["c5"].scaled(n)
+    z = cfg.zs[0] * n / 8192                           # N pitch^2/(lambda z) = 0.718 as in c5
+    amp_src, amp_dst, phi0 = W.gs_inputs_c5(cfg)
+    # iters = 0: the kinoform (section 7.1)
+    th = _gs_gpu(api, method, amp_src, amp_dst, phi0, cfg.pitch, cfg.lam, z, 0)
+    p = oracle.gs_init(method, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z)
+    assert _phasor_rel_l2(th, p) <= REL_L2
+    assert th.min() >= -np.pi - 1e-6 and th.max() <= np.pi + 1e-6
+    # restart parity along the oracle's trajectory: from the image-plane phase of
+    # iteration t, one init + one loop pass on both sides
+    for t in range(6):
+        p, G = oracle.gs_iter(method, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z, want_G=True)
+        if t in (0, 1, 5):
+            phi_t = np.angle(G).astype(np.float32)
+            th = _gs_gpu(api, method, amp_src, amp_dst, phi_t, cfg.pitch, cfg.lam, z, 1)
+            pr = oracle.gs_init(method, amp_dst, phi_t, cfg.pitch, cfg.pitch, cfg.lam, z)
+            pr = oracle.gs_iter(method, amp_src, amp_dst, pr, cfg.pitch, cfg.pitch, cfg.lam, z)
+            assert _phasor_rel_l2(th, pr) <= REL_L2, "restart at t=%d" % t
+
+
+def test_gs_error_curve_matches_oracle(api, oracle):
+    # eps_t from the GPU trajectory equals the oracle's to <= 1e-5 at every t
+    n = 256
+    cfg = W.CONFIGS["c5"].scaled(n)
+    z = cfg.zs[0] * n / 8192
+    amp_src, amp_dst, phi0 = W.gs_inputs_c5(cfg)
+    p = oracle.gs_init(0, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z)
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    errs = []
+    for t in range(8):
+        e_ref = oracle.gs_error(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z)
+        th = _gs_gpu(api, 0, amp_src, amp_dst, phi0, cfg.pitch, cfg.lam, z, t)
+        field = _dev((amp_src * np.exp(1j * th.astype(np.float64))).astype(np.complex64))
+        rec = torch.empty_like(field)
+        api.cwo_fresnel_conv(plan, field, rec, z)
+        e_gpu = float(torch.linalg.vector_norm(rec.abs() - _dev(amp_dst)) / torch.linalg.vector_norm(_dev(amp_dst)))
+        assert abs(e_gpu - e_ref) <= 1e-5, (t, e_gpu, e_ref)
+        errs.append(e_gpu)
+        p = oracle.gs_iter(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z)
+    assert errs[-1] < errs[0]
+
+
+def test_gs_c5_full_size(api, oracle):
+    # 8192^2, 20 iterations in the bench configuration: runs, stays finite and in range, improves the
+    # reconstruction; the kinoform step is spot-checked against the direct sum.
+    cfg = W.CONFIGS["c5"]
+    n, z = cfg.N, cfg.zs[0]
+    amp_src, amp_dst, phi0 = W.gs_inputs_c5(cfg)
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    d_src, d_dst = _dev(amp_src), _dev(amp_dst)
+
+    def recon_error(theta):
+        field = torch.polar(d_src, theta)
+        rec = torch.empty_like(field)
+        api.cwo_fresnel_conv(plan, field, rec, z)
+        return float(torch.linalg.vector_norm(rec.abs() - d_dst) / torch.linalg.vector_norm(d_dst))
+
+    th0 = _dev(phi0.copy())
+    api.cwo_gs(plan, d_src, d_dst, z, 0, th0)
+    torch.cuda.synchronize()
+    r = np.random.default_rng(3)
+    ms = r.integers(0, n, 6); ns = r.integers(0, n, 6)
+    G0 = (amp_dst.astype(np.float64) * np.exp(1j * phi0.astype(np.float64)))
+    ref = oracle.fresnel_points(G0, cfg.pitch, cfg.pitch, cfg.lam, -z, ms, ns)
+    got = np.exp(1j * th0.cpu().numpy()[ns, ms].astype(np.float64))
+    assert np.max(np.abs(got - ref / np.abs(ref))) < 2e-4
+    e0 = recon_error(th0)
+    th = _dev(phi0.copy())
+    api.cwo_gs(plan, d_src, d_dst, z, cfg.iters, th)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(th).all()) and float(th.abs().max()) <= np.pi + 1e-6
+    assert recon_error(th) < e0
+
+
+# ---------------------------------------------------------------- boundary -------------------------------------
+
+def test_error_codes(api):
+    plan = api.cwo_plan(64, 64, 1e-5, 633e-9)
+    u = torch.zeros((64, 64), dtype=torch.complex64, device="cuda")
+    with pytest.raises(api.CwoError) as e:
+        api.cwo_fresnel_conv(plan, u, u, 0.0)
+    assert e.value.code == api.CWO_EINVAL
+    L = api.lib()
+    assert L.cwo_asm(plan._h, u.data_ptr(), u.data_ptr(), 0.1) in (api.CWO_OK, api.CWO_EWORKSPACE)
+    plan2 = api.cwo_plan(64, 64, 1e-5, 633e-9)
+    assert L.cwo_asm(plan2._h, u.data_ptr(), u.data_ptr(), 0.1) == api.CWO_EWORKSPACE
+    assert L.cwo_asm(plan2._h, u.data_ptr() + 8, u.data_ptr(), 0.1) == api.CWO_EINVAL
+    assert L.cwo_asm(plan2._h, u.data_ptr(), u.data_ptr(), float("nan")) == api.CWO_EINVAL
+    with pytest.raises(api.CwoError):
+        api.cwo_plan(48, 64, 1e-5, 633e-9)
+    big = api.cwo_plan(16384, 32, 1e-5, 633e-9)
+    ub = torch.zeros((32, 16384), dtype=torch.complex64, device="cuda")
+    with pytest.raises(api.CwoError):
+        api.cwo_fresnel_conv(big, ub, ub, 0.1)      # 2*16384 exceeds the supported transform length
+    assert plan.launch_count >= 2
