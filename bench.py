@@ -1,0 +1,314 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of cwo-b200: propagations/s for the 4096^2 angular spectrum method.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+A step is one pass of the whole hot path (plan tables for a NEW z, row pass, fused column pass,
+inverse row pass) over one 4096 x 4096 complex64 field of BASELINE.json config c3; z cycles through
+{0.01, 0.1, 0.5} m so every step is the paper's "re-calculation" case.  Prints ONE JSON line.
+
+  value      whole-job propagations/s, inputs resident in HBM, CUDA events on the launching stream
+  e2e        same metric through the public binding with HOST (pinned) buffers: H2D of u1 and D2H of
+             u2 inside the timed region
+  roofline   the dominant kernel (fused column pass): algorithmic 16*N^2 bytes per launch / its
+             average duration from CUDA events recorded by the library (CWO_OPT_TIMING)
+  cpu_baseline  the fp64 oracle as it stands on the host cores (reported baseline, not the target)
+
+--impl reference times the oracle itself (this tier has no installable reference implementation).
+N > 1: the path does not shard (replicas only) -- every rank propagates its own field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "propagations/sec (4096^2 ASM, new z per call); effective HBM GB/s for 48*N^2 algorithmic bytes"
+UNIT = "propagations/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json's "~8 TB/s peak" (the target's denominator)
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def _peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def _ncu_traffic(kernel_key: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
+    try:
+        for line in open(p):
+            t = [x.strip() for x in line.split(",")]
+            if t and t[0] == kernel_key:
+                return float(t[1]) + float(t[2])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+                for nme, v in zip(names, r[2:6]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nme)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def _dist():
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ------------------------------------------------------------------------------------------------------
+# oracle arm (--impl reference) and the cpu_baseline leg: the ONLY places that touch oracle/
+# ------------------------------------------------------------------------------------------------------
+
+def _oracle_time_props(cfg, n_props: int, size: int):
+    """Seconds for n_props oracle ASM propagations of a size x size field (same pitch/lambda/z cycle)."""
+    from oracle import oracle as O
+    from paper_1107_5578_b200 import workloads as W
+    threads = O.max_threads()
+    O.set_threads(threads)
+    u1 = W.make_field(cfg.scaled(size) if size != cfg.N else cfg)
+    t0 = time.perf_counter()
+    for i in range(n_props):
+        O.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[i % len(cfg.zs)])
+    return time.perf_counter() - t0, threads
+
+
+def cpu_baseline(cfg, budget_s: float = 20.0):
+    """The oracle as it stands, on a bounded sample: whole 4096^2 propagations while they fit the budget."""
+    t1, threads = _oracle_time_props(cfg, 1, cfg.N)
+    n = int(max(1, min(8, budget_s // max(t1, 1e-3))))
+    t, _ = _oracle_time_props(cfg, n, cfg.N)
+    return {"value": n / t, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d full %dx%d fp64 oracle propagation(s), %d OpenMP threads, %.2f s" % (n, cfg.N, cfg.N, threads, t)}
+
+
+def run_reference(args):
+    rank, world, _ = _dist()
+    if rank != 0:
+        return
+    from paper_1107_5578_b200 import workloads as W
+    cfg = W.CONFIGS["c3"]
+    t_full, threads = _oracle_time_props(cfg, 1, cfg.N)
+    total = args.steps + args.warmup
+    size, scale = cfg.N, 1.0
+    while size > 512 and t_full * scale * total > 150.0:     # keep the whole run within a few minutes
+        size //= 2
+        scale = (size * size * np.log2(size)) / (cfg.N * cfg.N * np.log2(cfg.N))
+    _oracle_time_props(cfg, args.warmup, size)
+    t, _ = _oracle_time_props(cfg, args.steps, size)
+    value = args.steps / t * scale                            # 4096^2-equivalent propagations/s
+    sample = ("each step = one fp64 oracle ASM propagation of %dx%d (same pitch/lambda/z cycle)%s, %d threads"
+              % (size, size, "" if size == cfg.N else "; value scaled by N^2 log2 N to 4096^2", threads))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "c3: ASM 4096x4096 complex field, lambda 633 nm, pitch 4 um, z cycling {0.01,0.1,0.5} m"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------------
+
+def run_cuda(args):
+    import torch
+    from paper_1107_5578_b200 import api, workloads as W
+
+    rank, world, local = _dist()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    use_dist = world > 1
+    if use_dist:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = W.CONFIGS["c3"]
+    N, zs = cfg.N, cfg.zs
+    NBUF = 3
+    # three independent seeded fields (one per z) so successive steps never re-read the previous step's data
+    host_fields = []
+    for i in range(NBUF):
+        c = W.Config(cfg.name, cfg.op, cfg.N, cfg.lam, cfg.pitch, cfg.zs, index=cfg.index + 100 * (i + rank * NBUF))
+        host_fields.append(W.field_c3(c))
+    u1 = [torch.from_numpy(h).cuda() for h in host_fields]
+    u2 = [torch.empty_like(u1[0]) for _ in range(NBUF)]
+    plan = api.cwo_plan(N, N, cfg.pitch, cfg.lam)
+    plan.ensure_workspace(api.CWO_OP_ASM)
+    stream = torch.cuda.current_stream()
+
+    def step(i):
+        api.cwo_asm(plan, u1[i % NBUF], u2[i % NBUF], zs[i % len(zs)])
+
+    # ---- device-resident timing -----------------------------------------------------------------
+    for i in range(max(args.warmup, 3)):
+        step(i)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = plan.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for i in range(args.steps):
+        step(i)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = plan.launch_count - l0
+    clocks = sampler.stop() if rank == 0 else None
+    if use_dist:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = world * args.steps / (ms * 1e-3)
+
+    # ---- per-kernel durations (library-recorded CUDA events on the same stream) -------------------
+    plan.set_option(api.CWO_OPT_TIMING, 1)
+    reps = min(max(args.steps, 6), 60)
+    for i in range(reps):
+        step(i)
+    tm = plan.timings()
+    plan.set_option(api.CWO_OPT_TIMING, 0)
+    per_kind = {}
+    for tag, t_ms in tm:
+        per_kind.setdefault(tag & 15, []).append(t_ms)
+    names = {0: "pass_R (row FFT)", 2: "pass_C (fused column FFT*H*IFFT)", 1: "pass_R' (row IFFT)"}
+    passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
+    dom_kind = max(per_kind, key=lambda k: np.mean(per_kind[k]))
+    dom_ms = float(np.mean(per_kind[dom_kind]))
+    peak, peak_src = _peak()
+    alg_bytes = 16.0 * N * N                      # each pass reads 8 and writes 8 bytes per sample
+    achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
+    traffic = _ncu_traffic({0: "pass_R", 1: "pass_Rinv", 2: "pass_C"}[dom_kind])
+    roofline = {"bound": "hbm", "kernel": names[dom_kind], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms,
+                "pass_ms": passes, "step_share": dom_ms / sum(passes.values())}
+
+    # ---- end to end: host (pinned) buffers, H2D + propagate + D2H every step -----------------------
+    pin_in = [torch.from_numpy(h).pin_memory() for h in host_fields]
+    pin_out = torch.empty((N, N), dtype=torch.complex64).pin_memory()
+    d_in, d_out = torch.empty_like(u1[0]), torch.empty_like(u1[0])
+
+    def e2e_step(i):
+        d_in.copy_(pin_in[i % NBUF], non_blocking=True)
+        api.cwo_asm(plan, d_in, d_out, zs[i % len(zs)])
+        pin_out.copy_(d_out, non_blocking=True)
+
+    e2e_steps = max(3, min(args.steps, 20))
+    for i in range(3):
+        e2e_step(i)
+    barrier()
+    e0.record(stream)
+    for i in range(e2e_steps):
+        e2e_step(i)
+    e1.record(stream)
+    barrier()
+    ms_e2e = e0.elapsed_time(e1)
+    if use_dist:
+        t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t.item())
+    e2e = {"value": world * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT, "steps": e2e_steps,
+           "h2d_bytes_per_step": int(d_in.numel() * 8), "d2h_bytes_per_step": int(d_out.numel() * 8)}
+
+    if rank == 0:
+        ms_step = ms / args.steps
+        eff = 48.0 * N * N / (ms_step * 1e-3) / 1e9
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "c3: ASM 4096x4096 complex64 speckle field, lambda 633 nm, pitch 4 um, "
+                                       "z cycling {0.01,0.1,0.5} m (new z every call)",
+                           "l2": "working set 3 x 134 MB per step, rotating over 3 field pairs (> 126 MB L2); no flush",
+                           "parallelism": "replicas" if world > 1 else "single GPU",
+                           "bytes_per_propagation": 48 * N * N},
+                "effective_gbs": eff, "pct_of_8TBs": 100.0 * eff / NOMINAL_HBM_GBS, "pct_of_measured_copy": 100.0 * eff / peak,
+                "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(cfg)
+        print(json.dumps(line), flush=True)
+    if use_dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

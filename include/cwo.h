@@ -10,8 +10,8 @@
  *              Nx), 16-byte aligned.  Complex fields are interleaved (re, im) float pairs
  *              (8*Nx*Ny bytes); real fields are float (4*Nx*Ny bytes).
  *   Ownership  The caller owns every buffer, including the workspace.  A plan owns only small
- *              lookup tables (<= ~1.3 MiB) that it allocates with cudaMalloc at plan time or on the first call
- *              that needs them.  No call allocates or frees caller-visible memory.
+ *              lookup tables (a few MiB at most) that it allocates with cudaMalloc at plan time or on the
+ *              first call that needs them.  No call allocates or frees caller-visible memory.
  *   Asynchrony Every propagation call only enqueues kernels on the plan's stream and returns;
  *              results are valid once the caller has synchronised that stream.  No hidden
  *              host<->device copies of field data.  Host arrays (zs) are read before return.
@@ -51,8 +51,10 @@ enum {
 enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4 };
 
 enum {
-    CWO_OPT_GS_METHOD = 1   /* value: CWO_GS_FRESNEL (default; BASELINE config 5) or CWO_GS_ASM
+    CWO_OPT_GS_METHOD = 1,  /* value: CWO_GS_FRESNEL (default; BASELINE config 5) or CWO_GS_ASM
                                (the paper's Listing 8) */
+    CWO_OPT_TIMING = 2      /* value 1: bracket every pass kernel with a CUDA event pair on the plan's
+                               stream (read with cwo_plan_timings); 0 (default): off */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
 
@@ -112,6 +114,13 @@ int cwo_gs(cwo_plan_t plan, const float* amp_src, const float* amp_dst, double z
 
 const char* cwo_strerror(int code);
 int cwo_last_cuda_error(cwo_plan_t plan);
+
+/* With CWO_OPT_TIMING on: synchronises the plan's stream, writes the device time in ms of each pass
+ * kernel launched since the option was set / since the last call (at most cap entries; tag_out, if
+ * not NULL, receives log2(transform length)*16 + kind, kind 0 = forward, 1 = inverse, 2 = fused
+ * forward x H x inverse, 3 = H x inverse), clears the record and returns the number of launches
+ * recorded (may exceed cap), or a negative error. */
+int cwo_plan_timings(cwo_plan_t plan, float* ms_out, int* tag_out, int cap);
 
 /* Number of kernels the library has launched through this plan so far (bench accounting). */
 long long cwo_plan_launch_count(cwo_plan_t plan);

@@ -23,11 +23,13 @@ _LIB_PATH = os.path.join(_HERE, "libcwo.so")
 CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA = 0, -1, -2, -3, -4
 CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS = 1, 2, 3, 4
 CWO_OPT_GS_METHOD = 1
+CWO_OPT_TIMING = 2
 CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 
 EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",
            "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_asm", "cwo_fresnel_conv",
-           "cwo_propagate_stack", "cwo_gs", "cwo_strerror", "cwo_last_cuda_error", "cwo_plan_launch_count"]
+           "cwo_propagate_stack", "cwo_gs", "cwo_strerror", "cwo_last_cuda_error", "cwo_plan_launch_count",
+           "cwo_plan_timings"]
 
 _lib = None
 
@@ -68,6 +70,7 @@ def lib() -> ctypes.CDLL:
     L.cwo_last_cuda_error.argtypes = [vp]
     L.cwo_plan_launch_count.argtypes = [vp]
     L.cwo_plan_launch_count.restype = ctypes.c_longlong
+    L.cwo_plan_timings.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(I), I]
     _lib = L
     return L
 
@@ -112,6 +115,14 @@ class Plan:
 
     def bind_stream(self) -> None:
         self._check(lib().cwo_plan_set_stream(self._h, torch.cuda.current_stream().cuda_stream), "cwo_plan_set_stream")
+
+    def timings(self, cap: int = 4096):
+        """[(tag, ms), ...] of the pass kernels launched since CWO_OPT_TIMING was set / last read."""
+        ms = (ctypes.c_float * cap)(); tag = (ctypes.c_int * cap)()
+        n = lib().cwo_plan_timings(self._h, ms, tag, cap)
+        if n < 0:
+            self._check(n, "cwo_plan_timings")
+        return [(int(tag[i]), float(ms[i])) for i in range(min(n, cap))]
 
     @property
     def launch_count(self) -> int:

@@ -5,6 +5,7 @@
 #include <new>
 #include <stdint.h>
 #include <string.h>
+#include <vector>
 
 #include "../../include/cwo.h"
 #include "cwo_internal.h"
@@ -24,6 +25,13 @@ struct cwo_plan_s {
     double2* tw64[MAX_LOGN + 2];    // fp64 twiddles for the chirp FFT
     float2* chirp[2][2];            // [set][axis] Fresnel spectra Cx, Cy (set 0: +z, 1: the other sign in GS)
     double2* chirp_scratch;         // 2 axes x 2M
+    float* asm_tab;                 // ASM split path: per plane [theta_x (Mx) | theta_y (My)]
+    int asm_tab_planes;             // capacity of asm_tab in planes
+    // CWO_OPT_TIMING: one CUDA event pair around every pass kernel
+    int timing;
+    std::vector<cudaEvent_t>* ev;   // 2 per recorded launch
+    std::vector<int>* ev_tag;       // logn*16 + kind
+    size_t ev_used;
 };
 
 static int ilog2_exact(int v) {
@@ -49,8 +57,22 @@ static const pass_launcher_t kLaunchers[MAX_LOGN + 1] = {
     launch_pass_5, launch_pass_6, launch_pass_7, launch_pass_8, launch_pass_9,
     launch_pass_10, launch_pass_11, launch_pass_12, launch_pass_13, launch_pass_14};
 
-static int launch(cwo_plan_t p, int logn, int kind, int n_tiles, const PassParams& pp) {
-    CWO_CUDA(p, kLaunchers[logn](kind, n_tiles, p->stream, pp));
+static int launch(cwo_plan_t p, int logn, int kind, int pad, int mid, int n_tiles, const PassParams& pp) {
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (p->timing) {
+        while (p->ev->size() < 2 * (p->ev_used + 1)) {
+            cudaEvent_t e;
+            CWO_CUDA(p, cudaEventCreate(&e));
+            p->ev->push_back(e);
+        }
+        e0 = (*p->ev)[2 * p->ev_used]; e1 = (*p->ev)[2 * p->ev_used + 1];
+        if (p->ev_tag->size() <= p->ev_used) p->ev_tag->push_back(0);
+        (*p->ev_tag)[p->ev_used] = logn * 16 + kind;
+        p->ev_used++;
+        CWO_CUDA(p, cudaEventRecord(e0, p->stream));
+    }
+    CWO_CUDA(p, kLaunchers[logn](kind, pad, mid, n_tiles, p->stream, pp));
+    if (p->timing) CWO_CUDA(p, cudaEventRecord(e1, p->stream));
     p->launches++;
     return CWO_OK;
 }
@@ -86,6 +108,8 @@ extern "C" int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t*
     p->Nx = Nx; p->Ny = Ny; p->lognx = lx; p->logny = ly;
     p->px = p->py = pitch; p->lambda = lambda;
     p->gs_method = CWO_GS_FRESNEL;
+    p->ev = new std::vector<cudaEvent_t>();
+    p->ev_tag = new std::vector<int>();
     int rc = CWO_OK;
     if (lx >= MIN_LOGN) rc = ensure_twiddles(p, lx, false);
     if (rc == CWO_OK && ly >= MIN_LOGN) rc = ensure_twiddles(p, ly, false);
@@ -100,6 +124,9 @@ extern "C" int cwo_plan_destroy(cwo_plan_t p) {
     for (int i = 0; i < MAX_LOGN + 2; ++i) { cudaFree(p->tw[i]); cudaFree(p->tw64[i]); }
     for (int s = 0; s < 2; ++s) for (int a = 0; a < 2; ++a) cudaFree(p->chirp[s][a]);
     cudaFree(p->chirp_scratch);
+    cudaFree(p->asm_tab);
+    if (p->ev) { for (cudaEvent_t e : *p->ev) cudaEventDestroy(e); delete p->ev; }
+    delete p->ev_tag;
     delete p;
     return CWO_OK;
 }
@@ -120,6 +147,11 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
     if (!p) return CWO_EINVAL;
     if (key == CWO_OPT_GS_METHOD && (value == CWO_GS_FRESNEL || value == CWO_GS_ASM)) {
         p->gs_method = value;
+        return CWO_OK;
+    }
+    if (key == CWO_OPT_TIMING && (value == 0 || value == 1)) {
+        p->timing = value;
+        p->ev_used = 0;
         return CWO_OK;
     }
     return CWO_EINVAL;
@@ -165,60 +197,104 @@ extern "C" const char* cwo_strerror(int code) {
 }
 
 extern "C" int cwo_last_cuda_error(cwo_plan_t p) { return p ? p->last_cuda_error : 0; }
+
+extern "C" int cwo_plan_timings(cwo_plan_t p, float* ms_out, int* tag_out, int cap) {
+    if (!p || cap < 0 || (cap > 0 && !ms_out)) return CWO_EINVAL;
+    CWO_CUDA(p, cudaStreamSynchronize(p->stream));
+    const int n = (int)p->ev_used;
+    for (int i = 0; i < n && i < cap; ++i) {
+        CWO_CUDA(p, cudaEventElapsedTime(&ms_out[i], (*p->ev)[2 * i], (*p->ev)[2 * i + 1]));
+        if (tag_out) tag_out[i] = (*p->ev_tag)[i];
+    }
+    p->ev_used = 0;
+    return n;
+}
 extern "C" long long cwo_plan_launch_count(cwo_plan_t p) { return p ? p->launches : 0; }
 
-// ---- addressing of the three passes ---------------------------------------------------------
+// ---- geometry of a propagation ------------------------------------------------------------------
 
-static Addr addr_rowmajor_rows(int rb, int pitch) {
-    Addr a; a.tile_stride = (long long)rb * pitch; a.lane_stride = (unsigned)pitch;
-    a.sh = 0; a.hi_stride = 1; a.mask = 0; a.lo_stride = 0;
-    return a;
-}
-// column-tiled workspace T[x / Wc][y][x % Wc], ly rows kept; seen from a row pass (lanes = rows)
-static Addr addr_tiled_rows(int rb, int logwc, int ly) {
-    const int wc = 1 << logwc;
-    Addr a; a.tile_stride = (long long)rb * wc; a.lane_stride = (unsigned)wc;
-    a.sh = logwc; a.hi_stride = (unsigned)ly * wc; a.mask = wc - 1; a.lo_stride = 1;
-    return a;
-}
-// the same workspace seen from a column pass (lanes = columns of the tile, points = rows)
-static Addr addr_tiled_cols(int logwc, int ly) {
-    const int wc = 1 << logwc;
-    Addr a; a.tile_stride = (long long)ly * wc; a.lane_stride = 1;
-    a.sh = 0; a.hi_stride = (unsigned)wc; a.mask = 0; a.lo_stride = 0;
-    return a;
+enum { ROW_FWD = 0, ROW_INV = 1, COL_FWD = 2, COL_FUSED = 3, COL_MIDINV = 4 };   // == pass_kernel.cuh
+
+static int tile_logw_host(int logn) {   // == fft_core.cuh tile_logw
+    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn <= 13 ? 1 : 0;
 }
 
-// ---- one propagation = three passes ---------------------------------------------------------
+struct Geometry { int pad, logmx, logmy, mx, my, rb, logwc, wc; };
+
+static Geometry geometry(cwo_plan_t p, int method) {
+    Geometry g;
+    g.pad = (method == CWO_GS_ASM) ? 0 : 1;
+    g.logmx = p->lognx + g.pad; g.logmy = p->logny + g.pad;
+    g.mx = 1 << g.logmx; g.my = 1 << g.logmy;
+    g.rb = 1 << tile_logw_host(g.logmx);          // rows per row-pass tile
+    g.logwc = tile_logw_host(g.logmy); g.wc = 1 << g.logwc;   // columns per column-pass tile
+    return g;
+}
 
 struct PropIO {
     int in_mode; const float2* in; const float* in_amp; const float* in_phase;
     int out_mode; void* out; const float* out_amp;
 };
 
-struct Geometry { int logmx, logmy, mx, my, rb, logwc, wc; };
+// ---- transfer-function tables (S2) ----------------------------------------------------------------
 
-static Geometry geometry(cwo_plan_t p, int method) {
-    Geometry g;
-    const int pad = (method == CWO_GS_ASM) ? 0 : 1;
-    g.logmx = p->lognx + pad; g.logmy = p->logny + pad;
-    g.mx = 1 << g.logmx; g.my = 1 << g.logmy;
-    g.rb = 1 << tile_logw(g.logmx);
-    g.logwc = tile_logw(g.logmy); g.wc = 1 << g.logwc;
-    return g;
+// ASM: decide between the fp32 split-phase path and the per-sample fp64 path, and fill the Mid fields.
+// Split path requires: no evanescent bin (s_max well below 1) and a small non-paraxial residual for
+// every z of the call (fp32 evaluates it to ~1e-7 relative).
+static bool asm_split_ok(cwo_plan_t p, const Geometry& g, const double* zs, int n) {
+    const double fxm = 0.5 / p->px, fym = 0.5 / p->py;          // |f| <= Nyquist
+    const double smax = p->lambda * p->lambda * (fxm * fxm + fym * fym);
+    if (!(smax <= 0.5)) return false;
+    const double r = 1.0 + sqrt(1.0 - smax);
+    for (int i = 0; i < n; ++i)
+        if (fabs(zs[i]) / p->lambda * smax * smax / (2.0 * r * r) > 32.0) return false;
+    (void)g;
+    return true;
 }
 
-static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, PassParams& pp) {
-    pp.mid_mode = MID_ASM_F64;
-    pp.z = z;
-    pp.inv_lam2 = 1.0 / (p->lambda * p->lambda);
-    pp.df_lane = 1.0 / ((double)g.mx * p->px);
-    pp.df_point = 1.0 / ((double)g.my * p->py);
+static int ensure_asm_tab(cwo_plan_t p, const Geometry& g, int planes) {
+    if (p->asm_tab_planes >= planes) return CWO_OK;
+    if (p->asm_tab) { CWO_CUDA(p, cudaStreamSynchronize(p->stream)); cudaFree(p->asm_tab); p->asm_tab = nullptr; }
+    CWO_CUDA(p, cudaMalloc(&p->asm_tab, sizeof(float) * (size_t)planes * (g.mx + g.my)));
+    p->asm_tab_planes = planes;
+    return CWO_OK;
+}
+
+static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, int n) {
+    int rc = ensure_asm_tab(p, g, n);
+    if (rc != CWO_OK) return rc;
+    const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
+    for (int i0 = 0; i0 < n; i0 += ASM_PLANE_BATCH) {
+        AsmPlaneBatch b;
+        const int m = n - i0 < ASM_PLANE_BATCH ? n - i0 : ASM_PLANE_BATCH;
+        for (int i = 0; i < m; ++i) {
+            const double z = zs[i0 + i], kz = z / p->lambda;
+            b.p[i].c0 = kz - floor(kz);
+            b.p[i].ax = z * p->lambda * dfx * dfx * 0.5;
+            b.p[i].ay = z * p->lambda * dfy * dfy * 0.5;
+        }
+        CWO_CUDA(p, build_asm_phase_tables(p->asm_tab + (size_t)i0 * (g.mx + g.my), b, m, g.mx, g.my, p->stream));
+        p->launches++;
+    }
+    return CWO_OK;
+}
+
+static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, int plane, PassParams& pp) {
+    const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
     pp.n_lane_bins = g.mx;
-    pp.mid_scale = (float)(1.0 / ((double)g.mx * (double)g.my));
+    if (split) {
+        const float* t = p->asm_tab + (size_t)plane * (g.mx + g.my);
+        pp.tab_lane = (const float2*)t; pp.tab_point = (const float2*)(t + g.mx);
+        pp.res_a = (float)(p->lambda * p->lambda * dfx * dfx);
+        pp.res_b = (float)(p->lambda * p->lambda * dfy * dfy);
+        pp.res_c = (float)(z / p->lambda);
+    } else {
+        pp.z = z; pp.inv_lam2 = 1.0 / (p->lambda * p->lambda);
+        pp.df_lane = dfx; pp.df_point = dfy;
+    }
 }
 
-// Build Cx, Cy for distance z into table set `set` (S2/S7: coefficient and 1/(MxMy) folded in).
+// Fresnel: Cx, Cy for distance z into table set `set` (coefficient of Eq.(1) and 1/(MxMy) folded in).
 static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int set) {
     int rc;
     if ((rc = ensure_twiddles(p, g.logmx, true)) != CWO_OK) return rc;
@@ -243,44 +319,55 @@ static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int s
     ay.out = p->chirp[set][1]; ay.scratch = p->chirp_scratch + 2 * (size_t)g.mx; ay.tw64 = p->tw64[g.logmy]; ay.logm = g.logmy;
     ay.a_cycles = p->py * p->py / (2.0 * p->lambda * z);
     ay.coef = make_double2(rt, 0.0);
-    CWO_CUDA(p, build_chirp_spectrum(ax, &ay, p->stream));
+    CWO_CUDA(p, build_chirp_spectrum(ax, ay, p->stream));
     p->launches++;
     return CWO_OK;
 }
 
-// The three passes.  `ws` holds Ny rows x Mx columns in column-tile order.  For Fresnel the
-// tables of set `set` must already hold the spectra for this z.
-static int run_passes(cwo_plan_t p, int method, double z, int set, const PropIO& io, float2* ws) {
+// ---- the passes ---------------------------------------------------------------------------------------
+
+static void row_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
+    memset(&pp, 0, sizeof(pp));
+    pp.rows = p->Ny; pp.pitch = p->Nx; pp.ly = p->Ny; pp.logwc = g.logwc;
+    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f;
+}
+static void col_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
+    memset(&pp, 0, sizeof(pp));
+    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f;
+}
+
+static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float2* ws) {
+    PassParams pp; row_params(p, g, pp);
+    pp.in = io.in; pp.in_amp = io.in_amp; pp.in_phase = io.in_phase; pp.in_mode = io.in_mode; pp.out = ws;
+    return launch(p, g.logmx, ROW_FWD, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
+}
+static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const float2* ws, float scale) {
+    PassParams pp; row_params(p, g, pp);
+    pp.in = ws; pp.out = (float2*)io.out; pp.out_mode = io.out_mode; pp.out_amp = io.out_amp; pp.out_scale = scale;
+    return launch(p, g.logmx, ROW_INV, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
+}
+
+// One propagation = pass R, pass C (fused), pass R'.  `ws` holds Ny rows x Mx columns in column-tile
+// order.  Fresnel: table set `set` must hold the spectra for this z.  ASM: tables (if split) at plane 0.
+static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, const PropIO& io, float2* ws) {
     const Geometry g = geometry(p, method);
     int rc;
     if ((rc = ensure_twiddles(p, g.logmx, false)) != CWO_OK) return rc;
     if ((rc = ensure_twiddles(p, g.logmy, false)) != CWO_OK) return rc;
-    PassParams pp;
-    // pass R: rows of u1 (zero padded to Mx) -> FFT -> ws
-    memset(&pp, 0, sizeof(pp));
-    pp.in = io.in; pp.in_amp = io.in_amp; pp.in_phase = io.in_phase; pp.in_mode = io.in_mode;
-    pp.out = ws; pp.out_mode = OUT_COMPLEX; pp.out_scale = 1.0f;
-    pp.ain = addr_rowmajor_rows(g.rb, p->Nx); pp.aout = addr_tiled_rows(g.rb, g.logwc, p->Ny);
-    pp.aux_pitch = p->Nx; pp.p_in_valid = p->Nx; pp.p_out_valid = g.mx; pp.lanes_total = p->Ny;
-    pp.tw = p->tw[g.logmx];
-    if ((rc = launch(p, g.logmx, KIND_FWD, (p->Ny + g.rb - 1) / g.rb, pp)) != CWO_OK) return rc;
-    // pass C: columns (Ny stored rows, zero padded to My) -> FFT -> x H -> IFFT -> first Ny rows, in place
-    memset(&pp, 0, sizeof(pp));
-    pp.in = ws; pp.out = ws; pp.in_mode = IN_COMPLEX; pp.out_mode = OUT_COMPLEX; pp.out_scale = 1.0f;
-    pp.ain = pp.aout = addr_tiled_cols(g.logwc, p->Ny);
-    pp.p_in_valid = p->Ny; pp.p_out_valid = p->Ny; pp.lanes_total = g.mx;
-    pp.tw = p->tw[g.logmy];
-    if (method == CWO_GS_ASM) fill_asm_mid(p, g, z, pp);
-    else { pp.mid_mode = MID_TABLES; pp.tab_lane = p->chirp[set][0]; pp.tab_point = p->chirp[set][1]; }
-    if ((rc = launch(p, g.logmy, KIND_FUSED, g.mx / g.wc, pp)) != CWO_OK) return rc;
-    // pass R': rows of ws -> IFFT -> first Nx columns -> u2 (with the GS constraint if asked)
-    memset(&pp, 0, sizeof(pp));
-    pp.in = ws; pp.in_mode = IN_COMPLEX;
-    pp.out = (float2*)io.out; pp.out_mode = io.out_mode; pp.out_amp = io.out_amp; pp.out_scale = 1.0f;
-    pp.ain = addr_tiled_rows(g.rb, g.logwc, p->Ny); pp.aout = addr_rowmajor_rows(g.rb, p->Nx);
-    pp.aux_pitch = p->Nx; pp.p_in_valid = g.mx; pp.p_out_valid = p->Nx; pp.lanes_total = p->Ny;
-    pp.tw = p->tw[g.logmx];
-    return launch(p, g.logmx, KIND_INV, (p->Ny + g.rb - 1) / g.rb, pp);
+    if ((rc = pass_row_fwd(p, g, io, ws)) != CWO_OK) return rc;
+    PassParams pp; col_params(p, g, pp);
+    pp.in = ws; pp.out = ws;
+    int mid;
+    float scale = 1.0f;
+    if (method == CWO_GS_ASM) {
+        mid = split ? MID_ASM_SPLIT : MID_ASM_F64;
+        fill_asm_mid(p, g, z, split, 0, pp);
+        scale = (float)(1.0 / ((double)g.mx * (double)g.my));       // 1/(MxMy) of the inverse FFT (reading R3)
+    } else {
+        mid = MID_TABLES; pp.tab_lane = p->chirp[set][0]; pp.tab_point = p->chirp[set][1]; pp.n_lane_bins = g.mx;
+    }
+    if ((rc = launch(p, g.logmy, COL_FUSED, g.pad, mid, g.mx / g.wc, pp)) != CWO_OK) return rc;
+    return pass_row_inv(p, g, io, ws, scale);
 }
 
 static bool aligned16(const void* q) { return q && !((uintptr_t)q & 15); }
@@ -288,8 +375,12 @@ static bool aligned16(const void* q) { return q && !((uintptr_t)q & 15); }
 extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || !asm_sizes_ok(p)) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_ASM, 0)) return CWO_EWORKSPACE;
+    const Geometry g = geometry(p, CWO_GS_ASM);
+    const bool split = asm_split_ok(p, g, &z, 1);
+    int rc;
+    if (split && (rc = build_asm_tables(p, g, &z, 1)) != CWO_OK) return rc;
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
-    return run_passes(p, CWO_GS_ASM, z, 0, io, (float2*)p->ws);
+    return run_passes(p, CWO_GS_ASM, z, 0, split, io, (float2*)p->ws);
 }
 
 extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
@@ -298,7 +389,7 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0);
     if (rc != CWO_OK) return rc;
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
-    return run_passes(p, CWO_GS_FRESNEL, z, 0, io, (float2*)p->ws);
+    return run_passes(p, CWO_GS_FRESNEL, z, 0, false, io, (float2*)p->ws);
 }
 
 extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double* zs, int n, cwo_c64* out) {
@@ -307,38 +398,25 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_STACK, n)) return CWO_EWORKSPACE;
     const Geometry g = geometry(p, CWO_GS_ASM);
     const size_t f = (size_t)p->Nx * p->Ny;
-    float2* A = (float2*)p->ws;
-    float2* B = A + f;
+    float2* A = (float2*)p->ws;       // FFT2[u1] in column-tile order, computed once (S9)
+    float2* B = A + f;                // one plane in flight between its column and row pass
     int rc;
-    PassParams pp;
-    // forward FFT2 of u1 once (S9): pass R, then a forward-only column pass in place
-    memset(&pp, 0, sizeof(pp));
-    pp.in = (const float2*)u1; pp.out = A; pp.out_scale = 1.0f;
-    pp.ain = addr_rowmajor_rows(g.rb, p->Nx); pp.aout = addr_tiled_rows(g.rb, g.logwc, p->Ny);
-    pp.aux_pitch = p->Nx; pp.p_in_valid = p->Nx; pp.p_out_valid = g.mx; pp.lanes_total = p->Ny;
-    pp.tw = p->tw[g.logmx];
-    if ((rc = launch(p, g.logmx, KIND_FWD, (p->Ny + g.rb - 1) / g.rb, pp)) != CWO_OK) return rc;
-    memset(&pp, 0, sizeof(pp));
-    pp.in = A; pp.out = A; pp.out_scale = 1.0f;
-    pp.ain = pp.aout = addr_tiled_cols(g.logwc, p->Ny);
-    pp.p_in_valid = p->Ny; pp.p_out_valid = p->Ny; pp.lanes_total = g.mx;
-    pp.tw = p->tw[g.logmy];
-    if ((rc = launch(p, g.logmy, KIND_FWD, g.mx / g.wc, pp)) != CWO_OK) return rc;
+    const bool split = asm_split_ok(p, g, zs, n);
+    if (split && (rc = build_asm_tables(p, g, zs, n)) != CWO_OK) return rc;
+    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, nullptr, nullptr};
+    if ((rc = pass_row_fwd(p, g, io, A)) != CWO_OK) return rc;
+    PassParams pp; col_params(p, g, pp);
+    pp.in = A; pp.out = A;
+    if ((rc = launch(p, g.logmy, COL_FWD, 0, MID_NONE, g.mx / g.wc, pp)) != CWO_OK) return rc;
+    const float scale = (float)(1.0 / ((double)g.mx * (double)g.my));
     for (int k = 0; k < n; ++k) {
-        // per plane: x H(z_k) and inverse column transform, then inverse row transform
-        memset(&pp, 0, sizeof(pp));
-        pp.in = A; pp.out = B; pp.out_scale = 1.0f;
-        pp.ain = pp.aout = addr_tiled_cols(g.logwc, p->Ny);
-        pp.p_in_valid = p->Ny; pp.p_out_valid = p->Ny; pp.lanes_total = g.mx;
-        pp.tw = p->tw[g.logmy];
-        fill_asm_mid(p, g, zs[k], pp);
-        if ((rc = launch(p, g.logmy, KIND_MIDINV, g.mx / g.wc, pp)) != CWO_OK) return rc;
-        memset(&pp, 0, sizeof(pp));
-        pp.in = B; pp.out = (float2*)out + (size_t)k * f; pp.out_scale = 1.0f;
-        pp.ain = addr_tiled_rows(g.rb, g.logwc, p->Ny); pp.aout = addr_rowmajor_rows(g.rb, p->Nx);
-        pp.aux_pitch = p->Nx; pp.p_in_valid = g.mx; pp.p_out_valid = p->Nx; pp.lanes_total = p->Ny;
-        pp.tw = p->tw[g.logmx];
-        if ((rc = launch(p, g.logmx, KIND_INV, (p->Ny + g.rb - 1) / g.rb, pp)) != CWO_OK) return rc;
+        col_params(p, g, pp);
+        pp.in = A; pp.out = B;
+        fill_asm_mid(p, g, zs[k], split, k, pp);
+        if ((rc = launch(p, g.logmy, COL_MIDINV, 0, split ? MID_ASM_SPLIT : MID_ASM_F64, g.mx / g.wc, pp)) != CWO_OK)
+            return rc;
+        io.out = (float2*)out + (size_t)k * f;
+        if ((rc = pass_row_inv(p, g, io, B, scale)) != CWO_OK) return rc;
     }
     return CWO_OK;
 }
@@ -353,25 +431,33 @@ extern "C" int cwo_gs(cwo_plan_t p, const float* amp_src, const float* amp_dst, 
     const size_t f = (size_t)p->Nx * p->Ny;
     float2* g = (float2*)p->ws;          // the constrained field between propagations (8 B/px)
     float2* ws = g + f;
+    const Geometry geo = geometry(p, method);
     int rc;
+    bool split = false;
     if (method == CWO_GS_FRESNEL) {      // set 0: P(-z), set 1: P(+z)
-        const Geometry geo = geometry(p, method);
         if ((rc = build_fresnel_tables(p, geo, -z, 0)) != CWO_OK) return rc;
         if (iters > 0 && (rc = build_fresnel_tables(p, geo, +z, 1)) != CWO_OK) return rc;
+    } else {
+        split = asm_split_ok(p, geo, &z, 1);
     }
+    // The ASM tables hold one z at a time (plane 0); they are rebuilt before each propagation (tiny kernel).
+    auto prop = [&](double zz, int set, const PropIO& io) -> int {
+        if (method == CWO_GS_ASM && split) { int r = build_asm_tables(p, geo, &zz, 1); if (r != CWO_OK) return r; }
+        return run_passes(p, method, zz, set, split, io, ws);
+    };
     // steps 1-2: G = amp_dst exp(i phi0); p = phasor(P(-z)[G]); the store already forms amp_src * p
     PropIO io = {IN_AMP_PHASE, nullptr, amp_dst, phase_out,
                  iters == 0 ? OUT_PHASE : OUT_PHASOR_AMP, iters == 0 ? (void*)phase_out : (void*)g, amp_src};
-    if ((rc = run_passes(p, method, -z, 0, io, ws)) != CWO_OK) return rc;
+    if ((rc = prop(-z, 0, io)) != CWO_OK) return rc;
     for (int t = 0; t < iters; ++t) {
         // G = P(+z)[amp_src p]; q = phasor(G); store amp_dst * q
         PropIO fwd = {IN_COMPLEX, g, nullptr, nullptr, OUT_PHASOR_AMP, g, amp_dst};
-        if ((rc = run_passes(p, method, +z, 1, fwd, ws)) != CWO_OK) return rc;
+        if ((rc = prop(+z, 1, fwd)) != CWO_OK) return rc;
         // p = phasor(P(-z)[amp_dst q]); store amp_src * p, or the phase after the last pass
         const bool last = (t == iters - 1);
         PropIO bwd = {IN_COMPLEX, g, nullptr, nullptr, last ? OUT_PHASE : OUT_PHASOR_AMP,
                       last ? (void*)phase_out : (void*)g, amp_src};
-        if ((rc = run_passes(p, method, -z, 0, bwd, ws)) != CWO_OK) return rc;
+        if ((rc = prop(-z, 0, bwd)) != CWO_OK) return rc;
     }
     return CWO_OK;
 }

@@ -1,16 +1,20 @@
 // fft_core.cuh -- register/shared-memory FFT building blocks (complex64, sm_100a).
 //
 // A CTA owns a tile of W independent length-n transforms ("lanes", n = 2^LOGN).  The work is cut
-// into units of 16 points: unit (u, w), u in [0, n/16), always holds the points u + e*(n/16),
-// e = 0..15, of lane w in registers.  A Stockham autosort stage of radix R (2,4,8,16) does 16/R
-// butterflies per unit on those registers, then the tile is exchanged through shared memory
-// ([point][lane], one pad row every 16 points => conflict-free 64-bit accesses for every stage).
-// n = R0 * 16^m with R0 in {1,2,4,8}: the small radix runs first (SMALL_FIRST) or last, so that
-// a forward transform ending in a radix-16 stage and an inverse one starting with a radix-16 stage
-// hold the same 16 points per unit and can be chained without an exchange (fused column pass).
-// Only the forward kernel exp(-i 2 pi jk/n) is implemented; inverse = conj . forward . conj.
+// into units of 16 points: unit (u, w), u in [0, n/16), holds the points u + e*(n/16), e = 0..15,
+// of lane w in registers.  A thread owns two units ("slots"): the same u in two adjacent lanes
+// (PAIR: twiddles are shared and shared-memory accesses are 128-bit), or, when the tile has a
+// single lane (n = 16384), units u and u + n/32.
+// A Stockham autosort stage of radix R (2,4,8,16) does 16/R butterflies per unit on those registers,
+// then the tile is exchanged through shared memory ([point][lane], one pad row every 16 points).
+// n = R0 * 16^m with R0 in {1,2,4,8}: the small radix runs first in a forward transform and last in
+// an inverse one, so that a forward transform (ending in a radix-16 stage) and the following inverse
+// one (starting with a radix-16 stage) hold the same 16 points per unit and chain without an
+// exchange (fused column pass).  The radix-16 stages run as ONE runtime loop so the code stays
+// small enough for the instruction cache.  Only the forward kernel exp(-i 2 pi jk/n) is
+// implemented; inverse = conj . forward . conj.
 //
-// Defines the transform of S4/S6 in SURVEY.md section 8(a) (paper: "FFT", "IFFT").
+// This is the transform of S4/S6 in SURVEY.md section 8(a) (paper: "FFT", "IFFT").
 #pragma once
 #include <cuda_runtime.h>
 
@@ -25,16 +29,14 @@ __device__ __forceinline__ float2 csqr(float2 a) {
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ float2 cconj(float2 a) { return make_float2(a.x, -a.y); }
-// a * (-i)
-__device__ __forceinline__ float2 cmul_mi(float2 a) { return make_float2(a.y, -a.x); }
+__device__ __forceinline__ float2 cmul_mi(float2 a) { return make_float2(a.y, -a.x); }   // a * (-i)
 
 #define CWO_C8 0.70710678118654752440f   // cos(pi/4)
 #define CWO_C16 0.92387953251128675613f  // cos(pi/8)
 #define CWO_S16 0.38268343236508977173f  // sin(pi/8)
 
-// ---- in-register DFTs on v[base + r*S], r = 0..R-1; forward kernel -------------------------
-// Output X_q lands at register base + perm<R>(q)*S.
-template <int R> __device__ __forceinline__ constexpr int perm(int q) {
+// ---- in-register DFTs on v[b + r*S], r = 0..R-1; forward kernel; X_q lands at b + perm<R>(q)*S ----
+template <int R> __host__ __device__ constexpr int perm(int q) {
     return R == 16 ? ((q & 3) * 4 + (q >> 2)) : R == 8 ? ((q >> 2) + 2 * (q & 3)) : q;
 }
 
@@ -44,8 +46,7 @@ template <int S> __device__ __forceinline__ void dft2(float2 (&v)[16], int b) {
     v[b + S] = csub(a0, a1);
 }
 
-// natural-order 4-point DFT on v[b], v[b+S], v[b+2S], v[b+3S]
-template <int S> __device__ __forceinline__ void dft4(float2 (&v)[16], int b) {
+template <int S> __device__ __forceinline__ void dft4(float2 (&v)[16], int b) {   // natural order
     float2 a = cadd(v[b], v[b + 2 * S]), c = csub(v[b], v[b + 2 * S]);
     float2 e = cadd(v[b + S], v[b + 3 * S]), d = cmul_mi(csub(v[b + S], v[b + 3 * S]));
     v[b] = cadd(a, e);
@@ -58,31 +59,28 @@ template <int S> __device__ __forceinline__ void dft4(float2 (&v)[16], int b) {
 template <int S> __device__ __forceinline__ void dft8(float2 (&v)[16], int b) {
     dft4<2 * S>(v, b);
     dft4<2 * S>(v, b + S);
-    // r1 = 1: registers b + (1 + 2 q2) S, q2 = 1,2,3
-    {
-        float2 t = v[b + 3 * S];
-        v[b + 3 * S] = make_float2(CWO_C8 * (t.x + t.y), CWO_C8 * (t.y - t.x));   // * (c8, -c8)
-        v[b + 5 * S] = cmul_mi(v[b + 5 * S]);
-        t = v[b + 7 * S];
-        v[b + 7 * S] = make_float2(CWO_C8 * (t.y - t.x), -CWO_C8 * (t.x + t.y));  // * (-c8, -c8)
-    }
+    float2 t = v[b + 3 * S];
+    v[b + 3 * S] = make_float2(CWO_C8 * (t.x + t.y), CWO_C8 * (t.y - t.x));   // * (c8, -c8)
+    v[b + 5 * S] = cmul_mi(v[b + 5 * S]);
+    t = v[b + 7 * S];
+    v[b + 7 * S] = make_float2(CWO_C8 * (t.y - t.x), -CWO_C8 * (t.x + t.y));  // * (-c8, -c8)
 #pragma unroll
     for (int q2 = 0; q2 < 4; ++q2) dft2<S>(v, b + 2 * q2 * S);
 }
 
-// 16 = 4 x 4 (S = 1 only): DFT4 over r2 (r = r1 + 4 r2), twiddle w16^(r1 q2), DFT4 over r1.
+// 16 = 4 x 4: DFT4 over r2 (r = r1 + 4 r2), twiddle w16^(r1 q2), DFT4 over r1.
 __device__ __forceinline__ void dft16(float2 (&v)[16]) {
 #pragma unroll
     for (int r1 = 0; r1 < 4; ++r1) dft4<4>(v, r1);
     // v[r1 + 4 q2] *= w16^(r1 q2), w16^m = (cos(pi m/8), -sin(pi m/8))
     v[5] = cmul(v[5], make_float2(CWO_C16, -CWO_S16));     // m = 1
-    v[6] = cmul(v[6], make_float2(CWO_C8, -CWO_C8));       // m = 2
+    v[6] = make_float2(CWO_C8 * (v[6].x + v[6].y), CWO_C8 * (v[6].y - v[6].x));     // m = 2
     v[7] = cmul(v[7], make_float2(CWO_S16, -CWO_C16));     // m = 3
-    v[9] = cmul(v[9], make_float2(CWO_C8, -CWO_C8));       // m = 2
+    v[9] = make_float2(CWO_C8 * (v[9].x + v[9].y), CWO_C8 * (v[9].y - v[9].x));     // m = 2
     v[10] = cmul_mi(v[10]);                                // m = 4
-    v[11] = cmul(v[11], make_float2(-CWO_C8, -CWO_C8));    // m = 6
+    v[11] = make_float2(CWO_C8 * (v[11].y - v[11].x), -CWO_C8 * (v[11].x + v[11].y));   // m = 6
     v[13] = cmul(v[13], make_float2(CWO_S16, -CWO_C16));   // m = 3
-    v[14] = cmul(v[14], make_float2(-CWO_C8, -CWO_C8));    // m = 6
+    v[14] = make_float2(CWO_C8 * (v[14].y - v[14].x), -CWO_C8 * (v[14].x + v[14].y));   // m = 6
     v[15] = cmul(v[15], make_float2(-CWO_C16, CWO_S16));   // m = 9
 #pragma unroll
     for (int q2 = 0; q2 < 4; ++q2) dft4<1>(v, 4 * q2);
@@ -95,116 +93,154 @@ template <int R> __device__ __forceinline__ void dftR(float2 (&v)[16], int b) {
     else dft2<8>(v, b);
 }
 
-// v[b + r*S] *= w1^r, r = 1..R-1.  Powers by squaring/multiplying (depth <= 4 products).
-template <int R> __device__ __forceinline__ void twiddle(float2 (&v)[16], int b, float2 w1) {
-    constexpr int S = 16 / R;
-    v[b + S] = cmul(v[b + S], w1);
-    if constexpr (R >= 4) {
-        float2 w2 = csqr(w1), w3 = cmul(w2, w1);
-        v[b + 2 * S] = cmul(v[b + 2 * S], w2);
-        v[b + 3 * S] = cmul(v[b + 3 * S], w3);
-        if constexpr (R >= 8) {
-            float2 w4 = csqr(w2), w5 = cmul(w4, w1), w6 = csqr(w3), w7 = cmul(w4, w3);
-            v[b + 4 * S] = cmul(v[b + 4 * S], w4);
-            v[b + 5 * S] = cmul(v[b + 5 * S], w5);
-            v[b + 6 * S] = cmul(v[b + 6 * S], w6);
-            v[b + 7 * S] = cmul(v[b + 7 * S], w7);
-            if constexpr (R >= 16) {
-                float2 w8 = csqr(w4);
-                v[b + 8 * S] = cmul(v[b + 8 * S], w8);
-                v[b + 9 * S] = cmul(v[b + 9 * S], cmul(w8, w1));
-                v[b + 10 * S] = cmul(v[b + 10 * S], csqr(w5));
-                v[b + 11 * S] = cmul(v[b + 11 * S], cmul(w8, w3));
-                v[b + 12 * S] = cmul(v[b + 12 * S], csqr(w6));
-                v[b + 13 * S] = cmul(v[b + 13 * S], cmul(w8, w5));
-                v[b + 14 * S] = cmul(v[b + 14 * S], csqr(w7));
-                v[b + 15 * S] = cmul(v[b + 15 * S], cmul(w8, w7));
-            }
-        }
+// Powers w^1 .. w^(R-1) by squaring/multiplying (depth <= 4 products).
+template <int R> __device__ __forceinline__ void powers(float2 w1, float2 (&w)[16]) {
+    w[1] = w1;
+    if constexpr (R >= 4) { w[2] = csqr(w1); w[3] = cmul(w[2], w1); }
+    if constexpr (R >= 8) { w[4] = csqr(w[2]); w[5] = cmul(w[4], w1); w[6] = csqr(w[3]); w[7] = cmul(w[4], w[3]); }
+    if constexpr (R >= 16) {
+        w[8] = csqr(w[4]); w[9] = cmul(w[8], w1); w[10] = csqr(w[5]); w[11] = cmul(w[8], w[3]);
+        w[12] = csqr(w[6]); w[13] = cmul(w[8], w[5]); w[14] = csqr(w[7]); w[15] = cmul(w[8], w[7]);
     }
 }
+
+// v[b + r*S] *= w[r], r = 1..R-1
+template <int R> __device__ __forceinline__ void apply_powers(float2 (&v)[16], int b, const float2 (&w)[16]) {
+    constexpr int S = 16 / R;
+#pragma unroll
+    for (int r = 1; r < R; ++r) v[b + r * S] = cmul(v[b + r * S], w[r]);
+}
+
+// register renaming after the last stage of a transform: register i + q*S <- X_q of butterfly i
+template <int R> __device__ __forceinline__ void unpermute(float2 (&v)[16]) {
+    constexpr int S = 16 / R;
+    float2 t[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) t[e] = v[e];
+#pragma unroll
+    for (int i = 0; i < S; ++i)
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[i + q * S] = t[i + perm<R>(q) * S];
+}
+
+// ---- tile configuration (one place: host sizing and kernels must agree) -----------------------
+constexpr int tile_logw(int logn) {
+    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn <= 13 ? 1 : 0;
+}
+template <int LOGN> struct Tile {
+    static constexpr int N = 1 << LOGN, Q = N / 16;
+    static constexpr int LOGW = tile_logw(LOGN), W = 1 << LOGW;
+    static constexpr bool PAIR = W >= 2;               // a thread's two slots are adjacent lanes
+    static constexpr int T = PAIR ? Q * (W / 2) : Q / 2;
+    static constexpr int MINB = LOGN <= 12 ? 2 : 1;
+    static constexpr int L0 = LOGN & 3, M = LOGN >> 2; // n = 2^L0 * 16^M
+    static constexpr size_t SMEM_BYTES = sizeof(float2) * (size_t)(N + N / 16) * W;
+};
 
 // shared-memory index of (point p, lane w): one pad row of W elements every 16 points
 template <int LOGW> __device__ __forceinline__ int sidx(int p, int w) { return ((p + (p >> 4)) << LOGW) + w; }
 
-template <int LOGN, int LOGW> struct TileShape {
-    static constexpr int N = 1 << LOGN, W = 1 << LOGW, Q = N / 16;
-    static constexpr int SMEM_ELEMS = (N + N / 16) * W;
-    static constexpr size_t SMEM_BYTES = sizeof(float2) * (size_t)SMEM_ELEMS;
-};
-
-// One Stockham stage (radix 2^LR, Ns = 2^LNS points already combined) on every unit of the thread.
-// FIRST: no preceding smem traffic to wait for.  LAST: results stay in registers in natural unit
-// order (register e <-> point u + e*Q); otherwise they are exchanged through smem and the thread
-// comes back holding the inputs of the next stage.
-template <int LOGN, int LOGW, int UPT, int LR, int LNS, bool LAST>
-__device__ __forceinline__ void stage(float2 (&v)[UPT][16], const int (&uu)[UPT], const int (&ww)[UPT],
-                                      float2* sm, const float2* __restrict__ tw) {
-    constexpr int R = 1 << LR, S = 16 / R, Q = (1 << LOGN) / 16, NS = 1 << LNS;
-#pragma unroll
-    for (int it = 0; it < UPT; ++it) {
+// Write the outputs of a radix-2^LR stage with Ns = 2^lns to shared memory in Stockham order and read
+// back the inputs of the next stage.  u[], w0: the thread's units (see top of file).
+template <int LOGN, int LR>
+__device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], int w0, int lns, float2* sm) {
+    using C = Tile<LOGN>;
+    constexpr int R = 1 << LR, S = 16 / R;
+    __syncthreads();                       // everyone has finished reading the previous contents
+    if constexpr (C::PAIR) {
 #pragma unroll
         for (int i = 0; i < S; ++i) {
-            if constexpr (LNS > 0) {
-                int j = uu[it] + i * Q;
-                int k = j & (NS - 1);
-                float2 w1 = __ldg(&tw[k << (LOGN - LNS - LR)]);
-                twiddle<R>(v[it], i, w1);
-            }
-            dftR<R>(v[it], i);
-        }
-    }
-    if constexpr (LAST) {
+            const int j = u[0] + i * C::Q;
+            const int j0 = ((j >> lns) << (lns + LR)) + (j & ((1 << lns) - 1));
 #pragma unroll
-        for (int it = 0; it < UPT; ++it) {
-            float2 t[16];
-#pragma unroll
-            for (int e = 0; e < 16; ++e) t[e] = v[it][e];
-#pragma unroll
-            for (int i = 0; i < S; ++i)
-#pragma unroll
-                for (int q = 0; q < R; ++q) v[it][i + q * S] = t[i + perm<R>(q) * S];
-        }
-    } else {
-        __syncthreads();   // everyone has finished reading the previous contents of sm
-#pragma unroll
-        for (int it = 0; it < UPT; ++it) {
-#pragma unroll
-            for (int i = 0; i < S; ++i) {
-                int j = uu[it] + i * Q;
-                int k = j & (NS - 1);
-                int j0 = ((j >> LNS) << (LNS + LR)) + k;
-#pragma unroll
-                for (int q = 0; q < R; ++q)
-                    sm[sidx<LOGW>(j0 + (q << LNS), ww[it])] = v[it][i + perm<R>(q) * S];
+            for (int q = 0; q < R; ++q) {
+                const float2 a = v[0][i + perm<R>(q) * S], b = v[1][i + perm<R>(q) * S];
+                *reinterpret_cast<float4*>(&sm[sidx<C::LOGW>(j0 + (q << lns), w0)]) = make_float4(a.x, a.y, b.x, b.y);
             }
         }
         __syncthreads();
 #pragma unroll
-        for (int it = 0; it < UPT; ++it)
+        for (int e = 0; e < 16; ++e) {
+            const float4 t = *reinterpret_cast<const float4*>(&sm[sidx<C::LOGW>(u[0] + e * C::Q, w0)]);
+            v[0][e] = make_float2(t.x, t.y);
+            v[1][e] = make_float2(t.z, t.w);
+        }
+    } else {
 #pragma unroll
-            for (int e = 0; e < 16; ++e) v[it][e] = sm[sidx<LOGW>(uu[it] + e * Q, ww[it])];
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+            for (int i = 0; i < S; ++i) {
+                const int j = u[s] + i * C::Q;
+                const int j0 = ((j >> lns) << (lns + LR)) + (j & ((1 << lns) - 1));
+#pragma unroll
+                for (int q = 0; q < R; ++q) sm[sidx<0>(j0 + (q << lns), 0)] = v[s][i + perm<R>(q) * S];
+            }
+        __syncthreads();
+#pragma unroll
+        for (int s = 0; s < 2; ++s)
+#pragma unroll
+            for (int e = 0; e < 16; ++e) v[s][e] = sm[sidx<0>(u[s] + e * C::Q, 0)];
     }
 }
 
-// Full forward transform of the tile held in registers (in: register e of unit u = point
-// u + e*Q; out: the same mapping in the frequency domain).
-template <int LOGN, int LOGW, int UPT, bool SMALL_FIRST>
-__device__ __forceinline__ void fft_tile(float2 (&v)[UPT][16], const int (&uu)[UPT], const int (&ww)[UPT],
-                                         float2* sm, const float2* __restrict__ tw) {
-    constexpr int L0 = LOGN & 3;        // log2 of the small radix (0 = none)
-    constexpr int M = LOGN >> 2;        // number of radix-16 stages
+// Twiddle (if lns > 0) and butterflies of one radix-2^LR stage on both slots.
+template <int LOGN, int LR>
+__device__ __forceinline__ void butterflies(float2 (&v)[2][16], const int (&u)[2], int lns,
+                                            const float2* __restrict__ tw) {
+    using C = Tile<LOGN>;
+    constexpr int R = 1 << LR, S = 16 / R;
+#pragma unroll
+    for (int i = 0; i < S; ++i) {
+        if (lns > 0) {
+            float2 w[16];
+            const int k0 = (u[0] + i * C::Q) & ((1 << lns) - 1);
+            powers<R>(__ldg(&tw[k0 << (LOGN - lns - LR)]), w);
+            apply_powers<R>(v[0], i, w);
+            if constexpr (!C::PAIR) {
+                const int k1 = (u[1] + i * C::Q) & ((1 << lns) - 1);
+                powers<R>(__ldg(&tw[k1 << (LOGN - lns - LR)]), w);
+            }
+            apply_powers<R>(v[1], i, w);
+        }
+        dftR<R>(v[0], i);
+        dftR<R>(v[1], i);
+    }
+}
+
+// Forward and/or inverse transform of the tile held in registers, with `mid` applied between them
+// (mid must also conjugate so that the second forward transform acts as an inverse one).
+// In / out: register e of unit u <-> point u + e*Q.
+template <int LOGN, bool HAS_FWD, bool HAS_INV, class Mid>
+__device__ __forceinline__ void transform(float2 (&v)[2][16], const int (&u)[2], int w0, float2* sm,
+                                          const float2* __restrict__ tw, Mid mid) {
+    using C = Tile<LOGN>;
+    constexpr int L0 = C::L0, M = C::M;
     static_assert(M >= 1, "n >= 16");
-    if constexpr (SMALL_FIRST) {
-        if constexpr (L0 > 0) stage<LOGN, LOGW, UPT, L0, 0, false>(v, uu, ww, sm, tw);
-        if constexpr (M >= 1) stage<LOGN, LOGW, UPT, 4, L0, M == 1>(v, uu, ww, sm, tw);
-        if constexpr (M >= 2) stage<LOGN, LOGW, UPT, 4, L0 + 4, M == 2>(v, uu, ww, sm, tw);
-        if constexpr (M >= 3) stage<LOGN, LOGW, UPT, 4, L0 + 8, M == 3>(v, uu, ww, sm, tw);
-    } else {
-        if constexpr (M >= 1) stage<LOGN, LOGW, UPT, 4, 0, (M == 1 && L0 == 0)>(v, uu, ww, sm, tw);
-        if constexpr (M >= 2) stage<LOGN, LOGW, UPT, 4, 4, (M == 2 && L0 == 0)>(v, uu, ww, sm, tw);
-        if constexpr (M >= 3) stage<LOGN, LOGW, UPT, 4, 8, (M == 3 && L0 == 0)>(v, uu, ww, sm, tw);
-        if constexpr (L0 > 0) stage<LOGN, LOGW, UPT, L0, 4 * M, true>(v, uu, ww, sm, tw);
+    if constexpr (HAS_FWD && L0 > 0) {                      // small radix first, no twiddles
+        butterflies<LOGN, L0>(v, u, 0, tw);
+        exchange<LOGN, L0>(v, u, w0, 0, sm);
+    }
+    constexpr int NST = (HAS_FWD ? M : 0) + (HAS_INV ? M : 0);
+#pragma unroll 1
+    for (int s = 0; s < NST; ++s) {
+        const bool inv_half = HAS_FWD ? (s >= M) : true;
+        const int sl = (HAS_FWD && inv_half) ? s - M : s;
+        const int lns = inv_half ? 4 * sl : L0 + 4 * sl;
+        butterflies<LOGN, 4>(v, u, lns, tw);
+        if (sl == M - 1) {
+            if (!inv_half) {                                 // end of the forward transform
+                unpermute<16>(v[0]); unpermute<16>(v[1]);
+                if constexpr (HAS_INV) mid(v);
+                continue;
+            }
+            if (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); break; }
+        }
+        exchange<LOGN, 4>(v, u, w0, lns, sm);
+    }
+    if constexpr (!HAS_FWD && HAS_INV) { /* mid (if any) was applied by the caller before the call */ }
+    if constexpr (HAS_INV && L0 > 0) {                      // small radix last
+        butterflies<LOGN, L0>(v, u, 4 * M, tw);
+        unpermute<(1 << L0)>(v[0]); unpermute<(1 << L0)>(v[1]);
     }
 }
 

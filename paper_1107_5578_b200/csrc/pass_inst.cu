@@ -9,7 +9,8 @@
 namespace cwo {
 #define CWO_CAT2(a, b) a##b
 #define CWO_CAT(a, b) CWO_CAT2(a, b)
-cudaError_t CWO_CAT(launch_pass_, CWO_LOGN)(int kind, int n_tiles, cudaStream_t s, const PassParams& p) {
-    return launch_pass_impl<CWO_LOGN>(kind, n_tiles, s, p);
+cudaError_t CWO_CAT(launch_pass_, CWO_LOGN)(int kind, int pad, int mid, int n_tiles, cudaStream_t s,
+                                            const PassParams& p) {
+    return launch_pass_impl<CWO_LOGN>(kind, pad, mid, n_tiles, s, p);
 }
 }  // namespace cwo

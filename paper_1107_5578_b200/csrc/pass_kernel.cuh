@@ -1,192 +1,349 @@
 // pass_kernel.cuh -- one streaming pass over the field: every CTA loads a tile of W lanes x n points,
-// transforms it on chip and stores it.  The three passes of a propagation
-// are instances of this kernel:
-//   KIND_FWD     load -> FFT -> store                         (row pass R; column pass of the stack)
-//   KIND_INV     load -> IFFT -> store                        (row pass R')
-//   KIND_FUSED   load -> FFT -> x H -> IFFT -> store          (column pass C: S4 second half, S5, S6 first half)
-//   KIND_MIDINV  load -> x H -> IFFT -> store                 (stack: column pass per plane, S9)
-// Zero padding (S3) and cropping (S8) are point-validity bounds of the load / store; the GS
-// constraints (S10) are load/store modes; H (S2) is produced in registers by mid().
+// transforms it on chip and stores it.  The passes of a propagation:
+//   ROW_FWD     rows of u1 (row-major)  -> FFT_x  -> workspace in column-tile order      (pass R)
+//   COL_FUSED   column tile of the workspace -> FFT_y -> x H -> IFFT_y -> same tile        (pass C)
+//   ROW_INV     rows of the workspace   -> IFFT_x -> u2 (row-major)                        (pass R')
+//   COL_FWD / COL_MIDINV   the two halves of pass C, for the depth stack (S9)
+// PAD (Fresnel): the transform length is twice the number of stored points; the zero half is never
+// loaded (S3) and the discarded half never stored (S8) -- the compiler prunes the butterflies that
+// only see zeros / only feed discarded outputs.  GS constraints (S10) are load/store modes of the
+// row passes.  H (S2) is produced in registers by the Mid functors.
+//
+// Workspace layout ("column-tile order"): T[x / Wc][y][x % Wc], y < Ny, Wc = lanes of the column
+// pass; a column pass reads and writes one contiguous Ny*Wc block.
 #pragma once
 #include "cwo_internal.h"
 #include "fft_core.cuh"
 
 namespace cwo {
 
-__device__ __forceinline__ size_t addr_of(const Addr& a, long long tile_off, int w, int p) {
-    return (size_t)tile_off + (size_t)w * a.lane_stride + (size_t)(p >> a.sh) * a.hi_stride +
-           (size_t)(p & a.mask) * a.lo_stride;
-}
+enum { ROW_FWD = 0, ROW_INV = 1, COL_FWD = 2, COL_FUSED = 3, COL_MIDINV = 4 };
 
-// Transfer-function multiply for one unit: register e holds point l = u + e*Q of lane k.
-// Computes v <- conj(v * m) so that the following forward transform acts as the inverse one.
-template <int LOGN>
-__device__ __forceinline__ void mid_unit(float2 (&v)[16], int u, int lane, const PassParams& P) {
-    constexpr int N = 1 << LOGN, Q = N / 16;
-    if (P.mid_mode == MID_TABLES) {
-        // Fresnel: FFT2 of the sampled separable chirp is the outer product Cx[k]*Cy[l]
-        float2 cx = __ldg(&P.tab_lane[lane]);
+struct MidNone {
+    __device__ __forceinline__ void operator()(float2 (&)[2][16]) const {}
+};
+
+// Fresnel: FFT2 of the sampled separable chirp is the outer product Cx[k]*Cy[l] (S2, S7 folded in)
+template <int LOGN> struct MidTables {
+    const PassParams& P; const int (&u)[2]; int lane0; float2* sm;
+    __device__ __forceinline__ void operator()(float2 (&v)[2][16]) const {
+        using C = Tile<LOGN>;
+        const float2 cx0 = __ldg(&P.tab_lane[lane0]);
+        const float2 cx1 = __ldg(&P.tab_lane[C::PAIR ? lane0 + 1 : lane0]);
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-            float2 m = cmul(cx, __ldg(&P.tab_point[u + e * Q]));
-            v[e] = cconj(cmul(v[e], m));
+            const float2 cy0 = __ldg(&P.tab_point[u[0] + e * C::Q]);
+            const float2 cy1 = C::PAIR ? cy0 : __ldg(&P.tab_point[u[1] + e * C::Q]);
+            v[0][e] = cconj(cmul(v[0][e], cmul(cx0, cy0)));
+            v[1][e] = cconj(cmul(v[1][e], cmul(cx1, cy1)));
         }
-    } else if (P.mid_mode == MID_ASM_F64) {
-        // Eq.(16) P:L203 with the phase in cycles evaluated in fp64:
-        // w = 1/lambda^2 - (fx^2 + fy^2) (same expression and rounding as the oracle's evanescent test)
-        int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
-        double fx = (double)ks * P.df_lane;
-        double fx2 = __dmul_rn(fx, fx);
+    }
+};
+
+// ASM, Eq.(16), phase in cycles = z/lambda - ax k^2 - ay l^2 - res(k,l):
+// constant + paraxial parts from fp64-built 1-D tables (theta_lane includes z/lambda), the small
+// non-paraxial residual res = (z/lambda) s^2 / (2 (1+sqrt(1-s))^2), s = lambda^2 (fx^2+fy^2), in fp32
+// (no cancellation).  Only used when the plan has verified that no bin is evanescent and res is small.
+template <int LOGN> struct MidAsmSplit {
+    const PassParams& P; const int (&u)[2]; int lane0; float2* sm;
+    __device__ __forceinline__ void operator()(float2 (&v)[2][16]) const {
+        using C = Tile<LOGN>;
+        const float* thl = reinterpret_cast<const float*>(P.tab_lane);
+        const float* thp = reinterpret_cast<const float*>(P.tab_point);
+        float thx[2], sx[2];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int lane = lane0 + (C::PAIR ? s : 0);
+            const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+            thx[s] = __ldg(&thl[lane]);
+            sx[s] = P.res_a * (float)ks * (float)ks;
+        }
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-            int l = u + e * Q;
-            int ls = (l < N / 2) ? l : l - N;
-            double fy = (double)ls * P.df_point;
-            double w = __dsub_rn(P.inv_lam2, __dadd_rn(fx2, __dmul_rn(fy, fy)));
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int l = u[C::PAIR ? 0 : s] + e * C::Q;
+                const int ls = (l < C::N / 2) ? l : l - C::N;
+                const float sv = fmaf(P.res_b * (float)ls, (float)ls, sx[s]);
+                const float om = 1.0f - sv;
+                const float r = 1.0f + om * rsqrtf(om);
+                const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
+                float ph = thx[s] + __ldg(&thp[l]) - res;
+                ph -= rintf(ph);
+                float sn, cs;
+                __sincosf(6.283185307179586f * ph, &sn, &cs);
+                v[s][e] = cconj(cmul(v[s][e], make_float2(cs, sn)));
+            }
+        }
+    }
+};
+
+// ASM with the phase evaluated in fp64 per sample (general path: evanescent bins, long distances).
+// w = 1/lambda^2 - (fx^2 + fy^2) uses the oracle's expression and rounding for the evanescent test.
+// H is staged through the (idle) tile buffer by a rolled loop to keep the code small.
+template <int LOGN> struct MidAsmF64 {
+    const PassParams& P; const int (&u)[2]; int lane0; float2* sm;
+    __device__ __forceinline__ void operator()(float2 (&v)[2][16]) const {
+        using C = Tile<LOGN>;
+        __syncthreads();                                   // tile buffer no longer being read
+        float2* mine = sm + threadIdx.x;
+#pragma unroll 1
+        for (int i = 0; i < 32; ++i) {
+            const int s = i & 1, e = i >> 1;
+            const int lane = lane0 + (C::PAIR ? s : 0);
+            const int l = u[C::PAIR ? 0 : s] + e * C::Q;
+            const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+            const int ls = (l < C::N / 2) ? l : l - C::N;
+            const double fx = (double)ks * P.df_lane, fy = (double)ls * P.df_point;
+            const double w = __dsub_rn(P.inv_lam2, __dadd_rn(__dmul_rn(fx, fx), __dmul_rn(fy, fy)));
             float2 m = make_float2(0.f, 0.f);
             if (w >= 0.0) {
                 double c = P.z * sqrt(w);
                 c -= rint(c);
-                float s, co;
-                sincospif(2.0f * (float)c, &s, &co);
-                m = make_float2(co * P.mid_scale, s * P.mid_scale);
+                float sn, cs;
+                sincospif(2.0f * (float)c, &sn, &cs);
+                m = make_float2(cs, sn);
             }
-            v[e] = cconj(cmul(v[e], m));
+            mine[i * C::T] = m;
         }
-    } else if (P.mid_mode == MID_ASM_SPLIT) {
-        // H = c0*Ex[k] * Ey[l] * exp(-i 2 pi res), res = (z/lambda) s^2 / (2 (1+sqrt(1-s))^2),
-        // s = lambda^2 (fx^2 + fy^2): constant and paraxial parts from fp64 1-D tables, the small
-        // non-paraxial residual in fp32 (no cancellation).  Only used when no bin is evanescent.
-        int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
-        float2 ex = __ldg(&P.tab_lane[lane]);
-        float sx = P.res_a * (float)ks * (float)ks;          // lambda^2 fx^2
 #pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            int l = u + e * Q;
-            int ls = (l < N / 2) ? l : l - N;
-            float s = fmaf(P.res_b * (float)ls, (float)ls, sx);
-            float r = 1.0f + sqrtf(1.0f - s);
-            float res = P.res_c * s * s / (2.0f * r * r);       // cycles
-            res -= rintf(res);
-            float sn, cs;
-            sincospif(-2.0f * res, &sn, &cs);
-            float2 m = cmul(cmul(ex, __ldg(&P.tab_point[l])), make_float2(cs, sn));
-            v[e] = cconj(cmul(v[e], m));
-        }
+        for (int e = 0; e < 16; ++e)
+#pragma unroll
+            for (int s = 0; s < 2; ++s) v[s][e] = cconj(cmul(v[s][e], mine[(2 * e + s) * C::T]));
     }
-}
+};
 
-template <int LOGN, int KIND>
-__global__ void __launch_bounds__(tile_threads(LOGN), tile_minblocks(LOGN))
+template <int LOGN, int MID> struct MidSelect;
+template <int LOGN> struct MidSelect<LOGN, MID_TABLES> { using type = MidTables<LOGN>; };
+template <int LOGN> struct MidSelect<LOGN, MID_ASM_SPLIT> { using type = MidAsmSplit<LOGN>; };
+template <int LOGN> struct MidSelect<LOGN, MID_ASM_F64> { using type = MidAsmF64<LOGN>; };
+
+// IOM: ROW_FWD -> InMode of the load, ROW_INV -> OutMode of the store, column passes -> 0.
+template <int LOGN, int KIND, bool PAD, int MID, int IOM>
+__global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB)
 pass_kernel(const __grid_constant__ PassParams P) {
-    constexpr int LOGW = tile_logw(LOGN), W = 1 << LOGW, T = tile_threads(LOGN), UPT = tile_upt(LOGN);
-    constexpr int N = 1 << LOGN, Q = N / 16;
+    using C = Tile<LOGN>;
+    constexpr int W = C::W, Q = C::Q;
+    constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
+    constexpr int NE = PAD ? 8 : 16;        // PAD: points >= n/2 are zero on load / dropped on store
     extern __shared__ float2 sm[];
 
     const int tile = blockIdx.x;
-    int uu[UPT], ww[UPT];
-    bool ok[UPT];
-#pragma unroll
-    for (int it = 0; it < UPT; ++it) {
-        int unit = threadIdx.x + it * T;
-        ww[it] = unit & (W - 1);
-        uu[it] = unit >> LOGW;
-        ok[it] = (tile * W + ww[it]) < P.lanes_total;
+    int u[2], w0;
+    if constexpr (C::PAIR) {
+        w0 = 2 * (threadIdx.x % (W / 2));
+        u[0] = u[1] = threadIdx.x / (W / 2);
+    } else {
+        w0 = 0;
+        u[0] = threadIdx.x; u[1] = threadIdx.x + Q / 2;
     }
+    const int lane0 = tile * W + w0;        // row (row pass) or column (column pass) of slot 0
+    float2 v[2][16];
 
-    float2 v[UPT][16];
-    // ---- load (zero padding = points >= p_in_valid) ------------------------------------------
-    {
-        const long long toff = (long long)tile * P.ain.tile_stride;
+    // ---- load -----------------------------------------------------------------------------------
+    if constexpr (KIND == ROW_FWD) {
+        // rows of a row-major field; slot s = row lane0 + s (PAIR) / same row, second unit (!PAIR)
+        if constexpr (IOM == IN_COMPLEX) {
 #pragma unroll
-        for (int it = 0; it < UPT; ++it) {
+            for (int s = 0; s < 2; ++s) {
+                const int row = lane0 + (C::PAIR ? s : 0);
+                const bool ok = row < P.rows;
+                const size_t base = (size_t)row * P.pitch + u[s];
+#pragma unroll
+                for (int e = 0; e < 16; ++e)
+                    v[s][e] = (e < NE && ok) ? P.in[base + e * Q] : make_float2(0.f, 0.f);
+            }
+        } else {
+            // GS step 1: amp * exp(i phase) (Listing 8 lines 3-5).  Accurate sincosf is bulky, so the
+            // samples are formed by a rolled loop and staged through the thread's own slots of the
+            // (still idle) tile buffer.
+            float2* mine = sm + threadIdx.x;
+#pragma unroll 1
+            for (int i = 0; i < 2 * NE; ++i) {
+                const int s = i & 1, e = i >> 1;
+                const int row = lane0 + (C::PAIR ? s : 0);
+                float2 x = make_float2(0.f, 0.f);
+                if (row < P.rows) {
+                    const size_t a = (size_t)row * P.pitch + (s ? u[1] : u[0]) + e * Q;
+                    float sn, cs;
+                    sincosf(P.in_phase[a], &sn, &cs);
+                    const float am = P.in_amp[a];
+                    x = make_float2(am * cs, am * sn);
+                }
+                mine[i * C::T] = x;
+            }
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int e = 0; e < 16; ++e) v[s][e] = (e < NE) ? mine[(2 * e + s) * C::T] : make_float2(0.f, 0.f);
+        }
+    } else if constexpr (KIND == ROW_INV) {
+        // rows of the column-tiled workspace
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int row = lane0 + (C::PAIR ? s : 0);
+            const bool ok = row < P.rows;
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
-                int p = uu[it] + e * Q;
-                float2 x = make_float2(0.f, 0.f);
-                if (ok[it] && p < P.p_in_valid) {
-                    if (P.in_mode == IN_COMPLEX) {
-                        x = P.in[addr_of(P.ain, toff, ww[it], p)];
-                    } else {   // GS step 1: amp * exp(i phase)  (Listing 8 lines 3-5)
-                        size_t a = (size_t)(tile * W + ww[it]) * P.aux_pitch + p;
-                        float s, c;
-                        sincosf(P.in_phase[a], &s, &c);
-                        float am = P.in_amp[a];
-                        x = make_float2(am * c, am * s);
-                    }
-                }
-                if constexpr (KIND == KIND_INV) x = cconj(x);
-                v[it][e] = x;
+                const int p = u[s] + e * Q;
+                const size_t a = ((size_t)(p >> P.logwc) * P.ly + row) * (1u << P.logwc) + (p & ((1 << P.logwc) - 1));
+                v[s][e] = ok ? cconj(P.in[a]) : make_float2(0.f, 0.f);
             }
+        }
+    } else {
+        // column tile: contiguous [ly][W] block; a PAIR thread reads both lanes with one 128-bit load
+        const float2* src = P.in + (size_t)tile * P.ly * W;
+        if constexpr (C::PAIR) {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                if (e < NE) {
+                    const float4 t = *reinterpret_cast<const float4*>(&src[(size_t)(u[0] + e * Q) * W + w0]);
+                    v[0][e] = make_float2(t.x, t.y); v[1][e] = make_float2(t.z, t.w);
+                } else {
+                    v[0][e] = v[1][e] = make_float2(0.f, 0.f);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int e = 0; e < 16; ++e)
+                    v[s][e] = (!PAD || u[s] + e * Q < C::N / 2) ? src[u[s] + e * Q] : make_float2(0.f, 0.f);
         }
     }
 
-    // ---- transform ---------------------------------------------------------------------------
-    if constexpr (KIND == KIND_FWD) {
-        fft_tile<LOGN, LOGW, UPT, true>(v, uu, ww, sm, P.tw);
-    } else if constexpr (KIND == KIND_INV) {
-        fft_tile<LOGN, LOGW, UPT, false>(v, uu, ww, sm, P.tw);
+    // ---- transform ------------------------------------------------------------------------------
+    if constexpr (KIND == ROW_FWD || KIND == COL_FWD) {
+        transform<LOGN, true, false>(v, u, w0, sm, P.tw, MidNone());
+    } else if constexpr (KIND == ROW_INV) {
+        transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone());
     } else {
-        if constexpr (KIND == KIND_FUSED) fft_tile<LOGN, LOGW, UPT, true>(v, uu, ww, sm, P.tw);
-#pragma unroll
-        for (int it = 0; it < UPT; ++it) mid_unit<LOGN>(v[it], uu[it], tile * W + ww[it], P);
-        fft_tile<LOGN, LOGW, UPT, false>(v, uu, ww, sm, P.tw);
+        typename MidSelect<LOGN, MID>::type mid{P, u, lane0, sm};
+        if constexpr (KIND == COL_FUSED) {
+            transform<LOGN, true, true>(v, u, w0, sm, P.tw, mid);
+        } else {
+            mid(v);
+            transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone());
+        }
     }
 
-    // ---- store (crop = points >= p_out_valid; conj completes the inverse transform) ----------
-    {
-        const long long toff = (long long)tile * P.aout.tile_stride;
-        const float sc = P.out_scale;
+    // ---- store (conj completes an inverse transform) -----------------------------------------------
+    if constexpr (KIND == ROW_FWD) {
 #pragma unroll
-        for (int it = 0; it < UPT; ++it) {
+        for (int s = 0; s < 2; ++s) {
+            const int row = lane0 + (C::PAIR ? s : 0);
+            if (row < P.rows) {
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                int p = uu[it] + e * Q;
-                if (!(ok[it] && p < P.p_out_valid)) continue;
-                float2 x = v[it][e];
-                if constexpr (KIND != KIND_FWD) x.y = -x.y;
-                if (P.out_mode == OUT_COMPLEX) {
-                    P.out[addr_of(P.aout, toff, ww[it], p)] = make_float2(x.x * sc, x.y * sc);
-                } else {
-                    size_t a = (size_t)(tile * W + ww[it]) * P.aux_pitch + p;
-                    if (P.out_mode == OUT_PHASOR_AMP) {
-                        // phase constraint then amplitude constraint (Listing 8 lines 11-13 / 15-16):
-                        // keep u/|u| (1 where u == 0), replace the amplitude by that of the next plane
-                        float m2 = x.x * x.x + x.y * x.y;
-                        float am = P.out_amp[a];
-                        float2 ph = make_float2(1.f, 0.f);
-                        if (m2 > 0.f) { float r = rsqrtf(m2); ph = make_float2(x.x * r, x.y * r); }
-                        P.out[addr_of(P.aout, toff, ww[it], p)] = make_float2(am * ph.x, am * ph.y);
-                    } else {   // OUT_PHASE: Eq.(25) P:L482 as atan2
-                        reinterpret_cast<float*>(P.out)[a] = atan2f(x.y, x.x);
-                    }
+                for (int e = 0; e < 16; ++e) {
+                    const int p = u[s] + e * Q;
+                    const size_t a = ((size_t)(p >> P.logwc) * P.ly + row) * (1u << P.logwc) + (p & ((1 << P.logwc) - 1));
+                    P.out[a] = v[s][e];
                 }
             }
+        }
+    } else if constexpr (KIND == ROW_INV) {
+        if constexpr (IOM == OUT_COMPLEX) {
+            const float sc = P.out_scale;
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int row = lane0 + (C::PAIR ? s : 0);
+                if (row >= P.rows) continue;
+                const size_t base = (size_t)row * P.pitch + u[s];
+#pragma unroll
+                for (int e = 0; e < NE; ++e) P.out[base + e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
+            }
+        } else {
+            // GS constraints (S10) by a rolled loop over the thread's samples, staged through its own
+            // slots of the tile buffer (rsqrt / atan2f would otherwise be unrolled 32 times).
+            __syncthreads();                               // tile buffer no longer being read
+            float2* mine = sm + threadIdx.x;
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int e = 0; e < NE; ++e) mine[(2 * e + s) * C::T] = v[s][e];
+#pragma unroll 1
+            for (int i = 0; i < 2 * NE; ++i) {
+                const int s = i & 1, e = i >> 1;
+                const int row = lane0 + (C::PAIR ? s : 0);
+                if (row >= P.rows) continue;
+                const size_t a = (size_t)row * P.pitch + (s ? u[1] : u[0]) + e * Q;
+                const float2 x = mine[i * C::T];          // the sample is conj(x)
+                if constexpr (IOM == OUT_PHASOR_AMP) {
+                    // phase constraint then amplitude constraint (Listing 8 lines 11-13 / 15-16): keep
+                    // u/|u| (1 where u == 0), replace the amplitude by that of the next plane
+                    const float m2 = x.x * x.x + x.y * x.y;
+                    const float am = P.out_amp[a];
+                    float2 ph = make_float2(1.f, 0.f);
+                    if (m2 > 0.f) { const float r = rsqrtf(m2); ph = make_float2(x.x * r, -x.y * r); }
+                    P.out[a] = make_float2(am * ph.x, am * ph.y);
+                } else {   // OUT_PHASE: Eq.(25) P:L482 as atan2
+                    reinterpret_cast<float*>(P.out)[a] = atan2f(-x.y, x.x);
+                }
+            }
+        }
+    } else {
+        float2* dst = P.out + (size_t)tile * P.ly * W;
+        constexpr bool CONJ = (KIND != COL_FWD);
+        if constexpr (C::PAIR) {
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                const float2 a = v[0][e], b = v[1][e];
+                *reinterpret_cast<float4*>(&dst[(size_t)(u[0] + e * Q) * W + w0]) =
+                    CONJ ? make_float4(a.x, -a.y, b.x, -b.y) : make_float4(a.x, a.y, b.x, b.y);
+            }
+        } else {
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+#pragma unroll
+                for (int e = 0; e < 16; ++e)
+                    if (!PAD || u[s] + e * Q < C::N / 2)
+                        dst[u[s] + e * Q] = CONJ ? cconj(v[s][e]) : v[s][e];
         }
     }
 }
 
-template <int LOGN, int KIND>
+template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
-    constexpr size_t smem = TileShape<LOGN, tile_logw(LOGN)>::SMEM_BYTES;
+    constexpr size_t smem = Tile<LOGN>::SMEM_BYTES;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(pass_kernel<LOGN, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(pass_kernel<LOGN, KIND, PAD, MID, IOM>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    pass_kernel<LOGN, KIND><<<n_tiles, tile_threads(LOGN), smem, s>>>(p);
+    pass_kernel<LOGN, KIND, PAD, MID, IOM><<<n_tiles, Tile<LOGN>::T, smem, s>>>(p);
     return cudaGetLastError();
 }
 
+template <int LOGN, int KIND, bool PAD, int MID>
+static cudaError_t launch_iom(int iom, int n_tiles, cudaStream_t s, const PassParams& p) {
+    if constexpr (KIND == ROW_FWD) {
+        return iom == IN_COMPLEX ? launch_one<LOGN, KIND, PAD, MID, IN_COMPLEX>(n_tiles, s, p)
+                                 : launch_one<LOGN, KIND, PAD, MID, IN_AMP_PHASE>(n_tiles, s, p);
+    } else if constexpr (KIND == ROW_INV) {
+        return iom == OUT_COMPLEX      ? launch_one<LOGN, KIND, PAD, MID, OUT_COMPLEX>(n_tiles, s, p)
+               : iom == OUT_PHASOR_AMP ? launch_one<LOGN, KIND, PAD, MID, OUT_PHASOR_AMP>(n_tiles, s, p)
+                                       : launch_one<LOGN, KIND, PAD, MID, OUT_PHASE>(n_tiles, s, p);
+    } else {
+        return launch_one<LOGN, KIND, PAD, MID, 0>(n_tiles, s, p);
+    }
+}
+
 template <int LOGN>
-static cudaError_t launch_pass_impl(int kind, int n_tiles, cudaStream_t s, const PassParams& p) {
-    switch (kind) {
-        case KIND_FWD: return launch_one<LOGN, KIND_FWD>(n_tiles, s, p);
-        case KIND_INV: return launch_one<LOGN, KIND_INV>(n_tiles, s, p);
-        case KIND_FUSED: return launch_one<LOGN, KIND_FUSED>(n_tiles, s, p);
-        case KIND_MIDINV: return launch_one<LOGN, KIND_MIDINV>(n_tiles, s, p);
+static cudaError_t launch_pass_impl(int kind, int pad, int mid, int n_tiles, cudaStream_t s, const PassParams& p) {
+    const int key = kind * 100 + pad * 10 + mid;
+    switch (key) {
+        case ROW_FWD * 100 + 0: return launch_iom<LOGN, ROW_FWD, false, MID_NONE>(p.in_mode, n_tiles, s, p);
+        case ROW_FWD * 100 + 10: return launch_iom<LOGN, ROW_FWD, true, MID_NONE>(p.in_mode, n_tiles, s, p);
+        case ROW_INV * 100 + 0: return launch_iom<LOGN, ROW_INV, false, MID_NONE>(p.out_mode, n_tiles, s, p);
+        case ROW_INV * 100 + 10: return launch_iom<LOGN, ROW_INV, true, MID_NONE>(p.out_mode, n_tiles, s, p);
+        case COL_FWD * 100 + 0: return launch_iom<LOGN, COL_FWD, false, MID_NONE>(0, n_tiles, s, p);
+        case COL_FUSED * 100 + 10 + MID_TABLES: return launch_iom<LOGN, COL_FUSED, true, MID_TABLES>(0, n_tiles, s, p);
+        case COL_FUSED * 100 + MID_ASM_SPLIT: return launch_iom<LOGN, COL_FUSED, false, MID_ASM_SPLIT>(0, n_tiles, s, p);
+        case COL_FUSED * 100 + MID_ASM_F64: return launch_iom<LOGN, COL_FUSED, false, MID_ASM_F64>(0, n_tiles, s, p);
+        case COL_MIDINV * 100 + MID_ASM_SPLIT: return launch_iom<LOGN, COL_MIDINV, false, MID_ASM_SPLIT>(0, n_tiles, s, p);
+        case COL_MIDINV * 100 + MID_ASM_F64: return launch_iom<LOGN, COL_MIDINV, false, MID_ASM_F64>(0, n_tiles, s, p);
     }
     return cudaErrorInvalidValue;
 }

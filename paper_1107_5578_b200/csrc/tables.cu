@@ -72,8 +72,29 @@ __global__ void __launch_bounds__(1024) chirp_fft_kernel(ChirpAxis ax0, ChirpAxi
     }
 }
 
-cudaError_t build_chirp_spectrum(const ChirpAxis& ax0, const ChirpAxis* ax1, cudaStream_t s) {
-    chirp_fft_kernel<<<ax1 ? 2 : 1, 1024, 0, s>>>(ax0, ax1 ? *ax1 : ax0);
+cudaError_t build_chirp_spectrum(const ChirpAxis& ax0, const ChirpAxis& ax1, cudaStream_t s) {
+    chirp_fft_kernel<<<2, 1024, 0, s>>>(ax0, ax1);
+    return cudaGetLastError();
+}
+
+// ASM split path (S2): per plane, theta_x[k] = frac(c0 - ax ks^2), theta_y[l] = frac(-ay ls^2) in cycles.
+// ax ks^2 reaches ~5e3 cycles (c3, z = 0.5 m): formed in fp64, reduced mod 1, then rounded to fp32.
+__global__ void asm_phase_kernel(float* tab, const __grid_constant__ AsmPlaneBatch planes, int mx, int my) {
+    const AsmPlane pl = planes.p[blockIdx.y];
+    float* t = tab + (size_t)blockIdx.y * (mx + my);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < mx + my; i += gridDim.x * blockDim.x) {
+        const bool isx = i < mx;
+        const int j = isx ? i : i - mx, m = isx ? mx : my;
+        const double b = (double)((j < m / 2) ? j : j - m);
+        double c = (isx ? pl.c0 : 0.0) - (isx ? pl.ax : pl.ay) * b * b;
+        c -= rint(c);
+        t[i] = (float)c;
+    }
+}
+
+cudaError_t build_asm_phase_tables(float* tab, const AsmPlaneBatch& planes, int n_planes, int mx, int my, cudaStream_t s) {
+    dim3 grid((mx + my + 255) / 256 > 64 ? 64 : (mx + my + 255) / 256, n_planes);
+    asm_phase_kernel<<<grid, 256, 0, s>>>(tab, planes, mx, my);
     return cudaGetLastError();
 }
 
