@@ -236,14 +236,14 @@ def run_cuda(args):
     per_kind = {}
     for tag, t_ms in tm:
         per_kind.setdefault(tag & 15, []).append(t_ms)
-    names = {0: "pass_R (row FFT)", 2: "pass_C (fused column FFT*H*IFFT)", 1: "pass_R' (row IFFT)"}
+    names = {0: "pass_R (row FFT)", 3: "pass_C (fused column FFT*H*IFFT)", 1: "pass_R' (row IFFT)"}
     passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
     dom_kind = max(per_kind, key=lambda k: np.mean(per_kind[k]))
     dom_ms = float(np.mean(per_kind[dom_kind]))
     peak, peak_src = _peak()
     alg_bytes = 16.0 * N * N                      # each pass reads 8 and writes 8 bytes per sample
     achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = _ncu_traffic({0: "pass_R", 1: "pass_Rinv", 2: "pass_C"}[dom_kind])
+    traffic = _ncu_traffic({0: "pass_R", 1: "pass_Rinv", 3: "pass_C"}[dom_kind])
     roofline = {"bound": "hbm", "kernel": names[dom_kind], "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms,

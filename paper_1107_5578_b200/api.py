@@ -18,7 +18,7 @@ from typing import Sequence
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libcwo.so")
+_LIB_PATH = os.environ.get("CWO_LIBRARY_PATH") or os.path.join(_HERE, "libcwo.so")
 
 CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA = 0, -1, -2, -3, -4
 CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS = 1, 2, 3, 4

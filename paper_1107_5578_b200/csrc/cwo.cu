@@ -215,8 +215,11 @@ extern "C" long long cwo_plan_launch_count(cwo_plan_t p) { return p ? p->launche
 
 enum { ROW_FWD = 0, ROW_INV = 1, COL_FWD = 2, COL_FUSED = 3, COL_MIDINV = 4 };   // == pass_kernel.cuh
 
+#ifndef CWO_LOGW12
+#define CWO_LOGW12 1
+#endif
 static int tile_logw_host(int logn) {   // == fft_core.cuh tile_logw
-    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn <= 13 ? 1 : 0;
+    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn == 12 ? CWO_LOGW12 : logn == 13 ? 1 : 0;
 }
 
 struct Geometry { int pad, logmx, logmy, mx, my, rb, logwc, wc; };

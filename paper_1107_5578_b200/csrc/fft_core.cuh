@@ -124,17 +124,26 @@ template <int R> __device__ __forceinline__ void unpermute(float2 (&v)[16]) {
 }
 
 // ---- tile configuration (one place: host sizing and kernels must agree) -----------------------
+#ifndef CWO_LOGW12
+#define CWO_LOGW12 1
+#endif
 constexpr int tile_logw(int logn) {
-    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn <= 13 ? 1 : 0;
+    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn == 12 ? CWO_LOGW12 : logn == 13 ? 1 : 0;
 }
 template <int LOGN> struct Tile {
     static constexpr int N = 1 << LOGN, Q = N / 16;
     static constexpr int LOGW = tile_logw(LOGN), W = 1 << LOGW;
     static constexpr bool PAIR = W >= 2;               // a thread's two slots are adjacent lanes
     static constexpr int T = PAIR ? Q * (W / 2) : Q / 2;
-    static constexpr int MINB = LOGN <= 12 ? 2 : 1;
+#ifndef CWO_MINB
+#define CWO_MINB 2
+#endif
+    static constexpr int MINB = (LOGN <= 12 && T <= 256) ? CWO_MINB : 1;
     static constexpr int L0 = LOGN & 3, M = LOGN >> 2; // n = 2^L0 * 16^M
     static constexpr size_t SMEM_BYTES = sizeof(float2) * (size_t)(N + N / 16) * W;
+    // unit-pair variants (W == 2): two lane planes, 2 pad elements every 16 points, planes 8 elements apart
+    static constexpr int XPLANE = N + N / 8 + 8;
+    static constexpr size_t SMEM_BYTES_X = sizeof(float2) * 2 * (size_t)XPLANE;
 };
 
 // shared-memory index of (point p, lane w): one pad row of W elements every 16 points
@@ -184,7 +193,7 @@ __device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], 
 }
 
 // Twiddle (if lns > 0) and butterflies of one radix-2^LR stage on both slots.
-template <int LOGN, int LR>
+template <int LOGN, int LR, bool SEP = !Tile<LOGN>::PAIR>
 __device__ __forceinline__ void butterflies(float2 (&v)[2][16], const int (&u)[2], int lns,
                                             const float2* __restrict__ tw) {
     using C = Tile<LOGN>;
@@ -196,7 +205,7 @@ __device__ __forceinline__ void butterflies(float2 (&v)[2][16], const int (&u)[2
             const int k0 = (u[0] + i * C::Q) & ((1 << lns) - 1);
             powers<R>(__ldg(&tw[k0 << (LOGN - lns - LR)]), w);
             apply_powers<R>(v[0], i, w);
-            if constexpr (!C::PAIR) {
+            if constexpr (SEP) {                  // the two slots are different units: own twiddles
                 const int k1 = (u[1] + i * C::Q) & ((1 << lns) - 1);
                 powers<R>(__ldg(&tw[k1 << (LOGN - lns - LR)]), w);
             }
@@ -239,6 +248,92 @@ __device__ __forceinline__ void transform(float2 (&v)[2][16], const int (&u)[2],
     }
     if constexpr (!HAS_FWD && HAS_INV) { /* mid (if any) was applied by the caller before the call */ }
     if constexpr (HAS_INV && L0 > 0) {                      // small radix last
+        butterflies<LOGN, L0>(v, u, 4 * M, tw);
+        unpermute<(1 << L0)>(v[0]); unpermute<(1 << L0)>(v[1]);
+    }
+}
+
+// ---- unit-pair mapping (tiles of W == 2 lanes) ------------------------------------------------------
+// Where a row pass meets the column-tiled workspace T[x/2][y][x%2], the 16 bytes that are contiguous in
+// memory are two neighbouring points (x, x+1) of ONE row.  For that one stage a thread therefore holds
+// the units 2i and 2i+1 of lane w (thread = 2i' + w) instead of unit u in both lanes, so that global
+// accesses are 128-bit and a thread pair covers a full 32-byte sector.
+
+// Forward transform; the LAST stage runs in unit-pair mapping.  In: standard mapping (u = thread,
+// both lanes).  Out: register e of slot s <-> point 2i + s + e*Q of lane w.
+template <int LOGN>
+__device__ __forceinline__ void transform_fwd_xlast(float2 (&v)[2][16], int t, float2* sm,
+                                                    const float2* __restrict__ tw) {
+    using C = Tile<LOGN>;
+    constexpr int L0 = C::L0, M = C::M, Q = C::Q;
+    static_assert(C::W == 2 && M >= 2, "unit-pair mapping needs a 2-lane tile");
+    const int u[2] = {t, t};
+    if constexpr (L0 > 0) {
+        butterflies<LOGN, L0>(v, u, 0, tw);
+        exchange<LOGN, L0>(v, u, 0, 0, sm);
+    }
+#pragma unroll 1
+    for (int s = 0; s < M - 2; ++s) {
+        butterflies<LOGN, 4>(v, u, L0 + 4 * s, tw);
+        exchange<LOGN, 4>(v, u, 0, L0 + 4 * s, sm);
+    }
+    constexpr int lns = L0 + 4 * (M - 2);
+    butterflies<LOGN, 4>(v, u, lns, tw);
+    // exchange into two lane planes, then read back unit pairs
+    const int w = t & 1, i2 = t & ~1;                      // units i2, i2 + 1
+    __syncthreads();
+    {
+        const int j0 = ((t >> lns) << (lns + 4)) + (t & ((1 << lns) - 1));
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const int p = j0 + (q << lns), pi = p + 2 * (p >> 4);
+            sm[pi] = v[0][perm<16>(q)];
+            sm[C::XPLANE + pi] = v[1][perm<16>(q)];
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int p = i2 + e * Q;
+        const float4 x = *reinterpret_cast<const float4*>(&sm[w * C::XPLANE + p + 2 * (p >> 4)]);
+        v[0][e] = make_float2(x.x, x.y);
+        v[1][e] = make_float2(x.z, x.w);
+    }
+    const int ux[2] = {i2, i2 + 1};
+    butterflies<LOGN, 4, true>(v, ux, L0 + 4 * (M - 1), tw);
+    unpermute<16>(v[0]); unpermute<16>(v[1]);
+}
+
+// Inverse transform (as conj . forward . conj, the conj being the caller's); the FIRST stage runs in
+// unit-pair mapping.  In: register e of slot s <-> point 2i + s + e*Q of lane w.  Out: standard mapping.
+template <int LOGN>
+__device__ __forceinline__ void transform_inv_xfirst(float2 (&v)[2][16], int t, float2* sm,
+                                                     const float2* __restrict__ tw) {
+    using C = Tile<LOGN>;
+    constexpr int L0 = C::L0, M = C::M, Q = C::Q;
+    static_assert(C::W == 2 && M >= 2, "unit-pair mapping needs a 2-lane tile");
+    const int w = t & 1, i2 = t & ~1;
+    dft16(v[0]); dft16(v[1]);                               // Ns = 1: no twiddles
+    __syncthreads();
+#pragma unroll
+    for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int q = 0; q < 16; ++q) sm[sidx<1>(16 * (i2 + s) + q, w)] = v[s][perm<16>(q)];
+    __syncthreads();
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const float4 x = *reinterpret_cast<const float4*>(&sm[sidx<1>(t + e * Q, 0)]);
+        v[0][e] = make_float2(x.x, x.y);
+        v[1][e] = make_float2(x.z, x.w);
+    }
+    const int u[2] = {t, t};
+#pragma unroll 1
+    for (int s = 1; s < M; ++s) {
+        butterflies<LOGN, 4>(v, u, 4 * s, tw);
+        if (L0 == 0 && s == M - 1) { unpermute<16>(v[0]); unpermute<16>(v[1]); break; }
+        exchange<LOGN, 4>(v, u, 0, 4 * s, sm);
+    }
+    if constexpr (L0 > 0) {
         butterflies<LOGN, L0>(v, u, 4 * M, tw);
         unpermute<(1 << L0)>(v[0]); unpermute<(1 << L0)>(v[1]);
     }

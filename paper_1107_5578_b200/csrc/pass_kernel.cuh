@@ -119,7 +119,8 @@ template <int LOGN> struct MidSelect<LOGN, MID_ASM_SPLIT> { using type = MidAsmS
 template <int LOGN> struct MidSelect<LOGN, MID_ASM_F64> { using type = MidAsmF64<LOGN>; };
 
 // IOM: ROW_FWD -> InMode of the load, ROW_INV -> OutMode of the store, column passes -> 0.
-template <int LOGN, int KIND, bool PAD, int MID, int IOM>
+// X (row passes over a workspace of 2-wide column tiles, W == 2): unit-pair mapping at the workspace side.
+template <int LOGN, int KIND, bool PAD, int MID, int IOM, bool X>
 __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB)
 pass_kernel(const __grid_constant__ PassParams P) {
     using C = Tile<LOGN>;
@@ -177,6 +178,15 @@ pass_kernel(const __grid_constant__ PassParams P) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) v[s][e] = (e < NE) ? mine[(2 * e + s) * C::T] : make_float2(0.f, 0.f);
         }
+    } else if constexpr (KIND == ROW_INV && X) {
+        // rows of the column-tiled workspace, 2-wide tiles: points (x, x+1) of row tile*2 + w are 16 bytes
+        const int row = tile * 2 + (threadIdx.x & 1);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int x = (threadIdx.x & ~1) + e * Q;
+            const float4 t4 = *reinterpret_cast<const float4*>(&P.in[((size_t)(x >> 1) * P.ly + row) * 2]);
+            v[0][e] = make_float2(t4.x, -t4.y); v[1][e] = make_float2(t4.z, -t4.w);
+        }
     } else if constexpr (KIND == ROW_INV) {
         // rows of the column-tiled workspace
 #pragma unroll
@@ -186,7 +196,11 @@ pass_kernel(const __grid_constant__ PassParams P) {
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
                 const int p = u[s] + e * Q;
+#ifdef CWO_DEBUG_ROWMAJOR_WS
+                const size_t a = (size_t)row * C::N + p;
+#else
                 const size_t a = ((size_t)(p >> P.logwc) * P.ly + row) * (1u << P.logwc) + (p & ((1 << P.logwc) - 1));
+#endif
                 v[s][e] = ok ? cconj(P.in[a]) : make_float2(0.f, 0.f);
             }
         }
@@ -213,7 +227,11 @@ pass_kernel(const __grid_constant__ PassParams P) {
     }
 
     // ---- transform ------------------------------------------------------------------------------
-    if constexpr (KIND == ROW_FWD || KIND == COL_FWD) {
+    if constexpr (KIND == ROW_FWD && X) {
+        transform_fwd_xlast<LOGN>(v, threadIdx.x, sm, P.tw);
+    } else if constexpr (KIND == ROW_INV && X) {
+        transform_inv_xfirst<LOGN>(v, threadIdx.x, sm, P.tw);
+    } else if constexpr (KIND == ROW_FWD || KIND == COL_FWD) {
         transform<LOGN, true, false>(v, u, w0, sm, P.tw, MidNone());
     } else if constexpr (KIND == ROW_INV) {
         transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone());
@@ -228,7 +246,15 @@ pass_kernel(const __grid_constant__ PassParams P) {
     }
 
     // ---- store (conj completes an inverse transform) -----------------------------------------------
-    if constexpr (KIND == ROW_FWD) {
+    if constexpr (KIND == ROW_FWD && X) {
+        const int row = tile * 2 + (threadIdx.x & 1);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int x = (threadIdx.x & ~1) + e * Q;
+            *reinterpret_cast<float4*>(&P.out[((size_t)(x >> 1) * P.ly + row) * 2]) =
+                make_float4(v[0][e].x, v[0][e].y, v[1][e].x, v[1][e].y);
+        }
+    } else if constexpr (KIND == ROW_FWD) {
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
             const int row = lane0 + (C::PAIR ? s : 0);
@@ -236,7 +262,11 @@ pass_kernel(const __grid_constant__ PassParams P) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
                     const int p = u[s] + e * Q;
+#ifdef CWO_DEBUG_ROWMAJOR_WS
+                    const size_t a = (size_t)row * C::N + p;
+#else
                     const size_t a = ((size_t)(p >> P.logwc) * P.ly + row) * (1u << P.logwc) + (p & ((1 << P.logwc) - 1));
+#endif
                     P.out[a] = v[s][e];
                 }
             }
@@ -302,18 +332,26 @@ pass_kernel(const __grid_constant__ PassParams P) {
     }
 }
 
-template <int LOGN, int KIND, bool PAD, int MID, int IOM>
-static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
-    constexpr size_t smem = Tile<LOGN>::SMEM_BYTES;
+template <int LOGN, int KIND, bool PAD, int MID, int IOM, bool X>
+static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
+    constexpr size_t smem = (X && KIND == ROW_FWD) ? Tile<LOGN>::SMEM_BYTES_X : Tile<LOGN>::SMEM_BYTES;
     static bool configured = false;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(pass_kernel<LOGN, KIND, PAD, MID, IOM>,
+        cudaError_t e = cudaFuncSetAttribute(pass_kernel<LOGN, KIND, PAD, MID, IOM, X>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    pass_kernel<LOGN, KIND, PAD, MID, IOM><<<n_tiles, Tile<LOGN>::T, smem, s>>>(p);
+    pass_kernel<LOGN, KIND, PAD, MID, IOM, X><<<n_tiles, Tile<LOGN>::T, smem, s>>>(p);
     return cudaGetLastError();
+}
+
+template <int LOGN, int KIND, bool PAD, int MID, int IOM>
+static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
+    if constexpr ((KIND == ROW_FWD || KIND == ROW_INV) && Tile<LOGN>::W == 2) {
+        if (p.logwc == 1) return launch_x<LOGN, KIND, PAD, MID, IOM, true>(n_tiles, s, p);
+    }
+    return launch_x<LOGN, KIND, PAD, MID, IOM, false>(n_tiles, s, p);
 }
 
 template <int LOGN, int KIND, bool PAD, int MID>
