@@ -53,8 +53,11 @@ enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4 };
 enum {
     CWO_OPT_GS_METHOD = 1,  /* value: CWO_GS_FRESNEL (default; BASELINE config 5) or CWO_GS_ASM
                                (the paper's Listing 8) */
-    CWO_OPT_TIMING = 2      /* value 1: bracket every pass kernel with a CUDA event pair on the plan's
+    CWO_OPT_TIMING = 2,     /* value 1: bracket every pass kernel with a CUDA event pair on the plan's
                                stream (read with cwo_plan_timings); 0 (default): off */
+    CWO_OPT_PIPELINE = 3    /* value 1 (default): transform lengths 1024..4096 run as persistent CTAs that
+                               prefetch their next tiles (TMA bulk copies); 0: one CTA per tile everywhere.
+                               Same arithmetic either way. */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
 

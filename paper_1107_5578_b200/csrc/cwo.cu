@@ -19,6 +19,7 @@ struct cwo_plan_s {
     void* ws;
     size_t ws_bytes;
     int gs_method;
+    int pipeline;
     int last_cuda_error;
     long long launches;
     float2* tw[MAX_LOGN + 2];       // fp32 twiddles per log2 length (lazily built)
@@ -108,6 +109,7 @@ extern "C" int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t*
     p->Nx = Nx; p->Ny = Ny; p->lognx = lx; p->logny = ly;
     p->px = p->py = pitch; p->lambda = lambda;
     p->gs_method = CWO_GS_FRESNEL;
+    p->pipeline = 1;
     p->ev = new std::vector<cudaEvent_t>();
     p->ev_tag = new std::vector<int>();
     int rc = CWO_OK;
@@ -147,6 +149,10 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
     if (!p) return CWO_EINVAL;
     if (key == CWO_OPT_GS_METHOD && (value == CWO_GS_FRESNEL || value == CWO_GS_ASM)) {
         p->gs_method = value;
+        return CWO_OK;
+    }
+    if (key == CWO_OPT_PIPELINE && (value == 0 || value == 1)) {
+        p->pipeline = value;
         return CWO_OK;
     }
     if (key == CWO_OPT_TIMING && (value == 0 || value == 1)) {
@@ -332,11 +338,11 @@ static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int s
 static void row_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
     pp.rows = p->Ny; pp.pitch = p->Nx; pp.ly = p->Ny; pp.logwc = g.logwc;
-    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f;
+    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline;
 }
 static void col_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
-    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f;
+    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline;
 }
 
 static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float2* ws) {

@@ -21,6 +21,8 @@ struct PassParams {
     int pitch;                // row passes: row pitch (elements) of the row-major field and real arrays
     int ly;                   // rows kept in the column-tiled workspace
     int logwc;                // row passes: log2 of the column-tile width of the workspace
+    int n_tiles;              // pipelined passes: total number of tiles (the grid is one CTA per SM)
+    int use_pipe;             // 1: use the pipelined form where it exists (CWO_OPT_PIPELINE)
     const float2* tw;         // forward twiddles exp(-i 2 pi m/n), m < n
     float out_scale;          // ROW_INV store
     // Mid (transfer function / impulse-response spectrum, S2/S5/S7); lane = x bin, point = y bin

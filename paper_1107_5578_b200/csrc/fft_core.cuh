@@ -141,9 +141,20 @@ template <int LOGN> struct Tile {
     static constexpr int MINB = (LOGN <= 12 && T <= 256) ? CWO_MINB : 1;
     static constexpr int L0 = LOGN & 3, M = LOGN >> 2; // n = 2^L0 * 16^M
     static constexpr size_t SMEM_BYTES = sizeof(float2) * (size_t)(N + N / 16) * W;
-    // unit-pair variants (W == 2): two lane planes, 2 pad elements every 16 points, planes 8 elements apart
-    static constexpr int XPLANE = N + N / 8 + 8;
-    static constexpr size_t SMEM_BYTES_X = sizeof(float2) * 2 * (size_t)XPLANE;
+    // unit-pair variants: one plane per lane, 2 pad elements every 16 points, plane offsets staggered
+    // over the banks (16/W elements mod 16)
+    static constexpr int XPLANE = N + N / 8 + (W >= 2 ? 16 / W : 8);
+    static constexpr size_t SMEM_BYTES_X = sizeof(float2) * (size_t)W * (size_t)XPLANE;
+};
+
+// Barrier over the threads that share a tile: the whole CTA (one tile per CTA), or a named barrier over
+// one 256-thread group of a persistent CTA that keeps several tiles in flight (pipe_kernel.cuh).
+struct SyncCta {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+struct SyncGroup {
+    int id;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 256;" ::"r"(id) : "memory"); }
 };
 
 // shared-memory index of (point p, lane w): one pad row of W elements every 16 points
@@ -151,11 +162,12 @@ template <int LOGW> __device__ __forceinline__ int sidx(int p, int w) { return (
 
 // Write the outputs of a radix-2^LR stage with Ns = 2^lns to shared memory in Stockham order and read
 // back the inputs of the next stage.  u[], w0: the thread's units (see top of file).
-template <int LOGN, int LR>
-__device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], int w0, int lns, float2* sm) {
+template <int LOGN, int LR, class SY>
+__device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], int w0, int lns, float2* sm,
+                                         const SY& sync) {
     using C = Tile<LOGN>;
     constexpr int R = 1 << LR, S = 16 / R;
-    __syncthreads();                       // everyone has finished reading the previous contents
+    sync();                       // everyone has finished reading the previous contents
     if constexpr (C::PAIR) {
 #pragma unroll
         for (int i = 0; i < S; ++i) {
@@ -167,7 +179,7 @@ __device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], 
                 *reinterpret_cast<float4*>(&sm[sidx<C::LOGW>(j0 + (q << lns), w0)]) = make_float4(a.x, a.y, b.x, b.y);
             }
         }
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             const float4 t = *reinterpret_cast<const float4*>(&sm[sidx<C::LOGW>(u[0] + e * C::Q, w0)]);
@@ -184,7 +196,7 @@ __device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], 
 #pragma unroll
                 for (int q = 0; q < R; ++q) sm[sidx<0>(j0 + (q << lns), 0)] = v[s][i + perm<R>(q) * S];
             }
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int s = 0; s < 2; ++s)
 #pragma unroll
@@ -219,15 +231,15 @@ __device__ __forceinline__ void butterflies(float2 (&v)[2][16], const int (&u)[2
 // Forward and/or inverse transform of the tile held in registers, with `mid` applied between them
 // (mid must also conjugate so that the second forward transform acts as an inverse one).
 // In / out: register e of unit u <-> point u + e*Q.
-template <int LOGN, bool HAS_FWD, bool HAS_INV, class Mid>
+template <int LOGN, bool HAS_FWD, bool HAS_INV, class Mid, class SY>
 __device__ __forceinline__ void transform(float2 (&v)[2][16], const int (&u)[2], int w0, float2* sm,
-                                          const float2* __restrict__ tw, Mid mid) {
+                                          const float2* __restrict__ tw, Mid mid, const SY& sync) {
     using C = Tile<LOGN>;
     constexpr int L0 = C::L0, M = C::M;
     static_assert(M >= 1, "n >= 16");
     if constexpr (HAS_FWD && L0 > 0) {                      // small radix first, no twiddles
         butterflies<LOGN, L0>(v, u, 0, tw);
-        exchange<LOGN, L0>(v, u, w0, 0, sm);
+        exchange<LOGN, L0>(v, u, w0, 0, sm, sync);
     }
     constexpr int NST = (HAS_FWD ? M : 0) + (HAS_INV ? M : 0);
 #pragma unroll 1
@@ -244,7 +256,7 @@ __device__ __forceinline__ void transform(float2 (&v)[2][16], const int (&u)[2],
             }
             if (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); break; }
         }
-        exchange<LOGN, 4>(v, u, w0, lns, sm);
+        exchange<LOGN, 4>(v, u, w0, lns, sm, sync);
     }
     if constexpr (!HAS_FWD && HAS_INV) { /* mid (if any) was applied by the caller before the call */ }
     if constexpr (HAS_INV && L0 > 0) {                      // small radix last
@@ -253,45 +265,47 @@ __device__ __forceinline__ void transform(float2 (&v)[2][16], const int (&u)[2],
     }
 }
 
-// ---- unit-pair mapping (tiles of W == 2 lanes) ------------------------------------------------------
-// Where a row pass meets the column-tiled workspace T[x/2][y][x%2], the 16 bytes that are contiguous in
+// ---- unit-pair mapping ---------------------------------------------------------------------------------
+// Where a row pass meets the column-tiled workspace T[x/Wc][y][x%Wc], the 16 bytes that are contiguous in
 // memory are two neighbouring points (x, x+1) of ONE row.  For that one stage a thread therefore holds
-// the units 2i and 2i+1 of lane w (thread = 2i' + w) instead of unit u in both lanes, so that global
-// accesses are 128-bit and a thread pair covers a full 32-byte sector.
+// the units 2i and 2i+1 of lane w (thread = i*W + w) instead of unit u in two adjacent lanes, so that
+// global accesses are 128-bit and neighbouring threads cover full 32-byte sectors.
 
-// Forward transform; the LAST stage runs in unit-pair mapping.  In: standard mapping (u = thread,
-// both lanes).  Out: register e of slot s <-> point 2i + s + e*Q of lane w.
-template <int LOGN>
+// Forward transform; the LAST stage runs in unit-pair mapping.  In: standard mapping.
+// Out: register e of slot s <-> point 2i + s + e*Q of lane w, (w, i) = (t % W, t / W).
+template <int LOGN, class SY>
 __device__ __forceinline__ void transform_fwd_xlast(float2 (&v)[2][16], int t, float2* sm,
-                                                    const float2* __restrict__ tw) {
+                                                    const float2* __restrict__ tw, const SY& sync) {
     using C = Tile<LOGN>;
-    constexpr int L0 = C::L0, M = C::M, Q = C::Q;
-    static_assert(C::W == 2 && M >= 2, "unit-pair mapping needs a 2-lane tile");
-    const int u[2] = {t, t};
+    constexpr int L0 = C::L0, M = C::M, Q = C::Q, W = C::W;
+    static_assert(C::PAIR && M >= 2, "unit-pair mapping needs a tile of >= 2 lanes");
+    const int us = t / (W / 2), w0 = 2 * (t % (W / 2));
+    const int u[2] = {us, us};
     if constexpr (L0 > 0) {
         butterflies<LOGN, L0>(v, u, 0, tw);
-        exchange<LOGN, L0>(v, u, 0, 0, sm);
+        exchange<LOGN, L0>(v, u, w0, 0, sm, sync);
     }
 #pragma unroll 1
     for (int s = 0; s < M - 2; ++s) {
         butterflies<LOGN, 4>(v, u, L0 + 4 * s, tw);
-        exchange<LOGN, 4>(v, u, 0, L0 + 4 * s, sm);
+        exchange<LOGN, 4>(v, u, w0, L0 + 4 * s, sm, sync);
     }
     constexpr int lns = L0 + 4 * (M - 2);
     butterflies<LOGN, 4>(v, u, lns, tw);
-    // exchange into two lane planes, then read back unit pairs
-    const int w = t & 1, i2 = t & ~1;                      // units i2, i2 + 1
-    __syncthreads();
+    // exchange into one plane per lane, then read back unit pairs
+    sync();
     {
-        const int j0 = ((t >> lns) << (lns + 4)) + (t & ((1 << lns) - 1));
+        const int j0 = ((us >> lns) << (lns + 4)) + (us & ((1 << lns) - 1));
+        float2* pl = sm + w0 * C::XPLANE;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             const int p = j0 + (q << lns), pi = p + 2 * (p >> 4);
-            sm[pi] = v[0][perm<16>(q)];
-            sm[C::XPLANE + pi] = v[1][perm<16>(q)];
+            pl[pi] = v[0][perm<16>(q)];
+            pl[C::XPLANE + pi] = v[1][perm<16>(q)];
         }
     }
-    __syncthreads();
+    sync();
+    const int w = t % W, i2 = 2 * (t / W);                 // units i2, i2 + 1 of lane w
 #pragma unroll
     for (int e = 0; e < 16; ++e) {
         const int p = i2 + e * Q;
@@ -306,32 +320,33 @@ __device__ __forceinline__ void transform_fwd_xlast(float2 (&v)[2][16], int t, f
 
 // Inverse transform (as conj . forward . conj, the conj being the caller's); the FIRST stage runs in
 // unit-pair mapping.  In: register e of slot s <-> point 2i + s + e*Q of lane w.  Out: standard mapping.
-template <int LOGN>
+template <int LOGN, class SY>
 __device__ __forceinline__ void transform_inv_xfirst(float2 (&v)[2][16], int t, float2* sm,
-                                                     const float2* __restrict__ tw) {
+                                                     const float2* __restrict__ tw, const SY& sync) {
     using C = Tile<LOGN>;
-    constexpr int L0 = C::L0, M = C::M, Q = C::Q;
-    static_assert(C::W == 2 && M >= 2, "unit-pair mapping needs a 2-lane tile");
-    const int w = t & 1, i2 = t & ~1;
+    constexpr int L0 = C::L0, M = C::M, Q = C::Q, W = C::W;
+    static_assert(C::PAIR && M >= 2, "unit-pair mapping needs a tile of >= 2 lanes");
+    const int w = t % W, i2 = 2 * (t / W);
     dft16(v[0]); dft16(v[1]);                               // Ns = 1: no twiddles
-    __syncthreads();
+    sync();
 #pragma unroll
     for (int s = 0; s < 2; ++s)
 #pragma unroll
-        for (int q = 0; q < 16; ++q) sm[sidx<1>(16 * (i2 + s) + q, w)] = v[s][perm<16>(q)];
-    __syncthreads();
+        for (int q = 0; q < 16; ++q) sm[sidx<C::LOGW>(16 * (i2 + s) + q, w)] = v[s][perm<16>(q)];
+    sync();
+    const int us = t / (W / 2), w0 = 2 * (t % (W / 2));
 #pragma unroll
     for (int e = 0; e < 16; ++e) {
-        const float4 x = *reinterpret_cast<const float4*>(&sm[sidx<1>(t + e * Q, 0)]);
+        const float4 x = *reinterpret_cast<const float4*>(&sm[sidx<C::LOGW>(us + e * Q, w0)]);
         v[0][e] = make_float2(x.x, x.y);
         v[1][e] = make_float2(x.z, x.w);
     }
-    const int u[2] = {t, t};
+    const int u[2] = {us, us};
 #pragma unroll 1
     for (int s = 1; s < M; ++s) {
         butterflies<LOGN, 4>(v, u, 4 * s, tw);
         if (L0 == 0 && s == M - 1) { unpermute<16>(v[0]); unpermute<16>(v[1]); break; }
-        exchange<LOGN, 4>(v, u, 0, 4 * s, sm);
+        exchange<LOGN, 4>(v, u, w0, 4 * s, sm, sync);
     }
     if constexpr (L0 > 0) {
         butterflies<LOGN, L0>(v, u, 4 * M, tw);

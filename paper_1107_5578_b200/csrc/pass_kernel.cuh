@@ -228,20 +228,20 @@ pass_kernel(const __grid_constant__ PassParams P) {
 
     // ---- transform ------------------------------------------------------------------------------
     if constexpr (KIND == ROW_FWD && X) {
-        transform_fwd_xlast<LOGN>(v, threadIdx.x, sm, P.tw);
+        transform_fwd_xlast<LOGN>(v, threadIdx.x, sm, P.tw, SyncCta());
     } else if constexpr (KIND == ROW_INV && X) {
-        transform_inv_xfirst<LOGN>(v, threadIdx.x, sm, P.tw);
+        transform_inv_xfirst<LOGN>(v, threadIdx.x, sm, P.tw, SyncCta());
     } else if constexpr (KIND == ROW_FWD || KIND == COL_FWD) {
-        transform<LOGN, true, false>(v, u, w0, sm, P.tw, MidNone());
+        transform<LOGN, true, false>(v, u, w0, sm, P.tw, MidNone(), SyncCta());
     } else if constexpr (KIND == ROW_INV) {
-        transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone());
+        transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone(), SyncCta());
     } else {
         typename MidSelect<LOGN, MID>::type mid{P, u, lane0, sm};
         if constexpr (KIND == COL_FUSED) {
-            transform<LOGN, true, true>(v, u, w0, sm, P.tw, mid);
+            transform<LOGN, true, true>(v, u, w0, sm, P.tw, mid, SyncCta());
         } else {
             mid(v);
-            transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone());
+            transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone(), SyncCta());
         }
     }
 
@@ -346,8 +346,19 @@ static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
     return cudaGetLastError();
 }
 
+// pipe_kernel.cuh: persistent, prefetching form of the same pass for the HBM-sized tile shapes
+constexpr bool pipe_supported(int logn) { return logn >= 10 && logn <= 12; }
+template <int LOGN, int KIND, bool PAD, int MID, int IOM>
+static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p);
+
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
+    constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
+    if constexpr (pipe_supported(LOGN) && MID != MID_ASM_F64 &&
+                  (!ROWPASS || (KIND == ROW_FWD && IOM == IN_COMPLEX) || (KIND == ROW_INV && IOM == OUT_COMPLEX))) {
+        if (p.use_pipe && (!ROWPASS || (p.logwc >= 1 && p.rows % Tile<LOGN>::W == 0)))
+            return launch_pipe<LOGN, KIND, PAD, MID, IOM>(n_tiles, s, p);
+    }
     if constexpr ((KIND == ROW_FWD || KIND == ROW_INV) && Tile<LOGN>::W == 2) {
         if (p.logwc == 1) return launch_x<LOGN, KIND, PAD, MID, IOM, true>(n_tiles, s, p);
     }
