@@ -5,6 +5,7 @@
 #include <new>
 #include <stdint.h>
 #include <string.h>
+#include <stdlib.h>
 #include <vector>
 
 #include "../../include/cwo.h"
@@ -335,24 +336,59 @@ static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int s
 
 // ---- the passes ---------------------------------------------------------------------------------------
 
+// The column-tiled workspace T[x/Wc][y][x%Wc] seen as a 2-D float tensor: inner dimension = one column
+// group (ly rows x Wc complex, contiguous), outer dimension = the Nx/Wc column groups.  A row tile
+// (W rows, every x) is a box of W*Wc complex x (up to) 256 column groups: 32..128 contiguous bytes per
+// column group, which TMA scatters/gathers without occupying the SM's load/store path.
+typedef CUresult (*encode_tiled_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static encode_tiled_t get_encode_tiled() {
+    static encode_tiled_t fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = (encode_tiled_t)f;
+    }
+    return fn;
+}
+static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int logwc, int w_rows) {
+    encode_tiled_t enc = get_encode_tiled();
+    if (!enc || logwc < 1) return false;
+    const int wc = 1 << logwc, groups = mx >> logwc;
+    cuuint64_t dims[2] = {(cuuint64_t)ly * wc * 2, (cuuint64_t)groups};
+    cuuint64_t strides[1] = {(cuuint64_t)ly * wc * 8};
+    cuuint32_t box[2] = {(cuuint32_t)(w_rows * wc * 2), (cuuint32_t)(groups < 256 ? groups : 256)};
+    cuuint32_t es[2] = {1, 1};
+    return enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(ws), dims, strides, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 static void row_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
     pp.rows = p->Ny; pp.pitch = p->Nx; pp.ly = p->Ny; pp.logwc = g.logwc;
-    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline;
+    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = getenv("CWO_DEBUG") ? atoi(getenv("CWO_DEBUG")) : 0;
 }
 static void col_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
-    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline;
+    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = getenv("CWO_DEBUG") ? atoi(getenv("CWO_DEBUG")) : 0;
 }
 
 static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float2* ws) {
     PassParams pp; row_params(p, g, pp);
     pp.in = io.in; pp.in_amp = io.in_amp; pp.in_phase = io.in_phase; pp.in_mode = io.in_mode; pp.out = ws;
+    pp.use_tmap = (p->pipeline && encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, g.logwc, g.rb)) ? 1 : 0;
     return launch(p, g.logmx, ROW_FWD, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
 }
 static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const float2* ws, float scale) {
     PassParams pp; row_params(p, g, pp);
     pp.in = ws; pp.out = (float2*)io.out; pp.out_mode = io.out_mode; pp.out_amp = io.out_amp; pp.out_scale = scale;
+    pp.use_tmap = (p->pipeline && encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, g.logwc, g.rb)) ? 1 : 0;
     return launch(p, g.logmx, ROW_INV, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
 }
 

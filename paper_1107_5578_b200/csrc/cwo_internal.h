@@ -1,6 +1,7 @@
 // cwo_internal.h -- pass descriptors and launcher declarations shared by the translation units
 // of libcwo.so.  Not part of the public ABI (see include/cwo.h).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stddef.h>
 
@@ -11,6 +12,8 @@ enum OutMode { OUT_COMPLEX = 0, OUT_PHASOR_AMP = 1, OUT_PHASE = 2 };
 enum MidMode { MID_NONE = 0, MID_TABLES = 1, MID_ASM_SPLIT = 2, MID_ASM_F64 = 3 };
 
 struct PassParams {
+    CUtensorMap tmap;         // pipelined row passes: the column-tiled workspace as a 2-D tensor (see encode_ws_tmap)
+    int use_tmap;             // 1: tmap is valid, the row pass moves its workspace side with TMA tensor copies
     const float2* in;
     float2* out;              // OUT_PHASE: float*
     const float* in_amp;      // IN_AMP_PHASE: amplitude [rows][pitch]
@@ -22,6 +25,7 @@ struct PassParams {
     int ly;                   // rows kept in the column-tiled workspace
     int logwc;                // row passes: log2 of the column-tile width of the workspace
     int n_tiles;              // pipelined passes: total number of tiles (the grid is one CTA per SM)
+    int dbg;                  // experiment switches (CWO_DEBUG env): 1 no stores, 2 no transform, 4 no loads
     int use_pipe;             // 1: use the pipelined form where it exists (CWO_OPT_PIPELINE)
     const float2* tw;         // forward twiddles exp(-i 2 pi m/n), m < n
     float out_scale;          // ROW_INV store

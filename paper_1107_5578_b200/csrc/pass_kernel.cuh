@@ -14,6 +14,7 @@
 #pragma once
 #include "cwo_internal.h"
 #include "fft_core.cuh"
+#include "pp_core.cuh"
 
 namespace cwo {
 
@@ -21,6 +22,7 @@ enum { ROW_FWD = 0, ROW_INV = 1, COL_FWD = 2, COL_FUSED = 3, COL_MIDINV = 4 };
 
 struct MidNone {
     __device__ __forceinline__ void operator()(float2 (&)[2][16]) const {}
+    __device__ __forceinline__ void slot(float2 (&)[16], int) const {}
 };
 
 // Fresnel: FFT2 of the sampled separable chirp is the outer product Cx[k]*Cy[l] (S2, S7 folded in)
@@ -37,6 +39,13 @@ template <int LOGN> struct MidTables {
             v[0][e] = cconj(cmul(v[0][e], cmul(cx0, cy0)));
             v[1][e] = cconj(cmul(v[1][e], cmul(cx1, cy1)));
         }
+    }
+    // one slot at a time (pp_core.cuh); lane pairs only
+    __device__ __forceinline__ void slot(float2 (&x)[16], int s) const {
+        using C = Tile<LOGN>;
+        const float2 cx = __ldg(&P.tab_lane[lane0 + s]);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) x[e] = cconj(cmul(x[e], cmul(cx, __ldg(&P.tab_point[u[0] + e * C::Q]))));
     }
 };
 
@@ -74,6 +83,30 @@ template <int LOGN> struct MidAsmSplit {
                 __sincosf(6.283185307179586f * ph, &sn, &cs);
                 v[s][e] = cconj(cmul(v[s][e], make_float2(cs, sn)));
             }
+        }
+    }
+    // one slot at a time (pp_core.cuh); lane pairs only
+    __device__ __forceinline__ void slot(float2 (&x)[16], int s) const {
+        using C = Tile<LOGN>;
+        const float* thl = reinterpret_cast<const float*>(P.tab_lane);
+        const float* thp = reinterpret_cast<const float*>(P.tab_point);
+        const int lane = lane0 + s;
+        const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+        const float thx = __ldg(&thl[lane]);
+        const float sx = P.res_a * (float)ks * (float)ks;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int l = u[0] + e * C::Q;
+            const int ls = (l < C::N / 2) ? l : l - C::N;
+            const float sv = fmaf(P.res_b * (float)ls, (float)ls, sx);
+            const float om = 1.0f - sv;
+            const float r = 1.0f + om * rsqrtf(om);
+            const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
+            float ph = thx + __ldg(&thp[l]) - res;
+            ph -= rintf(ph);
+            float sn, cs;
+            __sincosf(6.283185307179586f * ph, &sn, &cs);
+            x[e] = cconj(cmul(x[e], make_float2(cs, sn)));
         }
     }
 };
@@ -356,7 +389,7 @@ static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) 
     constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
     if constexpr (pipe_supported(LOGN) && MID != MID_ASM_F64 &&
                   (!ROWPASS || (KIND == ROW_FWD && IOM == IN_COMPLEX) || (KIND == ROW_INV && IOM == OUT_COMPLEX))) {
-        if (p.use_pipe && (!ROWPASS || (p.logwc >= 1 && p.rows % Tile<LOGN>::W == 0)))
+        if (p.use_pipe && (!ROWPASS || (p.use_tmap && p.rows % Tile<LOGN>::W == 0)))
             return launch_pipe<LOGN, KIND, PAD, MID, IOM>(n_tiles, s, p);
     }
     if constexpr ((KIND == ROW_FWD || KIND == ROW_INV) && Tile<LOGN>::W == 2) {

@@ -1,12 +1,13 @@
-// pipe_kernel.cuh -- the streaming passes of pass_kernel.cuh as ONE persistent CTA per SM that keeps
-// three tiles in flight: two 256-thread groups transform alternate tiles while the next tiles are
-// already on their way from HBM into the third shared-memory buffer (cp.async.bulk / cp.async signalled
-// through mbarriers).  Global loads therefore never stall the butterflies, and HBM always has ~64-128 KB
-// of requests outstanding per SM.  Results leave straight from registers (128-bit stores).
-//
-//   tile j of this CTA = blockIdx.x + j * gridDim.x, handled by group j % 2 in buffer j % 3.
-//   When a group has finished with the shared-memory image of tile j it issues the load of tile j + 3
-//   into the same buffer (the other group will consume it), then stores its results.
+// pipe_kernel.cuh -- the streaming passes of pass_kernel.cuh as ONE persistent, warp-specialised CTA per
+// SM that keeps three tiles in flight in three shared-memory buffers:
+//   * two 256-thread consumer groups transform alternate tiles (tile j of this CTA = blockIdx.x +
+//     j * gridDim.x, group j % 2, buffer j % 3); they touch global memory only for twiddles/tables;
+//   * one producer warp moves every tile: TMA bulk / tensor loads into a buffer (mbarrier full[b]),
+//     and, once the group has written its results back into the same buffer in the layout of the
+//     destination (mbarrier staged[b]), TMA bulk / tensor stores out of it, then the load of tile j + 3.
+// HBM therefore always has 64-192 KB of requests outstanding per SM, none of them waiting on a
+// butterfly, and the 32-byte scatter/gather of the column-tiled workspace never occupies the SM's
+// load/store path.
 //
 // Same arithmetic and the same tile/unit mapping as pass_kernel.cuh (S3-S10 of SURVEY.md section 8(a));
 // row passes always use the unit-pair mapping at the workspace side.
@@ -51,17 +52,43 @@ __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
 __device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// shared -> global tensor store of one box (2-D), bulk-group completion
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, const void* src, int c0, int c1) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(m),
+                 "r"(smem_u32(src)), "r"(c0), "r"(c1)
+                 : "memory");
+}
+// global -> shared tensor load of one box (2-D), completion counted in bytes on the mbarrier
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* m, int c0, int c1, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+            smem_u32(dst)),
+        "l"(m), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+        : "memory");
+}
+// shared -> global bulk copy (contiguous), bulk-group completion
+__device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+// all bulk stores of this thread have finished READING shared memory
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 // order this thread's generic-proxy accesses to shared memory before later async-proxy (bulk copy) writes
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 template <int LOGN, int KIND> struct PipeCfg {
     using C = Tile<LOGN>;
     static constexpr int GROUPS = 2, NBUF = 3, GT = 256;
+    static constexpr int THREADS = GROUPS * GT + 128;        // + the producer warpgroup (one working lane)
     static constexpr size_t BUF_RAW = (KIND == ROW_FWD && C::SMEM_BYTES_X > C::SMEM_BYTES) ? C::SMEM_BYTES_X : C::SMEM_BYTES;
     static constexpr size_t BUF = (BUF_RAW + 127) / 128 * 128;
     static constexpr size_t SMEM = NBUF * BUF + 64;
-    static constexpr bool CPASYNC = (KIND == ROW_INV);       // gather of 16-byte pieces; else bulk copies
-    // ROW_FWD staging: row r of the tile at element r * (points + ROWPAD) (bank stagger between lane pairs)
+    // row-major staging (ROW_FWD in, ROW_INV out): row r of the tile at element r * (points + ROWPAD)
+    // (bank stagger between lane pairs)
     static constexpr int ROWPAD = C::W > 2 ? 16 / C::W : 0;
 };
 
@@ -69,73 +96,94 @@ template <int LOGN, int KIND> struct PipeCfg {
 // lane pairs, W <= 8 (transform lengths 1024..4096): pipe_supported() in pass_kernel.cuh.
 
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
-__global__ void __launch_bounds__(512, 1) pipe_kernel(const __grid_constant__ PassParams P) {
+__global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(const __grid_constant__ PassParams P) {
     using C = Tile<LOGN>;
     using K = PipeCfg<LOGN, KIND>;
     static_assert(C::T == K::GT && C::PAIR && C::W <= 8, "tile shape");
     constexpr int W = C::W, Q = C::Q, N = C::N;
     constexpr int NE = PAD ? 8 : 16;           // PAD: points >= n/2 are zero on load / dropped on store
     constexpr int NP = PAD ? N / 2 : N;        // points per lane that exist in memory at the padded side
+    constexpr int RS = NP + K::ROWPAD;         // row stride of the row-major staging
     extern __shared__ __align__(128) unsigned char smraw[];
-    uint64_t* full = reinterpret_cast<uint64_t*>(smraw + K::NBUF * K::BUF);
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw + K::NBUF * K::BUF);   // tile landed in buffer b
+    uint64_t* staged = full + K::NBUF;                                        // results written back to buffer b
 
-    const int g = threadIdx.x >> 8, t = threadIdx.x & 255;
-    const SyncGroup sync{1 + g};
     const int nt = (P.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this CTA
+    const bool no_st = P.dbg & 1, no_ld = P.dbg & 4;
 
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int b = 0; b < K::NBUF; ++b) mbar_init(&full[b], K::CPASYNC ? K::GT : 1);
+        for (int b = 0; b < K::NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&staged[b], K::GT); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    // ---- load of tile j into buffer j % 3 (called by all 256 threads of one group) -------------------
-    auto issue = [&](int j) {
-        const int b = j % K::NBUF;
-        const int tile = blockIdx.x + j * gridDim.x;
-        unsigned char* dst = smraw + b * K::BUF;
-        if constexpr (KIND == ROW_FWD) {
-            // W rows of the row-major field, NP points each
-            if (t == 0) {
+    if (threadIdx.x >= K::GROUPS * K::GT) {
+        // ================================ producer warp (one lane) ================================
+        // the producer warpgroup hands its registers to the consumers (the CTA pool is 640 x 96: 512 x 112 + 128 x 24)
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (threadIdx.x != K::GROUPS * K::GT) return;
+        const int wc = 1 << P.logwc;
+        const int groups = N >> P.logwc, bg = groups < 256 ? groups : 256;    // column groups per TMA box
+        auto load = [&](int j) {
+            if (no_ld) return;
+            const int b = j % K::NBUF;
+            const int tile = blockIdx.x + j * gridDim.x;
+            unsigned char* dst = smraw + b * K::BUF;
+            if constexpr (KIND == ROW_FWD) {               // W rows of the row-major field, NP points each
                 mbar_expect_tx(&full[b], W * NP * 8);
 #pragma unroll
                 for (int r = 0; r < W; ++r)
-                    bulk_g2s(dst + (size_t)r * (NP + K::ROWPAD) * 8, P.in + (size_t)(tile * W + r) * P.pitch, NP * 8,
-                             &full[b]);
-            }
-        } else if constexpr (KIND == ROW_INV) {
-            // rows tile*W .. +W-1 of the column-tiled workspace: thread (w, i) fetches the 16-byte pieces
-            // (points 2i + e*Q, +1 of row w) it will consume itself
-            const int w = t % W, i2 = 2 * (t / W);
-            const int row = tile * W + w;
-            const int wcm = (1 << P.logwc) - 1;
-#pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                const int x = i2 + e * Q;
-                const size_t a = (((size_t)(x >> P.logwc) * P.ly + row) << P.logwc) + (x & wcm);
-                cp_async16(dst + (size_t)(e * K::GT + t) * 16, P.in + a);
-            }
-            cp_async_arrive(&full[b]);
-        } else {
-            // column tile: one contiguous [ly][W] block
-            if (t == 0) {
+                    bulk_g2s(dst + (size_t)r * RS * 8, P.in + (size_t)(tile * W + r) * P.pitch, NP * 8, &full[b]);
+            } else if constexpr (KIND == ROW_INV) {        // W rows of the column-tiled workspace: [x/Wc][row][x%Wc]
+                mbar_expect_tx(&full[b], W * N * 8);
+                for (int c = 0; c < groups; c += bg)
+                    tma_load_2d(dst + (size_t)c * W * wc * 8, &P.tmap, tile * W * wc * 2, c, &full[b]);
+            } else {                                       // column tile: one contiguous [ly][W] block
                 const uint32_t bytes = (uint32_t)P.ly * W * 8;
                 mbar_expect_tx(&full[b], bytes);
                 const unsigned char* src = reinterpret_cast<const unsigned char*>(P.in + (size_t)tile * P.ly * W);
                 constexpr uint32_t CH = 16384;
                 for (uint32_t o = 0; o < bytes; o += CH) bulk_g2s(dst + o, src + o, bytes - o < CH ? bytes - o : CH, &full[b]);
             }
+        };
+        auto store = [&](int j) {
+            if (no_st) return;
+            const int b = j % K::NBUF;
+            const int tile = blockIdx.x + j * gridDim.x;
+            unsigned char* src = smraw + b * K::BUF;
+            if constexpr (KIND == ROW_FWD) {
+                for (int c = 0; c < groups; c += bg)
+                    tma_store_2d(&P.tmap, src + (size_t)c * W * wc * 8, tile * W * wc * 2, c);
+            } else if constexpr (KIND == ROW_INV) {        // W rows of the row-major field, NP points each
+#pragma unroll
+                for (int r = 0; r < W; ++r)
+                    bulk_s2g(P.out + (size_t)(tile * W + r) * P.pitch, src + (size_t)r * RS * 8, NP * 8);
+            } else {
+                const uint32_t bytes = (uint32_t)P.ly * W * 8;
+                unsigned char* dst = reinterpret_cast<unsigned char*>(P.out + (size_t)tile * P.ly * W);
+                constexpr uint32_t CH = 16384;
+                for (uint32_t o = 0; o < bytes; o += CH) bulk_s2g(dst + o, src + o, bytes - o < CH ? bytes - o : CH);
+            }
+            bulk_commit();
+        };
+        for (int j = 0; j < nt && j < K::NBUF; ++j) load(j);
+        for (int j = 0; j < nt; ++j) {
+            mbar_wait(&staged[j % K::NBUF], (j / K::NBUF) & 1);
+            store(j);
+            if (j + K::NBUF < nt) {
+                bulk_wait_read();                          // the stores have read the buffer
+                load(j + K::NBUF);
+            }
         }
-    };
-
-    if (g == 0) {
-        if (nt > 0) issue(0);
-        if (nt > 2) issue(2);
-    } else {
-        if (nt > 1) issue(1);
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        return;
     }
 
+    // ===================================== consumer groups =====================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    const int g = threadIdx.x >> 8, t = threadIdx.x & 255;
+    const SyncGroup sync{1 + g};
     const int us = t / (W / 2), w0 = 2 * (t % (W / 2));     // standard mapping: unit us, lanes w0, w0+1
     const int u[2] = {us, us};
     const int xw = t % W, xi2 = 2 * (t / W);                // unit-pair mapping: lane xw, units xi2, xi2+1
@@ -146,7 +194,7 @@ __global__ void __launch_bounds__(512, 1) pipe_kernel(const __grid_constant__ Pa
         const int tile = blockIdx.x + j * gridDim.x;
         float2* sm = reinterpret_cast<float2*>(smraw + b * K::BUF);
         float2 v[2][16];
-        mbar_wait(&full[b], (j / K::NBUF) & 1);
+        if (!no_ld) mbar_wait(&full[b], (j / K::NBUF) & 1);
 
         // ---- registers <- staged tile ------------------------------------------------------------
         if constexpr (KIND == ROW_FWD) {
@@ -154,11 +202,13 @@ __global__ void __launch_bounds__(512, 1) pipe_kernel(const __grid_constant__ Pa
             for (int s = 0; s < 2; ++s)
 #pragma unroll
                 for (int e = 0; e < 16; ++e)
-                    v[s][e] = (e < NE) ? sm[(w0 + s) * (NP + K::ROWPAD) + us + e * Q] : make_float2(0.f, 0.f);
+                    v[s][e] = (e < NE) ? sm[(w0 + s) * RS + us + e * Q] : make_float2(0.f, 0.f);
         } else if constexpr (KIND == ROW_INV) {
+            // [x/Wc][row][x%Wc]: points (x, x+1) of row xw, x = xi2 + e*Q, are 16 bytes
+            const float2* src = sm + ((((xi2 >> P.logwc) * W + xw) << P.logwc) + (xi2 & ((1 << P.logwc) - 1)));
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
-                const float4 t4 = reinterpret_cast<const float4*>(sm)[e * K::GT + t];
+                const float4 t4 = *reinterpret_cast<const float4*>(src + e * Q * W);
                 v[0][e] = make_float2(t4.x, -t4.y); v[1][e] = make_float2(t4.z, -t4.w);
             }
         } else {
@@ -173,58 +223,99 @@ __global__ void __launch_bounds__(512, 1) pipe_kernel(const __grid_constant__ Pa
             }
         }
 
-        // ---- transform (the first barrier inside also retires the staged image) ------------------
+        // ---- transform: ping-pong schedule of pp_core.cuh ----------------------------------------------
         const int lane0 = tile * W + w0;
+        constexpr int M = C::M, L0 = C::L0;
+        float2* rgA = sm;
+        float2* rgB = sm + PP<LOGN>::REGION;
+        const int wh = w0 >> 1;
         if constexpr (KIND == ROW_FWD) {
-            transform_fwd_xlast<LOGN>(v, t, sm, P.tw, sync);
+            sync();                                           // staged image retired
+            pp_run<LOGN, true, 0, M - 1, false, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
+            // stage M-2 -> one plane per lane, read back unit pairs, last stage in unit-pair mapping
+            constexpr int lns = L0 + 4 * (M - 2);
+            sync();
+            {
+                const int j0 = ((us >> lns) << (lns + 4)) + (us & ((1 << lns) - 1));
+                float2* pl = sm + w0 * C::XPLANE;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const int p = j0 + (q << lns), pi = p + 2 * (p >> 4);
+                    pl[pi] = v[0][perm<16>(q)];
+                    pl[C::XPLANE + pi] = v[1][perm<16>(q)];
+                }
+            }
+            sync();
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                const int p = xi2 + e * Q;
+                const float4 x = *reinterpret_cast<const float4*>(&sm[xw * C::XPLANE + p + 2 * (p >> 4)]);
+                v[0][e] = make_float2(x.x, x.y);
+                v[1][e] = make_float2(x.z, x.w);
+            }
+            const int ux[2] = {xi2, xi2 + 1};
+            butterflies<LOGN, 4, true>(v, ux, L0 + 4 * (M - 1), P.tw);
+            unpermute<16>(v[0]); unpermute<16>(v[1]);
         } else if constexpr (KIND == ROW_INV) {
-            transform_inv_xfirst<LOGN>(v, t, sm, P.tw, sync);
+            dft16(v[0]); dft16(v[1]);                         // unit-pair mapping, Ns = 1: no twiddles
+            sync();
+            {
+                float2* rg = (xw & 1) ? rgB : rgA;
+#pragma unroll
+                for (int s = 0; s < 2; ++s)
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) rg[ridx<LOGN>(16 * (xi2 + s) + q, xw >> 1)] = v[s][perm<16>(q)];
+            }
+            sync();
+            lds_slot<LOGN>(v[0], us, wh, rgA);
+            lds_slot<LOGN>(v[1], us, wh, rgB);
+            sync();                                           // regions free again for pp_run
+            pp_run<LOGN, false, M + 1, 2 * M, true, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
+            if constexpr (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); }
         } else if constexpr (KIND == COL_FWD) {
-            transform<LOGN, true, false>(v, u, w0, sm, P.tw, MidNone(), sync);
+            sync();
+            pp_run<LOGN, true, 0, M, false, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
+            unpermute<16>(v[0]); unpermute<16>(v[1]);
         } else {
             typename MidSelect<LOGN, MID>::type mid{P, u, lane0, sm};
             if constexpr (KIND == COL_FUSED) {
-                transform<LOGN, true, true>(v, u, w0, sm, P.tw, mid, sync);
+                sync();
+                pp_run<LOGN, true, 0, 2 * M, true, true>(v, us, wh, rgA, rgB, P.tw, mid, sync);
             } else {
                 mid(v);
-                transform<LOGN, false, true>(v, u, w0, sm, P.tw, MidNone(), sync);
+                sync();
+                pp_run<LOGN, false, M, 2 * M, true, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
             }
+            if constexpr (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); }
         }
 
-        // ---- this buffer is free: fetch tile j + 3 into it ----------------------------------------
-        fence_proxy_async();
-        sync();
-        if (j + K::NBUF < nt) issue(j + K::NBUF);
-
-        // ---- store (conj completes an inverse transform) ------------------------------------------
+        // ---- results -> the same buffer, in the layout of the destination; the producer stores them ----
+        sync();                                               // nobody still reads the exchange regions
         if constexpr (KIND == ROW_FWD) {
-            const int row = tile * W + xw;
-            const int wcm = (1 << P.logwc) - 1;
+            // [x/Wc][row][x%Wc]; register e of slot s <-> point xi2 + s + e*Q of row xw
+            float2* d = sm + ((((xi2 >> P.logwc) * W + xw) << P.logwc) + (xi2 & ((1 << P.logwc) - 1)));
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                const int x = xi2 + e * Q;
-                const size_t a = (((size_t)(x >> P.logwc) * P.ly + row) << P.logwc) + (x & wcm);
-                *reinterpret_cast<float4*>(&P.out[a]) = make_float4(v[0][e].x, v[0][e].y, v[1][e].x, v[1][e].y);
-            }
+            for (int e = 0; e < 16; ++e)
+                *reinterpret_cast<float4*>(d + e * Q * W) = make_float4(v[0][e].x, v[0][e].y, v[1][e].x, v[1][e].y);
         } else if constexpr (KIND == ROW_INV) {
             static_assert(IOM == OUT_COMPLEX, "GS store modes run in pass_kernel");
-            const float sc = P.out_scale;
+            const float sc = P.out_scale;                     // conj completes the inverse transform
 #pragma unroll
-            for (int s = 0; s < 2; ++s) {
-                float2* dst = P.out + (size_t)(tile * W + w0 + s) * P.pitch + us;
+            for (int s = 0; s < 2; ++s)
 #pragma unroll
-                for (int e = 0; e < NE; ++e) dst[e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
-            }
+                for (int e = 0; e < NE; ++e)
+                    sm[(w0 + s) * RS + us + e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
         } else {
-            float2* dst = P.out + (size_t)tile * P.ly * W;
             constexpr bool CONJ = (KIND != COL_FWD);
 #pragma unroll
             for (int e = 0; e < NE; ++e) {
                 const float2 a = v[0][e], c = v[1][e];
-                *reinterpret_cast<float4*>(&dst[(size_t)(us + e * Q) * W + w0]) =
+                *reinterpret_cast<float4*>(&sm[(us + e * Q) * W + w0]) =
                     CONJ ? make_float4(a.x, -a.y, c.x, -c.y) : make_float4(a.x, a.y, c.x, c.y);
             }
         }
+        fence_proxy_async();
+        mbar_arrive(&staged[b]);
     }
 }
 
@@ -249,7 +340,7 @@ static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p)
     PassParams q = p;
     q.n_tiles = n_tiles;
     const int grid = n_tiles < n_sm ? n_tiles : n_sm;
-    pipe_kernel<LOGN, KIND, PAD, MID, IOM><<<grid, 512, K::SMEM, s>>>(q);
+    pipe_kernel<LOGN, KIND, PAD, MID, IOM><<<grid, K::THREADS, K::SMEM, s>>>(q);
     return cudaGetLastError();
 }
 
