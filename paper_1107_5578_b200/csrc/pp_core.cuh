@@ -108,11 +108,15 @@ __device__ __forceinline__ void pp_run(float2 (&v)[2][16], int us, int wh, float
         const int sn = s + (merge ? 2 : 1);
         const bool has_next = (sn < SB) || (INV_SMALL && L0 > 0);
         const int lns_out = merge ? 0 : lns;
-        float2 w[16];
-        if (lns > 0) powers<16>(__ldg(&tw[(us & ((1 << lns) - 1)) << (LOGN - lns - 4)]), w);
+        const float2 w1 = __ldg(&tw[(us & ((1 << lns) - 1)) << (LOGN - lns - 4)]);
 #pragma unroll
         for (int sl = 0; sl < 2; ++sl) {
-            if (lns > 0) apply_powers<16>(v[sl], 0, w);
+            if (lns > 0) {
+                // powers rebuilt per slot: 15 fewer live complex registers across the exchange of the other slot
+                float2 w[16];
+                powers<16>(w1, w);
+                apply_powers<16>(v[sl], 0, w);
+            }
             dft16(v[sl]);
             if (merge) {
                 unpermute<16>(v[sl]);
