@@ -169,7 +169,7 @@ def run_reference(args):
 
 def run_cuda(args):
     import torch
-    from paper_1107_5578_b200 import api, workloads as W
+    from paper_1107_5578_b200 import api, sharding as S, workloads as W
 
     rank, world, local = _dist()
     if not torch.cuda.is_available():
@@ -220,11 +220,8 @@ def run_cuda(args):
     ms = e0.elapsed_time(e1)
     launches = plan.launch_count - l0
     clocks = sampler.stop() if rank == 0 else None
-    if use_dist:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * args.steps / (ms * 1e-3)
+    ms = S.max_over_ranks(ms, device="cuda")
+    value = S.whole_job_rate([args.steps] * world, ms)
 
     # ---- per-kernel durations (library-recorded CUDA events on the same stream) -------------------
     plan.set_option(api.CWO_OPT_TIMING, 1)
@@ -269,11 +266,8 @@ def run_cuda(args):
     e1.record(stream)
     barrier()
     ms_e2e = e0.elapsed_time(e1)
-    if use_dist:
-        t = torch.tensor([ms_e2e], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_e2e = float(t.item())
-    e2e = {"value": world * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT, "steps": e2e_steps,
+    ms_e2e = S.max_over_ranks(ms_e2e, device="cuda")
+    e2e = {"value": S.whole_job_rate([e2e_steps] * world, ms_e2e), "unit": UNIT, "steps": e2e_steps,
            "h2d_bytes_per_step": int(d_in.numel() * 8), "d2h_bytes_per_step": int(d_out.numel() * 8)}
 
     if rank == 0:
