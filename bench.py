@@ -164,6 +164,119 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------------
+# workloads: c3 is the headline (BASELINE.json); the others time the same C-ABI calls on other configs
+# ------------------------------------------------------------------------------------------------------
+
+WORKLOADS = {"c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
+             "c2": ("fresnel", 1024), "fresnel2048": ("fresnel", 2048), "fresnel4096": ("fresnel", 4096),
+             "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c5": ("gs", 8192)}
+
+
+def make_workload(name, rank, torch, api, W):
+    """Device-resident inputs, the step function and the algorithmic byte counts of a workload."""
+    op, N = WORKLOADS[name]
+    NBUF = 3
+    n2 = float(N) * N
+    if op in ("asm", "fresnel"):
+        base = W.CONFIGS["c3"] if op == "asm" else (W.CONFIGS["c2"] if N <= 2048 else W.CONFIGS["c5"])
+        zs = base.zs if op == "asm" else (base.zs[0], 1.07 * base.zs[0], 0.93 * base.zs[0])
+        hosts = [W.field_c3(W.Config(name, op, N, base.lam, base.pitch, zs, index=base.index + 100 * (i + rank * NBUF)))
+                 for i in range(NBUF)]
+        u1 = [torch.from_numpy(h).cuda() for h in hosts]
+        u2 = [torch.empty_like(u1[0]) for _ in range(NBUF)]
+        plan = api.cwo_plan(N, N, base.pitch, base.lam)
+        call = api.cwo_asm if op == "asm" else api.cwo_fresnel_conv
+        plan.ensure_workspace(api.CWO_OP_ASM if op == "asm" else api.CWO_OP_FRESNEL)
+
+        def step(i):
+            call(plan, u1[i % NBUF], u2[i % NBUF], zs[i % len(zs)])
+
+        def e2e():
+            pin_in = [torch.from_numpy(h).pin_memory() for h in hosts]
+            pin_out = torch.empty((N, N), dtype=torch.complex64).pin_memory()
+            d_in, d_out = torch.empty_like(u1[0]), torch.empty_like(u1[0])
+
+            def f(i):
+                d_in.copy_(pin_in[i % NBUF], non_blocking=True)
+                call(plan, d_in, d_out, zs[i % len(zs)])
+                pin_out.copy_(d_out, non_blocking=True)
+            return f, 8 * n2, 8 * n2
+        if op == "asm":
+            kb = {0: 16 * n2, 3: 16 * n2, 1: 16 * n2}
+            bps = 48 * n2
+            desc = ("%s: ASM %dx%d complex64 speckle field, lambda %g nm, pitch %g um, z cycling %s m (new z every call)"
+                    % (name, N, N, base.lam * 1e9, base.pitch * 1e6, "{" + ",".join("%g" % z for z in zs) + "}"))
+        else:
+            kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2}       # R: 8 rd + 16 wr; C: 16 + 16; R': 16 rd + 8 wr
+            bps = 80 * n2
+            desc = ("%s: Fresnel convolution %dx%d complex64 speckle field (virtual %dx%d), lambda %g nm, pitch %g um, "
+                    "z cycling %s m (new z every call)" % (name, N, N, 2 * N, 2 * N, base.lam * 1e9, base.pitch * 1e6,
+                                                           "{" + ",".join("%.4g" % z for z in zs) + "}"))
+        ws = (24 if op == "asm" else 32) * n2             # u1 + u2 + workspace touched per step
+        l2 = ("working set %.0f MB per step, rotating over 3 field pairs (%s the 126 MB L2); no flush"
+              % (ws / 1e6, "larger than" if ws > 126e6 else "FITS in"))
+        return dict(plan=plan, step=step, N=N, props_per_step=1, bytes_per_step=bps, kind_bytes=kb, e2e=e2e, desc=desc,
+                    l2=l2, metric="propagations/sec (%s); effective HBM GB/s for the algorithmic bytes" % name)
+    if op == "stack":
+        cfg = W.CONFIGS["c4"]
+        n = len(cfg.zs)
+        host = W.make_field(cfg)
+        u1 = torch.from_numpy(host).cuda()
+        out = torch.empty((n, N, N), dtype=torch.complex64, device="cuda")
+        plan = api.cwo_plan(N, N, cfg.pitch, cfg.lam)
+        plan.ensure_workspace(api.CWO_OP_STACK, n)
+
+        def step(i):
+            api.cwo_propagate_stack(plan, u1, cfg.zs, out)
+
+        def e2e():
+            pin_in = torch.from_numpy(host).pin_memory()
+            pin_out = torch.empty((n, N, N), dtype=torch.complex64).pin_memory()
+            d_in = torch.empty_like(u1)
+
+            def f(i):
+                d_in.copy_(pin_in, non_blocking=True)
+                api.cwo_propagate_stack(plan, d_in, cfg.zs, out)
+                pin_out.copy_(out, non_blocking=True)
+            return f, 8 * n2, 8 * n2 * n
+        return dict(plan=plan, step=step, N=N, props_per_step=n, bytes_per_step=32 * n2 + n * 32 * n2,
+                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: 16 * n2, 1: 16 * n2}, e2e=e2e,
+                    desc="c4: depth stack, one 2048x2048 random-phase field to 64 planes z = 1..64 mm by ASM, lambda 633 nm, "
+                         "pitch 6.4 um, out 64x2048x2048 complex64",
+                    l2="spectrum (34 MB) stays in L2; the 2.1 GB output stack streams to HBM; no flush",
+                    metric="planes/sec (c4 depth stack); effective HBM GB/s for 32 N^2 + n 32 N^2 bytes")
+    cfg = W.CONFIGS["c5"]
+    a_src, a_dst, phi0 = W.gs_inputs_c5(cfg)
+    d_src, d_dst = torch.from_numpy(a_src).cuda(), torch.from_numpy(a_dst).cuda()
+    d_phi0 = torch.from_numpy(phi0).cuda()
+    d_phi = torch.empty_like(d_phi0)
+    plan = api.cwo_plan(N, N, cfg.pitch, cfg.lam)
+    plan.ensure_workspace(api.CWO_OP_GS)
+
+    def step(i):
+        d_phi.copy_(d_phi0)
+        api.cwo_gs(plan, d_src, d_dst, cfg.zs[0], cfg.iters, d_phi)
+
+    def e2e():
+        pins = [torch.from_numpy(x).pin_memory() for x in (a_src, a_dst, phi0)]
+        pin_out = torch.empty((N, N), dtype=torch.float32).pin_memory()
+
+        def f(i):
+            d_src.copy_(pins[0], non_blocking=True); d_dst.copy_(pins[1], non_blocking=True)
+            d_phi.copy_(pins[2], non_blocking=True)
+            api.cwo_gs(plan, d_src, d_dst, cfg.zs[0], cfg.iters, d_phi)
+            pin_out.copy_(d_phi, non_blocking=True)
+        return f, 12 * n2, 4 * n2
+    props = 2 * cfg.iters + 1
+    return dict(plan=plan, step=step, N=N, props_per_step=props, bytes_per_step=cfg.iters * 168 * n2 + 84 * n2,
+                kind_bytes={0: 24 * n2, 3: 32 * n2, 1: 28 * n2}, e2e=e2e,
+                desc="c5: Gerchberg-Saxton, 8192x8192, Fresnel convolution forward/back, lambda 532 nm, pitch 3.74 um, z 0.3 m, "
+                     "20 iterations (41 propagations per call)",
+                l2="537 MB field + 1074 MB workspace per propagation (>> 126 MB L2); no flush",
+                metric="propagations/sec inside cwo_gs (c5, 41 per call); effective HBM GB/s for 168 N^2 bytes per iteration")
+
+
+# ------------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ------------------------------------------------------------------------------------------------------
 
@@ -185,22 +298,10 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg = W.CONFIGS["c3"]
-    N, zs = cfg.N, cfg.zs
+    wl = make_workload(args.workload, rank, torch, api, W)
+    plan, step, N = wl["plan"], wl["step"], wl["N"]
     NBUF = 3
-    # three independent seeded fields (one per z) so successive steps never re-read the previous step's data
-    host_fields = []
-    for i in range(NBUF):
-        c = W.Config(cfg.name, cfg.op, cfg.N, cfg.lam, cfg.pitch, cfg.zs, index=cfg.index + 100 * (i + rank * NBUF))
-        host_fields.append(W.field_c3(c))
-    u1 = [torch.from_numpy(h).cuda() for h in host_fields]
-    u2 = [torch.empty_like(u1[0]) for _ in range(NBUF)]
-    plan = api.cwo_plan(N, N, cfg.pitch, cfg.lam)
-    plan.ensure_workspace(api.CWO_OP_ASM)
     stream = torch.cuda.current_stream()
-
-    def step(i):
-        api.cwo_asm(plan, u1[i % NBUF], u2[i % NBUF], zs[i % len(zs)])
 
     # ---- device-resident timing -----------------------------------------------------------------
     for i in range(max(args.warmup, 3)):
@@ -221,11 +322,11 @@ def run_cuda(args):
     launches = plan.launch_count - l0
     clocks = sampler.stop() if rank == 0 else None
     ms = S.max_over_ranks(ms, device="cuda")
-    value = S.whole_job_rate([args.steps] * world, ms)
+    value = S.whole_job_rate([args.steps * wl["props_per_step"]] * world, ms)
 
     # ---- per-kernel durations (library-recorded CUDA events on the same stream) -------------------
     plan.set_option(api.CWO_OPT_TIMING, 1)
-    reps = min(max(args.steps, 6), 60)
+    reps = min(max(args.steps, 6), 60) if wl["props_per_step"] == 1 else 2
     for i in range(reps):
         step(i)
     tm = plan.timings()
@@ -233,28 +334,23 @@ def run_cuda(args):
     per_kind = {}
     for tag, t_ms in tm:
         per_kind.setdefault(tag & 15, []).append(t_ms)
-    names = {0: "pass_R (row FFT)", 3: "pass_C (fused column FFT*H*IFFT)", 1: "pass_R' (row IFFT)"}
+    names = {0: "pass_R (row FFT)", 1: "pass_R' (row IFFT)", 2: "pass_C0 (column FFT)",
+             3: "pass_C (fused column FFT*H*IFFT)", 4: "pass_C' (H * column IFFT)"}
     passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
-    dom_kind = max(per_kind, key=lambda k: np.mean(per_kind[k]))
+    dom_kind = max(per_kind, key=lambda k: np.sum(per_kind[k]))
     dom_ms = float(np.mean(per_kind[dom_kind]))
     peak, peak_src = _peak()
-    alg_bytes = 16.0 * N * N                      # each pass reads 8 and writes 8 bytes per sample
+    alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves
     achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = _ncu_traffic({0: "pass_R", 1: "pass_Rinv", 3: "pass_C"}[dom_kind])
+    traffic = _ncu_traffic({0: "pass_R", 1: "pass_Rinv", 3: "pass_C"}.get(dom_kind, "-")) if args.workload == "c3" else None
+    tot = sum(float(np.sum(v)) for v in per_kind.values())
     roofline = {"bound": "hbm", "kernel": names[dom_kind], "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms,
-                "pass_ms": passes, "step_share": dom_ms / sum(passes.values())}
+                "pass_ms": passes, "step_share": float(np.sum(per_kind[dom_kind])) / tot}
 
     # ---- end to end: host (pinned) buffers, H2D + propagate + D2H every step -----------------------
-    pin_in = [torch.from_numpy(h).pin_memory() for h in host_fields]
-    pin_out = torch.empty((N, N), dtype=torch.complex64).pin_memory()
-    d_in, d_out = torch.empty_like(u1[0]), torch.empty_like(u1[0])
-
-    def e2e_step(i):
-        d_in.copy_(pin_in[i % NBUF], non_blocking=True)
-        api.cwo_asm(plan, d_in, d_out, zs[i % len(zs)])
-        pin_out.copy_(d_out, non_blocking=True)
+    e2e_step, h2d, d2h = wl["e2e"]()
 
     e2e_steps = max(3, min(args.steps, 20))
     for i in range(3):
@@ -267,24 +363,22 @@ def run_cuda(args):
     barrier()
     ms_e2e = e0.elapsed_time(e1)
     ms_e2e = S.max_over_ranks(ms_e2e, device="cuda")
-    e2e = {"value": S.whole_job_rate([e2e_steps] * world, ms_e2e), "unit": UNIT, "steps": e2e_steps,
-           "h2d_bytes_per_step": int(d_in.numel() * 8), "d2h_bytes_per_step": int(d_out.numel() * 8)}
+    e2e = {"value": S.whole_job_rate([e2e_steps * wl["props_per_step"]] * world, ms_e2e), "unit": UNIT, "steps": e2e_steps,
+           "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
 
     if rank == 0:
         ms_step = ms / args.steps
-        eff = 48.0 * N * N / (ms_step * 1e-3) / 1e9
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-                "config": {"workload": "c3: ASM 4096x4096 complex64 speckle field, lambda 633 nm, pitch 4 um, "
-                                       "z cycling {0.01,0.1,0.5} m (new z every call)",
-                           "l2": "working set 3 x 134 MB per step, rotating over 3 field pairs (> 126 MB L2); no flush",
+        eff = wl["bytes_per_step"] / (ms_step * 1e-3) / 1e9
+        line = {"metric": METRIC if args.workload == "c3" else wl["metric"], "value": value, "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": wl["desc"], "l2": wl["l2"],
                            "parallelism": "replicas" if world > 1 else "single GPU",
-                           "bytes_per_propagation": 48 * N * N},
+                           "bytes_per_step": int(wl["bytes_per_step"]), "propagations_per_step": wl["props_per_step"]},
                 "effective_gbs": eff, "pct_of_8TBs": 100.0 * eff / NOMINAL_HBM_GBS, "pct_of_measured_copy": 100.0 * eff / peak,
                 "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
-        if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(cfg)
+        if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
+            line["cpu_baseline"] = cpu_baseline(W.CONFIGS["c3"])
         print(json.dumps(line), flush=True)
     if use_dist:
         dist.destroy_process_group()
@@ -297,6 +391,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="c3", choices=sorted(WORKLOADS),
+                    help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -205,7 +205,7 @@ __device__ __forceinline__ void exchange(float2 (&v)[2][16], const int (&u)[2], 
 }
 
 // Twiddle (if lns > 0) and butterflies of one radix-2^LR stage on both slots.
-template <int LOGN, int LR, bool SEP = !Tile<LOGN>::PAIR>
+template <int LOGN, int LR, bool SEP = !Tile<LOGN>::PAIR, bool TW_SHARED = false>
 __device__ __forceinline__ void butterflies(float2 (&v)[2][16], const int (&u)[2], int lns,
                                             const float2* __restrict__ tw) {
     using C = Tile<LOGN>;
@@ -215,11 +215,11 @@ __device__ __forceinline__ void butterflies(float2 (&v)[2][16], const int (&u)[2
         if (lns > 0) {
             float2 w[16];
             const int k0 = (u[0] + i * C::Q) & ((1 << lns) - 1);
-            powers<R>(__ldg(&tw[k0 << (LOGN - lns - LR)]), w);
+            powers<R>(TW_SHARED ? tw[k0 << (LOGN - lns - LR)] : __ldg(&tw[k0 << (LOGN - lns - LR)]), w);
             apply_powers<R>(v[0], i, w);
             if constexpr (SEP) {                  // the two slots are different units: own twiddles
                 const int k1 = (u[1] + i * C::Q) & ((1 << lns) - 1);
-                powers<R>(__ldg(&tw[k1 << (LOGN - lns - LR)]), w);
+                powers<R>(TW_SHARED ? tw[k1 << (LOGN - lns - LR)] : __ldg(&tw[k1 << (LOGN - lns - LR)]), w);
             }
             apply_powers<R>(v[1], i, w);
         }

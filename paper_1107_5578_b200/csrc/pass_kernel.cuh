@@ -10,19 +10,41 @@
 // row passes.  H (S2) is produced in registers by the Mid functors.
 //
 // Workspace layout ("column-tile order"): T[x / Wc][y][x % Wc], y < Ny, Wc = lanes of the column
-// pass; a column pass reads and writes one contiguous Ny*Wc block.
+// pass; a column pass reads and writes one contiguous Ny*Wc block.  For Wc >= 2 two neighbouring
+// columns (x even, x + 1) share one 16-byte element stored PLANAR, (re_x, re_x+1, im_x, im_x+1): that is
+// the register-pair format of the packed arithmetic (fft_packed.cuh), so no pass ever shuffles registers
+// to (de)interleave.  Wc == 1 (n = 16384) keeps interleaved (re, im).
 #pragma once
 #include "cwo_internal.h"
 #include "fft_core.cuh"
 #include "pp_core.cuh"
+#include "fft_packed.cuh"
 
 namespace cwo {
 
 enum { ROW_FWD = 0, ROW_INV = 1, COL_FWD = 2, COL_FUSED = 3, COL_MIDINV = 4 };
 
+// element (x = p, y = row) of the column-tiled workspace, any tile width (generic, 32-bit accesses when planar)
+__device__ __forceinline__ size_t ws_block(int p, int row, int ly, int logwc) {
+    return ((size_t)(p >> logwc) * ly + row) << logwc;                         // complex elements
+}
+__device__ __forceinline__ float2 ws_load(const float2* ws, int p, int row, int ly, int logwc) {
+    const int c = p & ((1 << logwc) - 1);
+    if (logwc == 0) return ws[ws_block(p, row, ly, 0)];
+    const float* f = reinterpret_cast<const float*>(ws + ws_block(p, row, ly, logwc)) + ((c >> 1) << 2) + (c & 1);
+    return make_float2(f[0], f[2]);
+}
+__device__ __forceinline__ void ws_store(float2* ws, int p, int row, int ly, int logwc, float2 v) {
+    const int c = p & ((1 << logwc) - 1);
+    if (logwc == 0) { ws[ws_block(p, row, ly, 0)] = v; return; }
+    float* f = reinterpret_cast<float*>(ws + ws_block(p, row, ly, logwc)) + ((c >> 1) << 2) + (c & 1);
+    f[0] = v.x; f[2] = v.y;
+}
+
 struct MidNone {
     __device__ __forceinline__ void operator()(float2 (&)[2][16]) const {}
     __device__ __forceinline__ void slot(float2 (&)[16], int) const {}
+    __device__ __forceinline__ void packed(PV&) const {}
 };
 
 // Fresnel: FFT2 of the sampled separable chirp is the outer product Cx[k]*Cy[l] (S2, S7 folded in)
@@ -38,6 +60,19 @@ template <int LOGN> struct MidTables {
             const float2 cy1 = C::PAIR ? cy0 : __ldg(&P.tab_point[u[1] + e * C::Q]);
             v[0][e] = cconj(cmul(v[0][e], cmul(cx0, cy0)));
             v[1][e] = cconj(cmul(v[1][e], cmul(cx1, cy1)));
+        }
+    }
+    // both slots in packed form (fft_packed.cuh); lane pairs only
+    __device__ __forceinline__ void packed(PV& v) const {
+        using C = Tile<LOGN>;
+        const float2 cx0 = __ldg(&P.tab_lane[lane0]), cx1 = __ldg(&P.tab_lane[lane0 + 1]);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 cy = __ldg(&P.tab_point[u[0] + e * C::Q]);
+            float r0, r1, i0, i1;
+            pk_split(v.r[e], r0, r1); pk_split(v.i[e], i0, i1);
+            const float2 a = cmul(make_float2(r0, i0), cmul(cx0, cy)), b = cmul(make_float2(r1, i1), cmul(cx1, cy));
+            v.r[e] = pk_make(a.x, b.x); v.i[e] = pk_make(-a.y, -b.y);
         }
     }
     // one slot at a time (pp_core.cuh); lane pairs only
@@ -218,7 +253,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
         for (int e = 0; e < 16; ++e) {
             const int x = (threadIdx.x & ~1) + e * Q;
             const float4 t4 = *reinterpret_cast<const float4*>(&P.in[((size_t)(x >> 1) * P.ly + row) * 2]);
-            v[0][e] = make_float2(t4.x, -t4.y); v[1][e] = make_float2(t4.z, -t4.w);
+            v[0][e] = make_float2(t4.x, t4.z); v[1][e] = make_float2(t4.y, t4.w);
         }
     } else if constexpr (KIND == ROW_INV) {
         // rows of the column-tiled workspace
@@ -228,13 +263,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
             const bool ok = row < P.rows;
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
-                const int p = u[s] + e * Q;
-#ifdef CWO_DEBUG_ROWMAJOR_WS
-                const size_t a = (size_t)row * C::N + p;
-#else
-                const size_t a = ((size_t)(p >> P.logwc) * P.ly + row) * (1u << P.logwc) + (p & ((1 << P.logwc) - 1));
-#endif
-                v[s][e] = ok ? cconj(P.in[a]) : make_float2(0.f, 0.f);
+                v[s][e] = ok ? ws_load(P.in, u[s] + e * Q, row, P.ly, P.logwc) : make_float2(0.f, 0.f);
             }
         }
     } else {
@@ -245,7 +274,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
             for (int e = 0; e < 16; ++e) {
                 if (e < NE) {
                     const float4 t = *reinterpret_cast<const float4*>(&src[(size_t)(u[0] + e * Q) * W + w0]);
-                    v[0][e] = make_float2(t.x, t.y); v[1][e] = make_float2(t.z, t.w);
+                    v[0][e] = make_float2(t.x, t.z); v[1][e] = make_float2(t.y, t.w);
                 } else {
                     v[0][e] = v[1][e] = make_float2(0.f, 0.f);
                 }
@@ -285,7 +314,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
         for (int e = 0; e < 16; ++e) {
             const int x = (threadIdx.x & ~1) + e * Q;
             *reinterpret_cast<float4*>(&P.out[((size_t)(x >> 1) * P.ly + row) * 2]) =
-                make_float4(v[0][e].x, v[0][e].y, v[1][e].x, v[1][e].y);
+                make_float4(v[0][e].x, v[1][e].x, v[0][e].y, v[1][e].y);
         }
     } else if constexpr (KIND == ROW_FWD) {
 #pragma unroll
@@ -294,13 +323,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
             if (row < P.rows) {
 #pragma unroll
                 for (int e = 0; e < 16; ++e) {
-                    const int p = u[s] + e * Q;
-#ifdef CWO_DEBUG_ROWMAJOR_WS
-                    const size_t a = (size_t)row * C::N + p;
-#else
-                    const size_t a = ((size_t)(p >> P.logwc) * P.ly + row) * (1u << P.logwc) + (p & ((1 << P.logwc) - 1));
-#endif
-                    P.out[a] = v[s][e];
+                    ws_store(P.out, u[s] + e * Q, row, P.ly, P.logwc, v[s][e]);
                 }
             }
         }
@@ -346,13 +369,15 @@ pass_kernel(const __grid_constant__ PassParams P) {
         }
     } else {
         float2* dst = P.out + (size_t)tile * P.ly * W;
-        constexpr bool CONJ = (KIND != COL_FWD);
+        // An inverse column transform leaves conj(result) here: the conj that would complete it and the conj
+        // that opens the inverse row transform of pass R' cancel, so neither is applied.
+        constexpr bool CONJ = false;
         if constexpr (C::PAIR) {
 #pragma unroll
             for (int e = 0; e < NE; ++e) {
                 const float2 a = v[0][e], b = v[1][e];
                 *reinterpret_cast<float4*>(&dst[(size_t)(u[0] + e * Q) * W + w0]) =
-                    CONJ ? make_float4(a.x, -a.y, b.x, -b.y) : make_float4(a.x, a.y, b.x, b.y);
+                    CONJ ? make_float4(a.x, b.x, -a.y, -b.y) : make_float4(a.x, b.x, a.y, b.y);
             }
         } else {
 #pragma unroll

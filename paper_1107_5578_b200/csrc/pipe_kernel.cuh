@@ -16,6 +16,10 @@
 
 #include "pass_kernel.cuh"
 
+#ifndef CWO_SETMAXNREG
+#define CWO_SETMAXNREG 1
+#endif
+
 namespace cwo {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -37,6 +41,22 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
             : "r"(smem_u32(b)), "r"(parity)
             : "memory");
     } while (!ok);
+}
+// same, for the producer lane: back off between polls so that the spin does not take issue slots from the
+// four consumer warps that share its scheduler
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* b, uint32_t parity) {
+    uint32_t ok;
+    for (;;) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_u32(b)), "r"(parity)
+            : "memory");
+        if (ok) break;
+        __nanosleep(64);
+    }
 }
 // global -> shared bulk copy (TMA, no tensor map), completion counted in bytes on the mbarrier
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
@@ -80,13 +100,98 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 // order this thread's generic-proxy accesses to shared memory before later async-proxy (bulk copy) writes
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// Mid functors of the pipelined column passes: slot() only; tables that do not depend on the tile come
+// from shared memory, the per-lane values are fetched when the functor is built (top of the tile).
+template <int LOGN> struct PipeMidAsmSplit {
+    using C = Tile<LOGN>;
+    const PassParams& P; const float* thy; int us, lane0; float thx[2];
+    __device__ __forceinline__ PipeMidAsmSplit(const PassParams& P_, const int (&u)[2], int lane0_, const float* thy_)
+        : P(P_), thy(thy_), us(u[0]), lane0(lane0_) {
+        const float* thl = reinterpret_cast<const float*>(P.tab_lane);
+        const float2 t = __ldg(reinterpret_cast<const float2*>(&thl[lane0]));     // lane0 is even
+        thx[0] = t.x; thx[1] = t.y;
+    }
+    __device__ __forceinline__ void slot(float2 (&x)[16], int s) const {
+        const int lane = lane0 + s;
+        const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+        const float sx = P.res_a * (float)ks * (float)ks;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int l = us + e * C::Q;
+            const int ls = (l < C::N / 2) ? l : l - C::N;
+            const float sv = fmaf(P.res_b * (float)ls, (float)ls, sx);
+            const float om = 1.0f - sv;
+            const float r = 1.0f + om * rsqrtf(om);
+            const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
+            float ph = thx[s] + thy[l] - res;
+            ph -= rintf(ph);
+            float sn, cs;
+            __sincosf(6.283185307179586f * ph, &sn, &cs);
+            x[e] = cconj(cmul(x[e], make_float2(cs, sn)));
+        }
+    }
+    __device__ __forceinline__ void operator()(float2 (&v)[2][16]) const { slot(v[0], 0); slot(v[1], 1); }
+    // both slots in packed form (fft_packed.cuh): the phase is per sample, so this part stays scalar
+    __device__ __forceinline__ void packed(PV& v) const {
+        float sx[2];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int lane = lane0 + s;
+            const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+            sx[s] = P.res_a * (float)ks * (float)ks;
+        }
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int l = us + e * C::Q;
+            const int ls = (l < C::N / 2) ? l : l - C::N;
+            const float ty = thy[l], sy = P.res_b * (float)ls * (float)ls;
+            float xr[2], xi[2];
+            pk_split(v.r[e], xr[0], xr[1]); pk_split(v.i[e], xi[0], xi[1]);
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const float sv = sy + sx[s];
+                const float om = 1.0f - sv;
+                const float r = 1.0f + om * rsqrtf(om);
+                const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
+                float ph = thx[s] + ty - res;
+                ph -= rintf(ph);
+                float sn, cs;
+                __sincosf(6.283185307179586f * ph, &sn, &cs);
+                const float2 y = cmul(make_float2(xr[s], xi[s]), make_float2(cs, sn));
+                xr[s] = y.x; xi[s] = -y.y;
+            }
+            v.r[e] = pk_make(xr[0], xr[1]); v.i[e] = pk_make(xi[0], xi[1]);
+        }
+    }
+};
+template <int LOGN> struct PipeMidTables : MidTables<LOGN> {
+    __device__ __forceinline__ PipeMidTables(const PassParams& P, const int (&u)[2], int lane0, const float*)
+        : MidTables<LOGN>{P, u, lane0, nullptr} {}
+};
+struct PipeMidNone : MidNone {
+    __device__ __forceinline__ PipeMidNone(const PassParams&, const int (&)[2], int, const float*) {}
+};
+template <int LOGN, int MID> struct PipeMidSelect;
+template <int LOGN> struct PipeMidSelect<LOGN, MID_NONE> { using type = PipeMidNone; };
+template <int LOGN> struct PipeMidSelect<LOGN, MID_TABLES> { using type = PipeMidTables<LOGN>; };
+template <int LOGN> struct PipeMidSelect<LOGN, MID_ASM_SPLIT> { using type = PipeMidAsmSplit<LOGN>; };
+
 template <int LOGN, int KIND> struct PipeCfg {
     using C = Tile<LOGN>;
-    static constexpr int GROUPS = 2, NBUF = 3, GT = 256;
-    static constexpr int THREADS = GROUPS * GT + 128;        // + the producer warpgroup (one working lane)
+#ifndef CWO_GROUPS
+#define CWO_GROUPS 2
+#endif
+    static constexpr int GROUPS = CWO_GROUPS, NBUF = 3, GT = 256;
+    // + the producer: a warpgroup that hands its registers over (setmaxnreg: 112 / 24 per thread), or just one warp
+    // with the register file split evenly (65536 / 544 = 120 per thread)
+    static constexpr int THREADS = GROUPS * GT + (CWO_SETMAXNREG ? 128 : 32);
     static constexpr size_t BUF_RAW = (KIND == ROW_FWD && C::SMEM_BYTES_X > C::SMEM_BYTES) ? C::SMEM_BYTES_X : C::SMEM_BYTES;
     static constexpr size_t BUF = (BUF_RAW + 127) / 128 * 128;
-    static constexpr size_t SMEM = NBUF * BUF + 64;
+    static constexpr size_t TW_OFF = NBUF * BUF + 64;                       // after the mbarriers
+    static constexpr size_t TW_BYTES = sizeof(float2) * PP<LOGN>::NTW;
+    static constexpr size_t TAB_OFF = TW_OFF + TW_BYTES;                    // ASM: theta_y[l] (float, N entries)
+    static constexpr size_t TAB_BYTES = sizeof(float) * C::N;
+    static constexpr size_t SMEM_NOTAB = TAB_OFF, SMEM_TAB = TAB_OFF + TAB_BYTES;
     // row-major staging (ROW_FWD in, ROW_INV out): row r of the tile at element r * (points + ROWPAD)
     // (bank stagger between lane pairs)
     static constexpr int ROWPAD = C::W > 2 ? 16 / C::W : 0;
@@ -96,7 +201,12 @@ template <int LOGN, int KIND> struct PipeCfg {
 // lane pairs, W <= 8 (transform lengths 1024..4096): pipe_supported() in pass_kernel.cuh.
 
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
-__global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(const __grid_constant__ PassParams P) {
+#if CWO_SETMAXNREG
+__global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1)
+#else
+__global__ void __maxnreg__(120)
+#endif
+pipe_kernel(const __grid_constant__ PassParams P) {
     using C = Tile<LOGN>;
     using K = PipeCfg<LOGN, KIND>;
     static_assert(C::T == K::GT && C::PAIR && C::W <= 8, "tile shape");
@@ -116,12 +226,21 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
         for (int b = 0; b < K::NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&staged[b], K::GT); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    // per-CTA copies of the small tables every tile needs (the L1 left beside ~220 KB of tile buffers is a few
+    // KB: a global twiddle load would be an L2 round trip in the middle of every stage)
+    float2* tws = reinterpret_cast<float2*>(smraw + K::TW_OFF);
+    float* thy = reinterpret_cast<float*>(smraw + K::TAB_OFF);
+    for (int i = threadIdx.x; i < PP<LOGN>::NTW; i += K::THREADS) tws[i] = __ldg(&P.tw[i]);
+    if constexpr (MID == MID_ASM_SPLIT) {
+        const float* thp = reinterpret_cast<const float*>(P.tab_point);
+        for (int i = threadIdx.x; i < N; i += K::THREADS) thy[i] = __ldg(&thp[i]);
+    }
     __syncthreads();
 
     if (threadIdx.x >= K::GROUPS * K::GT) {
         // ================================ producer warp (one lane) ================================
         // the producer warpgroup hands its registers to the consumers (the CTA pool is 640 x 96: 512 x 112 + 128 x 24)
-        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if constexpr (CWO_SETMAXNREG) asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
         if (threadIdx.x != K::GROUPS * K::GT) return;
         const int wc = 1 << P.logwc;
         const int groups = N >> P.logwc, bg = groups < 256 ? groups : 256;    // column groups per TMA box
@@ -169,7 +288,7 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
         };
         for (int j = 0; j < nt && j < K::NBUF; ++j) load(j);
         for (int j = 0; j < nt; ++j) {
-            mbar_wait(&staged[j % K::NBUF], (j / K::NBUF) & 1);
+            mbar_wait_backoff(&staged[j % K::NBUF], (j / K::NBUF) & 1);
             store(j);
             if (j + K::NBUF < nt) {
                 bulk_wait_read();                          // the stores have read the buffer
@@ -181,20 +300,54 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
     }
 
     // ===================================== consumer groups =====================================
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    if constexpr (CWO_SETMAXNREG) asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
     const int g = threadIdx.x >> 8, t = threadIdx.x & 255;
     const SyncGroup sync{1 + g};
     const int us = t / (W / 2), w0 = 2 * (t % (W / 2));     // standard mapping: unit us, lanes w0, w0+1
     const int u[2] = {us, us};
     const int xw = t % W, xi2 = 2 * (t / W);                // unit-pair mapping: lane xw, units xi2, xi2+1
 
+    constexpr bool COLPASS = (KIND != ROW_FWD && KIND != ROW_INV);
 #pragma unroll 1
     for (int j = g; j < nt; j += K::GROUPS) {
         const int b = j % K::NBUF;
         const int tile = blockIdx.x + j * gridDim.x;
         float2* sm = reinterpret_cast<float2*>(smraw + b * K::BUF);
-        float2 v[2][16];
         if (!no_ld) mbar_wait(&full[b], (j / K::NBUF) & 1);
+
+        if constexpr (COLPASS) {
+            // ---- column passes: packed arithmetic, both slots in lockstep (fft_packed.cuh) ----------------
+            PV pv;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                if (e < NE) {
+                    const ulonglong2 t2 = *reinterpret_cast<const ulonglong2*>(&sm[(us + e * Q) * W + w0]);
+                    pv.r[e] = t2.x; pv.i[e] = t2.y;                    // the workspace stores lane pairs planar
+                } else {
+                    pv.r[e] = pv.i[e] = 0ull;
+                }
+            }
+            typename PipeMidSelect<LOGN, KIND == COL_FWD ? MID_NONE : MID>::type mid(P, u, tile * W + w0, thy);
+            if constexpr (KIND == COL_FWD) {
+                transform_p<LOGN, true, false, false>(pv, us, w0, sm, tws, mid, sync);
+            } else if constexpr (KIND == COL_FUSED) {
+                transform_p<LOGN, true, true, false>(pv, us, w0, sm, tws, mid, sync);
+            } else {
+                transform_p<LOGN, false, true, true>(pv, us, w0, sm, tws, mid, sync);
+            }
+            sync();                                           // nobody still reads the exchange image
+            // inverse column results stay conjugated: pass R' expects conj(field)
+#pragma unroll
+            for (int e = 0; e < NE; ++e) {
+                *reinterpret_cast<ulonglong2*>(&sm[(us + e * Q) * W + w0]) = make_ulonglong2(pv.r[e], pv.i[e]);
+            }
+            fence_proxy_async();
+            mbar_arrive(&staged[b]);
+            continue;
+        }
+        // ---- row passes: scalar arithmetic, the two slots half a stage apart (pp_core.cuh) --------------
+        static_assert(COLPASS || KIND == ROW_FWD || KIND == ROW_INV, "kind");
+        float2 v[2][16];
 
         // ---- registers <- staged tile ------------------------------------------------------------
         if constexpr (KIND == ROW_FWD) {
@@ -209,29 +362,18 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
 #pragma unroll
             for (int e = 0; e < 16; ++e) {
                 const float4 t4 = *reinterpret_cast<const float4*>(src + e * Q * W);
-                v[0][e] = make_float2(t4.x, -t4.y); v[1][e] = make_float2(t4.z, -t4.w);
-            }
-        } else {
-#pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                if (e < NE) {
-                    const float4 t4 = *reinterpret_cast<const float4*>(&sm[(us + e * Q) * W + w0]);
-                    v[0][e] = make_float2(t4.x, t4.y); v[1][e] = make_float2(t4.z, t4.w);
-                } else {
-                    v[0][e] = v[1][e] = make_float2(0.f, 0.f);
-                }
+                v[0][e] = make_float2(t4.x, t4.z); v[1][e] = make_float2(t4.y, t4.w);   // planar pair; conj(field): see the column store
             }
         }
 
         // ---- transform: ping-pong schedule of pp_core.cuh ----------------------------------------------
-        const int lane0 = tile * W + w0;
         constexpr int M = C::M, L0 = C::L0;
         float2* rgA = sm;
         float2* rgB = sm + PP<LOGN>::REGION;
         const int wh = w0 >> 1;
         if constexpr (KIND == ROW_FWD) {
             sync();                                           // staged image retired
-            pp_run<LOGN, true, 0, M - 1, false, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
+            pp_run<LOGN, true, 0, M - 1, false, false>(v, us, wh, rgA, rgB, tws, MidNone(), sync);
             // stage M-2 -> one plane per lane, read back unit pairs, last stage in unit-pair mapping
             constexpr int lns = L0 + 4 * (M - 2);
             sync();
@@ -254,7 +396,7 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
                 v[1][e] = make_float2(x.z, x.w);
             }
             const int ux[2] = {xi2, xi2 + 1};
-            butterflies<LOGN, 4, true>(v, ux, L0 + 4 * (M - 1), P.tw);
+            butterflies<LOGN, 4, true, true>(v, ux, L0 + 4 * (M - 1), tws);
             unpermute<16>(v[0]); unpermute<16>(v[1]);
         } else if constexpr (KIND == ROW_INV) {
             dft16(v[0]); dft16(v[1]);                         // unit-pair mapping, Ns = 1: no twiddles
@@ -270,22 +412,7 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
             lds_slot<LOGN>(v[0], us, wh, rgA);
             lds_slot<LOGN>(v[1], us, wh, rgB);
             sync();                                           // regions free again for pp_run
-            pp_run<LOGN, false, M + 1, 2 * M, true, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
-            if constexpr (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); }
-        } else if constexpr (KIND == COL_FWD) {
-            sync();
-            pp_run<LOGN, true, 0, M, false, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
-            unpermute<16>(v[0]); unpermute<16>(v[1]);
-        } else {
-            typename MidSelect<LOGN, MID>::type mid{P, u, lane0, sm};
-            if constexpr (KIND == COL_FUSED) {
-                sync();
-                pp_run<LOGN, true, 0, 2 * M, true, true>(v, us, wh, rgA, rgB, P.tw, mid, sync);
-            } else {
-                mid(v);
-                sync();
-                pp_run<LOGN, false, M, 2 * M, true, false>(v, us, wh, rgA, rgB, P.tw, MidNone(), sync);
-            }
+            pp_run<LOGN, false, M + 1, 2 * M, true, false>(v, us, wh, rgA, rgB, tws, MidNone(), sync);
             if constexpr (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); }
         }
 
@@ -296,7 +423,7 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
             float2* d = sm + ((((xi2 >> P.logwc) * W + xw) << P.logwc) + (xi2 & ((1 << P.logwc) - 1)));
 #pragma unroll
             for (int e = 0; e < 16; ++e)
-                *reinterpret_cast<float4*>(d + e * Q * W) = make_float4(v[0][e].x, v[0][e].y, v[1][e].x, v[1][e].y);
+                *reinterpret_cast<float4*>(d + e * Q * W) = make_float4(v[0][e].x, v[1][e].x, v[0][e].y, v[1][e].y);
         } else if constexpr (KIND == ROW_INV) {
             static_assert(IOM == OUT_COMPLEX, "GS store modes run in pass_kernel");
             const float sc = P.out_scale;                     // conj completes the inverse transform
@@ -305,14 +432,6 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
 #pragma unroll
                 for (int e = 0; e < NE; ++e)
                     sm[(w0 + s) * RS + us + e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
-        } else {
-            constexpr bool CONJ = (KIND != COL_FWD);
-#pragma unroll
-            for (int e = 0; e < NE; ++e) {
-                const float2 a = v[0][e], c = v[1][e];
-                *reinterpret_cast<float4*>(&sm[(us + e * Q) * W + w0]) =
-                    CONJ ? make_float4(a.x, -a.y, c.x, -c.y) : make_float4(a.x, a.y, c.x, c.y);
-            }
         }
         fence_proxy_async();
         mbar_arrive(&staged[b]);
@@ -322,6 +441,7 @@ __global__ void __launch_bounds__(PipeCfg<LOGN, KIND>::THREADS, 1) pipe_kernel(c
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p) {
     using K = PipeCfg<LOGN, KIND>;
+    constexpr size_t SM = (MID == MID_ASM_SPLIT) ? K::SMEM_TAB : K::SMEM_NOTAB;
     static int n_sm = 0;
     if (!n_sm) {
         int dev = 0;
@@ -333,14 +453,14 @@ static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p)
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(pipe_kernel<LOGN, KIND, PAD, MID, IOM>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM);
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     PassParams q = p;
     q.n_tiles = n_tiles;
     const int grid = n_tiles < n_sm ? n_tiles : n_sm;
-    pipe_kernel<LOGN, KIND, PAD, MID, IOM><<<grid, K::THREADS, K::SMEM, s>>>(q);
+    pipe_kernel<LOGN, KIND, PAD, MID, IOM><<<grid, K::THREADS, SM, s>>>(q);
     return cudaGetLastError();
 }
 

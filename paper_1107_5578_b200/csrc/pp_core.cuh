@@ -9,7 +9,8 @@
 // so every store is followed by a whole butterfly block of the other slot before the barrier that
 // publishes it, and shared-memory traffic is spread evenly between the FMA work of every warp.
 // Slot A (even lanes) and slot B (odd lanes) live in separate regions [point][W/2 lanes], one pad
-// element row every 16 points.  Arithmetic and operation order per sample are those of transform().
+// element row every 16 points.  `tw` is the CTA's shared-memory copy of the first PP::NTW twiddles (every
+// index used by a stage is below N/16, or below 16^M for the small inverse radix): plain loads, no __ldg.  Arithmetic and operation order per sample are those of transform().
 #pragma once
 #include "fft_core.cuh"
 
@@ -21,6 +22,8 @@ template <int LOGN> __device__ __forceinline__ int ridx(int p, int wh) {
 }
 template <int LOGN> struct PP {
     static constexpr int REGION = (Tile<LOGN>::N + Tile<LOGN>::N / 16) * (Tile<LOGN>::W / 2);   // elements
+    // twiddles a CTA keeps in shared memory: indices < N/16 for radix-16 stages, < 16^M for the small inverse radix
+    static constexpr int NTW = Tile<LOGN>::L0 == 0 ? Tile<LOGN>::Q : (1 << (4 * Tile<LOGN>::M));
 };
 
 // outputs of a radix-2^LR stage with Ns = 2^lns, one slot, Stockham order.  The padded index of
@@ -70,7 +73,7 @@ __device__ __forceinline__ void slot_small(float2 (&v)[16], int us, int lns, con
         if (lns > 0) {
             float2 w[16];
             const int k0 = (us + i * C::Q) & ((1 << lns) - 1);
-            powers<R>(__ldg(&tw[k0 << (LOGN - lns - LR)]), w);
+            powers<R>(tw[k0 << (LOGN - lns - LR)], w);
             apply_powers<R>(v, i, w);
         }
         dftR<R>(v, i);
@@ -108,7 +111,7 @@ __device__ __forceinline__ void pp_run(float2 (&v)[2][16], int us, int wh, float
         const int sn = s + (merge ? 2 : 1);
         const bool has_next = (sn < SB) || (INV_SMALL && L0 > 0);
         const int lns_out = merge ? 0 : lns;
-        const float2 w1 = __ldg(&tw[(us & ((1 << lns) - 1)) << (LOGN - lns - 4)]);
+        const float2 w1 = tw[(us & ((1 << lns) - 1)) << (LOGN - lns - 4)];
 #pragma unroll
         for (int sl = 0; sl < 2; ++sl) {
             if (lns > 0) {
