@@ -10,7 +10,10 @@
 // load/store path.
 //
 // Same arithmetic and the same tile/unit mapping as pass_kernel.cuh (S3-S10 of SURVEY.md section 8(a));
-// row passes always use the unit-pair mapping at the workspace side.
+// row passes always use the unit-pair mapping at the workspace side and run the scalar ping-pong schedule
+// of pp_core.cuh; column passes run both slots of a thread in lockstep on packed f32x2 operands
+// (fft_packed.cuh), fed directly by the planar lane-pair layout of the workspace.
+// The twiddles every stage needs, and the ASM theta_y table, are copied to shared memory once per CTA.
 #pragma once
 #include <stdint.h>
 
