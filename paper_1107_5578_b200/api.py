@@ -183,3 +183,55 @@ def cwo_gs(plan: Plan, amp_src: torch.Tensor, amp_dst: torch.Tensor, z: float, i
     c = _field(phase, torch.float32, s, "phase")
     plan.ensure_workspace(CWO_OP_GS); plan.bind_stream()
     plan._check(lib().cwo_gs(plan._h, a, b, float(z), int(iters), c), "cwo_gs")
+
+
+class HostPipeline:
+    """Propagate HOST (pinned) fields: step i's host->device copy, its kernels and its device->host copy run
+    on three streams over `depth` rotating device buffers, so the copies of neighbouring steps overlap the
+    kernels (and each other: the two directions use different copy engines).  Argument marshalling and
+    stream plumbing only -- every propagation is one cwo_asm / cwo_fresnel_conv call."""
+
+    def __init__(self, plan: Plan, op: str = "asm", depth: int = 3):
+        if op not in ("asm", "fresnel"):
+            raise ValueError("op must be 'asm' or 'fresnel'")
+        self.plan, self.depth, self.i = plan, int(depth), 0
+        self.call = cwo_asm if op == "asm" else cwo_fresnel_conv
+        shape = (plan.Ny, plan.Nx)
+        self.d_in = [torch.empty(shape, dtype=torch.complex64, device="cuda") for _ in range(self.depth)]
+        self.d_out = [torch.empty(shape, dtype=torch.complex64, device="cuda") for _ in range(self.depth)]
+        self.s_in, self.s_run, self.s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+        self.ev_in = [torch.cuda.Event() for _ in range(self.depth)]     # H2D of slot k done
+        self.ev_run = [torch.cuda.Event() for _ in range(self.depth)]    # kernels of slot k done
+        self.ev_out = [torch.cuda.Event() for _ in range(self.depth)]    # D2H of slot k done
+        self.used = [False] * self.depth
+        plan.ensure_workspace(CWO_OP_ASM if op == "asm" else CWO_OP_FRESNEL)
+
+    def start_after(self, stream: "torch.cuda.Stream") -> None:
+        """Order everything submitted from now on after the work already queued on `stream`."""
+        for s in (self.s_in, self.s_run, self.s_out):
+            s.wait_stream(stream)
+
+    def submit(self, host_in: torch.Tensor, host_out: torch.Tensor, z: float) -> None:
+        k = self.i % self.depth
+        self.i += 1
+        with torch.cuda.stream(self.s_in):
+            if self.used[k]:
+                self.s_in.wait_event(self.ev_run[k])          # the kernels that last read d_in[k]
+            self.d_in[k].copy_(host_in, non_blocking=True)
+            self.ev_in[k].record(self.s_in)
+        with torch.cuda.stream(self.s_run):
+            self.s_run.wait_event(self.ev_in[k])
+            if self.used[k]:
+                self.s_run.wait_event(self.ev_out[k])         # the copy that last read d_out[k]
+            self.call(self.plan, self.d_in[k], self.d_out[k], z)
+            self.ev_run[k].record(self.s_run)
+        with torch.cuda.stream(self.s_out):
+            self.s_out.wait_event(self.ev_run[k])
+            host_out.copy_(self.d_out[k], non_blocking=True)
+            self.ev_out[k].record(self.s_out)
+        self.used[k] = True
+
+    def join(self, stream: "torch.cuda.Stream") -> None:
+        """Make `stream` wait for everything submitted so far (no host synchronisation)."""
+        for s in (self.s_in, self.s_run, self.s_out):
+            stream.wait_stream(s)
