@@ -79,7 +79,8 @@ int cwo_plan_set_option(cwo_plan_t plan, int key, int value);
 /* Workspace a call needs, in bytes (n = number of planes for CWO_OP_STACK, ignored otherwise):
  *   ASM      8*Nx*Ny            (the row-transformed field in column-tile order)
  *   FRESNEL  16*Nx*Ny           (Ny rows x 2Nx columns; the 2Nx x 2Ny padded array is never stored)
- *   STACK    16*Nx*Ny           (spectrum + one plane in flight)
+ *   STACK    8*Nx*Ny*(1 + min(n, 16))   (spectrum + the planes in flight between their column and row pass;
+ *            cwo_propagate_stack accepts anything >= 16*Nx*Ny and batches as many planes as fit)
  *   GS       propagator's workspace + 8*Nx*Ny (the constrained field between propagations)
  * Returns 0 for an unknown op. */
 size_t cwo_plan_workspace_bytes(cwo_plan_t plan, int op, int n);

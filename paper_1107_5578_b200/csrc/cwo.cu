@@ -29,6 +29,8 @@ struct cwo_plan_s {
     double2* chirp_scratch;         // 2 axes x 2M
     float* asm_tab;                 // ASM split path: per plane [theta_x (Mx) | theta_y (My)]
     int asm_tab_planes;             // capacity of asm_tab in planes
+    float* stack_resc;              // batched stack: z/lambda of every plane
+    int stack_resc_cap;
     // CWO_OPT_TIMING: one CUDA event pair around every pass kernel
     int timing;
     std::vector<cudaEvent_t>* ev;   // 2 per recorded launch
@@ -128,6 +130,7 @@ extern "C" int cwo_plan_destroy(cwo_plan_t p) {
     for (int s = 0; s < 2; ++s) for (int a = 0; a < 2; ++a) cudaFree(p->chirp[s][a]);
     cudaFree(p->chirp_scratch);
     cudaFree(p->asm_tab);
+    cudaFree(p->stack_resc);
     if (p->ev) { for (cudaEvent_t e : *p->ev) cudaEventDestroy(e); delete p->ev; }
     delete p->ev_tag;
     delete p;
@@ -167,19 +170,23 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
 static bool asm_sizes_ok(cwo_plan_t p) { return p->lognx >= MIN_LOGN && p->logny >= MIN_LOGN; }
 static bool fresnel_sizes_ok(cwo_plan_t p) { return p->lognx + 1 <= MAX_LOGN && p->logny + 1 <= MAX_LOGN; }
 
+enum { STACK_BATCH = 16 };
+
 static size_t prop_ws_bytes(cwo_plan_t p, int method) {
     const size_t f = sizeof(float2) * (size_t)p->Nx * p->Ny;
     return method == CWO_GS_ASM ? f : 2 * f;
 }
 
 extern "C" size_t cwo_plan_workspace_bytes(cwo_plan_t p, int op, int n) {
-    (void)n;
     if (!p) return 0;
     const size_t f = sizeof(float2) * (size_t)p->Nx * p->Ny;
     switch (op) {
         case CWO_OP_ASM: return f;
         case CWO_OP_FRESNEL: return 2 * f;
-        case CWO_OP_STACK: return 2 * f;
+        case CWO_OP_STACK: {   // spectrum + the planes in flight: up to 16 planes per batch of launches (minimum 1)
+            const int nb = n < 1 ? 1 : (n > STACK_BATCH ? STACK_BATCH : n);
+            return (size_t)(1 + nb) * f;
+        }
         case CWO_OP_GS: return f + prop_ws_bytes(p, p->gs_method);
     }
     return 0;
@@ -289,6 +296,20 @@ static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, i
     return CWO_OK;
 }
 
+// z/lambda of every plane, for the batched stack kernels (host values copied with the stream's ordering)
+static int ensure_stack_resc(cwo_plan_t p, const double* zs, int n) {
+    if (p->stack_resc_cap < n) {
+        if (p->stack_resc) { CWO_CUDA(p, cudaStreamSynchronize(p->stream)); cudaFree(p->stack_resc); p->stack_resc = nullptr; }
+        CWO_CUDA(p, cudaMalloc(&p->stack_resc, sizeof(float) * (size_t)n));
+        p->stack_resc_cap = n;
+    }
+    std::vector<float> h((size_t)n);
+    for (int i = 0; i < n; ++i) h[(size_t)i] = (float)(zs[i] / p->lambda);
+    // pageable source: the copy is staged before the call returns, and ordered on the plan's stream
+    CWO_CUDA(p, cudaMemcpyAsync(p->stack_resc, h.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, p->stream));
+    return CWO_OK;
+}
+
 static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, int plane, PassParams& pp) {
     const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
     pp.n_lane_bins = g.mx;
@@ -356,11 +377,11 @@ static encode_tiled_t get_encode_tiled() {
     }
     return fn;
 }
-static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int logwc, int w_rows) {
+static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int logwc, int w_rows, int planes = 1) {
     encode_tiled_t enc = get_encode_tiled();
     if (!enc || logwc < 1) return false;
     const int wc = 1 << logwc, groups = mx >> logwc;
-    cuuint64_t dims[2] = {(cuuint64_t)ly * wc * 2, (cuuint64_t)groups};
+    cuuint64_t dims[2] = {(cuuint64_t)ly * wc * 2, (cuuint64_t)groups * planes};   // planes stack in the outer dimension
     cuuint64_t strides[1] = {(cuuint64_t)ly * wc * 8};
     cuuint32_t box[2] = {(cuuint32_t)(w_rows * wc * 2), (cuuint32_t)(groups < 256 ? groups : 256)};
     cuuint32_t es[2] = {1, 1};
@@ -440,7 +461,7 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
 extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double* zs, int n, cwo_c64* out) {
     if (!p || !aligned16(u1) || !aligned16(out) || !zs || n <= 0 || !asm_sizes_ok(p)) return CWO_EINVAL;
     for (int k = 0; k < n; ++k) if (!isfinite(zs[k])) return CWO_EINVAL;
-    if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_STACK, n)) return CWO_EWORKSPACE;
+    if (!p->ws || p->ws_bytes < 2 * sizeof(float2) * (size_t)p->Nx * p->Ny) return CWO_EWORKSPACE;   // the minimum: one plane in flight
     const Geometry g = geometry(p, CWO_GS_ASM);
     const size_t f = (size_t)p->Nx * p->Ny;
     float2* A = (float2*)p->ws;       // FFT2[u1] in column-tile order, computed once (S9)
@@ -454,6 +475,31 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     pp.in = A; pp.out = A;
     if ((rc = launch(p, g.logmy, COL_FWD, 0, MID_NONE, g.mx / g.wc, pp)) != CWO_OK) return rc;
     const float scale = (float)(1.0 / ((double)g.mx * (double)g.my));
+    // Batched form (pipelined kernels, split-phase H): one column launch and one row launch cover as many planes
+    // as the workspace holds, so the persistent CTAs fill and drain once per batch instead of once per plane.
+    const int cap = (int)(p->ws_bytes / (sizeof(float2) * f)) - 1;
+    const bool pipe_len = g.logmx >= 10 && g.logmx <= 12 && g.logmy >= 10 && g.logmy <= 12;
+    if (split && p->pipeline && pipe_len && cap >= 2 && p->Ny % g.rb == 0) {
+        if ((rc = ensure_stack_resc(p, zs, n)) != CWO_OK) return rc;
+        const int tab_stride = g.mx + g.my;
+        for (int k0 = 0; k0 < n;) {
+            const int nb = n - k0 < cap ? n - k0 : cap;
+            col_params(p, g, pp);
+            pp.in = A; pp.out = B;
+            fill_asm_mid(p, g, zs[k0], true, k0, pp);
+            pp.n_planes = nb; pp.tiles_per_plane = g.mx / g.wc; pp.in_plane_stride = 0; pp.out_plane_stride = f;
+            pp.tab_plane_stride = tab_stride; pp.plane_resc = p->stack_resc + k0;
+            if ((rc = launch(p, g.logmy, COL_MIDINV, 0, MID_ASM_SPLIT, nb * (g.mx / g.wc), pp)) != CWO_OK) return rc;
+            PassParams rp; row_params(p, g, rp);
+            rp.in = B; rp.out = (float2*)out + (size_t)k0 * f; rp.out_mode = OUT_COMPLEX; rp.out_scale = scale;
+            rp.n_planes = nb; rp.tiles_per_plane = p->Ny / g.rb; rp.in_plane_stride = f; rp.out_plane_stride = f;
+            rp.use_tmap = encode_ws_tmap(&rp.tmap, B, p->Ny, g.mx, g.logwc, g.rb, nb) ? 1 : 0;
+            if (!rp.use_tmap) return CWO_EUNSUPPORTED;
+            if ((rc = launch(p, g.logmx, ROW_INV, 0, MID_NONE, nb * (p->Ny / g.rb), rp)) != CWO_OK) return rc;
+            k0 += nb;
+        }
+        return CWO_OK;
+    }
     for (int k = 0; k < n; ++k) {
         col_params(p, g, pp);
         pp.in = A; pp.out = B;

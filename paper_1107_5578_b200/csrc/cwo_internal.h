@@ -25,6 +25,13 @@ struct PassParams {
     int ly;                   // rows kept in the column-tiled workspace
     int logwc;                // row passes: log2 of the column-tile width of the workspace
     int n_tiles;              // pipelined passes: total number of tiles (the grid is one CTA per SM)
+    // batched planes (depth stack, pipelined kernels only): tile t belongs to plane t / tiles_per_plane
+    int n_planes;             // 0 or 1: a single plane
+    int tiles_per_plane;
+    size_t in_plane_stride;   // complex elements between the planes of `in` (0: every plane reads the same data)
+    size_t out_plane_stride;  // same for `out`
+    int tab_plane_stride;     // MID_ASM_SPLIT: floats between the planes' [theta_x | theta_y] tables
+    const float* plane_resc;  // MID_ASM_SPLIT: res_c (= z/lambda) of every plane
     int dbg;                  // experiment switches (CWO_DEBUG env): 1 no stores, 2 no transform, 4 no loads
     int use_pipe;             // 1: use the pipelined form where it exists (CWO_OPT_PIPELINE)
     const float2* tw;         // forward twiddles exp(-i 2 pi m/n), m < n

@@ -107,10 +107,16 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // from shared memory, the per-lane values are fetched when the functor is built (top of the tile).
 template <int LOGN> struct PipeMidAsmSplit {
     using C = Tile<LOGN>;
-    const PassParams& P; const float* thy; int us, lane0; float thx[2];
-    __device__ __forceinline__ PipeMidAsmSplit(const PassParams& P_, const int (&u)[2], int lane0_, const float* thy_)
-        : P(P_), thy(thy_), us(u[0]), lane0(lane0_) {
-        const float* thl = reinterpret_cast<const float*>(P.tab_lane);
+    const PassParams& P; const float* thy; int us, lane0; float thx[2], res_c;
+    // plane > 0 or batched: the plane's tables are read from global memory (thy_ == nullptr)
+    __device__ __forceinline__ PipeMidAsmSplit(const PassParams& P_, const int (&u)[2], int lane0_, const float* thy_,
+                                               int plane = 0)
+        : P(P_), thy(thy_), us(u[0]), lane0(lane0_), res_c(P_.res_c) {
+        const float* thl = reinterpret_cast<const float*>(P.tab_lane) + (size_t)plane * P.tab_plane_stride;
+        if (!thy_) {
+            thy = reinterpret_cast<const float*>(P.tab_point) + (size_t)plane * P.tab_plane_stride;
+            res_c = __ldg(&P.plane_resc[plane]);
+        }
         const float2 t = __ldg(reinterpret_cast<const float2*>(&thl[lane0]));     // lane0 is even
         thx[0] = t.x; thx[1] = t.y;
     }
@@ -125,7 +131,7 @@ template <int LOGN> struct PipeMidAsmSplit {
             const float sv = fmaf(P.res_b * (float)ls, (float)ls, sx);
             const float om = 1.0f - sv;
             const float r = 1.0f + om * rsqrtf(om);
-            const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
+            const float res = __fdividef(res_c * sv * sv, 2.0f * r * r);
             float ph = thx[s] + thy[l] - res;
             ph -= rintf(ph);
             float sn, cs;
@@ -155,7 +161,7 @@ template <int LOGN> struct PipeMidAsmSplit {
                 const float sv = sy + sx[s];
                 const float om = 1.0f - sv;
                 const float r = 1.0f + om * rsqrtf(om);
-                const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
+                const float res = __fdividef(res_c * sv * sv, 2.0f * r * r);
                 float ph = thx[s] + ty - res;
                 ph -= rintf(ph);
                 float sn, cs;
@@ -168,11 +174,11 @@ template <int LOGN> struct PipeMidAsmSplit {
     }
 };
 template <int LOGN> struct PipeMidTables : MidTables<LOGN> {
-    __device__ __forceinline__ PipeMidTables(const PassParams& P, const int (&u)[2], int lane0, const float*)
+    __device__ __forceinline__ PipeMidTables(const PassParams& P, const int (&u)[2], int lane0, const float*, int = 0)
         : MidTables<LOGN>{P, u, lane0, nullptr} {}
 };
 struct PipeMidNone : MidNone {
-    __device__ __forceinline__ PipeMidNone(const PassParams&, const int (&)[2], int, const float*) {}
+    __device__ __forceinline__ PipeMidNone(const PassParams&, const int (&)[2], int, const float*, int = 0) {}
 };
 template <int LOGN, int MID> struct PipeMidSelect;
 template <int LOGN> struct PipeMidSelect<LOGN, MID_NONE> { using type = PipeMidNone; };
@@ -234,9 +240,10 @@ pipe_kernel(const __grid_constant__ PassParams P) {
     float2* tws = reinterpret_cast<float2*>(smraw + K::TW_OFF);
     float* thy = reinterpret_cast<float*>(smraw + K::TAB_OFF);
     for (int i = threadIdx.x; i < PP<LOGN>::NTW; i += K::THREADS) tws[i] = __ldg(&P.tw[i]);
+    const bool batched = P.n_planes > 1;
     if constexpr (MID == MID_ASM_SPLIT) {
         const float* thp = reinterpret_cast<const float*>(P.tab_point);
-        for (int i = threadIdx.x; i < N; i += K::THREADS) thy[i] = __ldg(&thp[i]);
+        if (!batched) for (int i = threadIdx.x; i < N; i += K::THREADS) thy[i] = __ldg(&thp[i]);
     }
     __syncthreads();
 
@@ -250,21 +257,24 @@ pipe_kernel(const __grid_constant__ PassParams P) {
         auto load = [&](int j) {
             if (no_ld) return;
             const int b = j % K::NBUF;
-            const int tile = blockIdx.x + j * gridDim.x;
+            const int gt = blockIdx.x + j * gridDim.x;
+            const int plane = batched ? gt / P.tiles_per_plane : 0;
+            const int tile = gt - plane * P.tiles_per_plane;
+            const float2* in = P.in + (size_t)plane * P.in_plane_stride;
             unsigned char* dst = smraw + b * K::BUF;
             if constexpr (KIND == ROW_FWD) {               // W rows of the row-major field, NP points each
                 mbar_expect_tx(&full[b], W * NP * 8);
 #pragma unroll
                 for (int r = 0; r < W; ++r)
-                    bulk_g2s(dst + (size_t)r * RS * 8, P.in + (size_t)(tile * W + r) * P.pitch, NP * 8, &full[b]);
+                    bulk_g2s(dst + (size_t)r * RS * 8, in + (size_t)(tile * W + r) * P.pitch, NP * 8, &full[b]);
             } else if constexpr (KIND == ROW_INV) {        // W rows of the column-tiled workspace: [x/Wc][row][x%Wc]
                 mbar_expect_tx(&full[b], W * N * 8);
                 for (int c = 0; c < groups; c += bg)
-                    tma_load_2d(dst + (size_t)c * W * wc * 8, &P.tmap, tile * W * wc * 2, c, &full[b]);
+                    tma_load_2d(dst + (size_t)c * W * wc * 8, &P.tmap, tile * W * wc * 2, plane * groups + c, &full[b]);
             } else {                                       // column tile: one contiguous [ly][W] block
                 const uint32_t bytes = (uint32_t)P.ly * W * 8;
                 mbar_expect_tx(&full[b], bytes);
-                const unsigned char* src = reinterpret_cast<const unsigned char*>(P.in + (size_t)tile * P.ly * W);
+                const unsigned char* src = reinterpret_cast<const unsigned char*>(in + (size_t)tile * P.ly * W);
                 constexpr uint32_t CH = 16384;
                 for (uint32_t o = 0; o < bytes; o += CH) bulk_g2s(dst + o, src + o, bytes - o < CH ? bytes - o : CH, &full[b]);
             }
@@ -272,18 +282,21 @@ pipe_kernel(const __grid_constant__ PassParams P) {
         auto store = [&](int j) {
             if (no_st) return;
             const int b = j % K::NBUF;
-            const int tile = blockIdx.x + j * gridDim.x;
+            const int gt = blockIdx.x + j * gridDim.x;
+            const int plane = batched ? gt / P.tiles_per_plane : 0;
+            const int tile = gt - plane * P.tiles_per_plane;
+            float2* out = P.out + (size_t)plane * P.out_plane_stride;
             unsigned char* src = smraw + b * K::BUF;
             if constexpr (KIND == ROW_FWD) {
                 for (int c = 0; c < groups; c += bg)
-                    tma_store_2d(&P.tmap, src + (size_t)c * W * wc * 8, tile * W * wc * 2, c);
+                    tma_store_2d(&P.tmap, src + (size_t)c * W * wc * 8, tile * W * wc * 2, plane * groups + c);
             } else if constexpr (KIND == ROW_INV) {        // W rows of the row-major field, NP points each
 #pragma unroll
                 for (int r = 0; r < W; ++r)
-                    bulk_s2g(P.out + (size_t)(tile * W + r) * P.pitch, src + (size_t)r * RS * 8, NP * 8);
+                    bulk_s2g(out + (size_t)(tile * W + r) * P.pitch, src + (size_t)r * RS * 8, NP * 8);
             } else {
                 const uint32_t bytes = (uint32_t)P.ly * W * 8;
-                unsigned char* dst = reinterpret_cast<unsigned char*>(P.out + (size_t)tile * P.ly * W);
+                unsigned char* dst = reinterpret_cast<unsigned char*>(out + (size_t)tile * P.ly * W);
                 constexpr uint32_t CH = 16384;
                 for (uint32_t o = 0; o < bytes; o += CH) bulk_s2g(dst + o, src + o, bytes - o < CH ? bytes - o : CH);
             }
@@ -314,7 +327,9 @@ pipe_kernel(const __grid_constant__ PassParams P) {
 #pragma unroll 1
     for (int j = g; j < nt; j += K::GROUPS) {
         const int b = j % K::NBUF;
-        const int tile = blockIdx.x + j * gridDim.x;
+        const int gt = blockIdx.x + j * gridDim.x;
+        const int plane = batched ? gt / P.tiles_per_plane : 0;
+        const int tile = gt - plane * P.tiles_per_plane;
         float2* sm = reinterpret_cast<float2*>(smraw + b * K::BUF);
         if (!no_ld) mbar_wait(&full[b], (j / K::NBUF) & 1);
 
@@ -330,7 +345,7 @@ pipe_kernel(const __grid_constant__ PassParams P) {
                     pv.r[e] = pv.i[e] = 0ull;
                 }
             }
-            typename PipeMidSelect<LOGN, KIND == COL_FWD ? MID_NONE : MID>::type mid(P, u, tile * W + w0, thy);
+            typename PipeMidSelect<LOGN, KIND == COL_FWD ? MID_NONE : MID>::type mid(P, u, tile * W + w0, batched ? nullptr : thy, plane);
             if constexpr (KIND == COL_FWD) {
                 transform_p<LOGN, true, false, false>(pv, us, w0, sm, tws, mid, sync);
             } else if constexpr (KIND == COL_FUSED) {
