@@ -83,6 +83,7 @@ static int launch(cwo_plan_t p, int logn, int kind, int pad, int mid, int n_tile
 
 static int ensure_twiddles(cwo_plan_t p, int logn, bool want64) {
     const int n = 1 << logn;
+    const bool built = !p->tw[logn] || (want64 && !p->tw64[logn]);
     if (!p->tw[logn]) {
         CWO_CUDA(p, cudaMalloc(&p->tw[logn], sizeof(float2) * n));
         CWO_CUDA(p, build_twiddles(p->tw[logn], n, p->stream));
@@ -93,6 +94,9 @@ static int ensure_twiddles(cwo_plan_t p, int logn, bool want64) {
         CWO_CUDA(p, build_twiddles_f64(p->tw64[logn], n, p->stream));
         p->launches++;
     }
+    // the pipelined kernels read these tables before they wait for their predecessor (programmatic dependent
+    // launch), so a table built on demand must be complete before anything else is enqueued (once per length)
+    if (built) CWO_CUDA(p, cudaStreamSynchronize(p->stream));
     return CWO_OK;
 }
 

@@ -245,6 +245,11 @@ pipe_kernel(const __grid_constant__ PassParams P) {
         const float* thp = reinterpret_cast<const float*>(P.tab_point);
         if (!batched) for (int i = threadIdx.x; i < N; i += K::THREADS) thy[i] = __ldg(&thp[i]);
     }
+    // Programmatic dependent launch: everything above reads only plan tables, which were complete before the
+    // previous kernel in the stream passed this same point, so it may run while that kernel drains.  From here
+    // on the previous kernel's results are needed; our successor may start its own prologue right away.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     __syncthreads();
 
     if (threadIdx.x >= K::GROUPS * K::GT) {
@@ -478,8 +483,14 @@ static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p)
     PassParams q = p;
     q.n_tiles = n_tiles;
     const int grid = n_tiles < n_sm ? n_tiles : n_sm;
-    pipe_kernel<LOGN, KIND, PAD, MID, IOM><<<grid, K::THREADS, SM, s>>>(q);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)K::THREADS);
+    cfg.dynamicSmemBytes = SM; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, pipe_kernel<LOGN, KIND, PAD, MID, IOM>, q);
 }
 
 }  // namespace cwo

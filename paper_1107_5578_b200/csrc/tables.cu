@@ -90,12 +90,21 @@ __global__ void asm_phase_kernel(float* tab, const __grid_constant__ AsmPlaneBat
         c -= rint(c);
         t[i] = (float)c;
     }
+    // Launched with programmatic stream serialization: the table depends on nothing earlier in the stream (its
+    // previous reader finished before the preceding kernel let this one start), so it is computed while that
+    // kernel drains; completing only after it keeps the stream's order for everything that follows.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
 cudaError_t build_asm_phase_tables(float* tab, const AsmPlaneBatch& planes, int n_planes, int mx, int my, cudaStream_t s) {
     dim3 grid((mx + my + 255) / 256 > 64 ? 64 : (mx + my + 255) / 256, n_planes);
-    asm_phase_kernel<<<grid, 256, 0, s>>>(tab, planes, mx, my);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, asm_phase_kernel, tab, planes, mx, my);
 }
 
 }  // namespace cwo
