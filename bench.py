@@ -302,6 +302,8 @@ def run_cuda(args):
 
     wl = make_workload(args.workload, rank, torch, api, W)
     plan, step, N = wl["plan"], wl["step"], wl["N"]
+    if args.no_pipeline:
+        plan.set_option(api.CWO_OPT_PIPELINE, 0)
     NBUF = 3
     stream = torch.cuda.current_stream()
 
@@ -399,6 +401,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-pipeline", action="store_true",
+                    help="CWO_OPT_PIPELINE = 0: one CTA per tile everywhere (comparison runs only)")
     ap.add_argument("--workload", default="c3", choices=sorted(WORKLOADS),
                     help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()

@@ -186,6 +186,10 @@ template <int LOGN> struct MidSelect<LOGN, MID_TABLES> { using type = MidTables<
 template <int LOGN> struct MidSelect<LOGN, MID_ASM_SPLIT> { using type = MidAsmSplit<LOGN>; };
 template <int LOGN> struct MidSelect<LOGN, MID_ASM_F64> { using type = MidAsmF64<LOGN>; };
 
+// Mid functors with a packed() form (pipe_kernel.cuh); constructor (P, u, lane0, theta_y in shared memory or
+// nullptr for the global table, plane)
+template <int LOGN, int MID> struct PipeMidSelect;
+
 // IOM: ROW_FWD -> InMode of the load, ROW_INV -> OutMode of the store, column passes -> 0.
 // X (row passes over a workspace of 2-wide column tiles, W == 2): unit-pair mapping at the workspace side.
 template <int LOGN, int KIND, bool PAD, int MID, int IOM, bool X>
@@ -196,6 +200,10 @@ pass_kernel(const __grid_constant__ PassParams P) {
     constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
     constexpr int NE = PAD ? 8 : 16;        // PAD: points >= n/2 are zero on load / dropped on store
     extern __shared__ float2 sm[];
+    // launched with programmatic stream serialization: resident as soon as the previous kernel's CTAs leave,
+    // running once its results are complete
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     const int tile = blockIdx.x;
     int u[2], w0;
@@ -207,6 +215,29 @@ pass_kernel(const __grid_constant__ PassParams P) {
         u[0] = threadIdx.x; u[1] = threadIdx.x + Q / 2;
     }
     const int lane0 = tile * W + w0;        // row (row pass) or column (column pass) of slot 0
+    if constexpr (!ROWPASS && C::PAIR && MID != MID_ASM_F64 && LOGN >= 8) {
+        // column passes on lane pairs: packed f32x2 arithmetic, both slots in lockstep (fft_packed.cuh); the
+        // workspace stores the pair planar, which is the register format
+        const ulonglong2* src = reinterpret_cast<const ulonglong2*>(P.in + (size_t)tile * P.ly * W);
+        ulonglong2* dst = reinterpret_cast<ulonglong2*>(P.out + (size_t)tile * P.ly * W);
+        PV pv;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            if (e < NE) {
+                const ulonglong2 t2 = src[((size_t)(u[0] + e * Q) * W + w0) >> 1];
+                pv.r[e] = t2.x; pv.i[e] = t2.y;
+            } else {
+                pv.r[e] = pv.i[e] = 0ull;
+            }
+        }
+        typename PipeMidSelect<LOGN, KIND == COL_FWD ? MID_NONE : MID>::type mid(P, u, lane0, nullptr, 0);
+        if constexpr (KIND == COL_FWD) transform_p<LOGN, true, false, false>(pv, u[0], w0, sm, P.tw, mid, SyncCta());
+        else if constexpr (KIND == COL_FUSED) transform_p<LOGN, true, true, false>(pv, u[0], w0, sm, P.tw, mid, SyncCta());
+        else transform_p<LOGN, false, true, true>(pv, u[0], w0, sm, P.tw, mid, SyncCta());
+#pragma unroll
+        for (int e = 0; e < NE; ++e) dst[((size_t)(u[0] + e * Q) * W + w0) >> 1] = make_ulonglong2(pv.r[e], pv.i[e]);
+        return;
+    }
     float2 v[2][16];
 
     // ---- load -----------------------------------------------------------------------------------
@@ -400,8 +431,16 @@ static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    pass_kernel<LOGN, KIND, PAD, MID, IOM, X><<<n_tiles, Tile<LOGN>::T, smem, s>>>(p);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)n_tiles); cfg.blockDim = dim3((unsigned)Tile<LOGN>::T);
+    cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    // measured: early residency helps grids of a few waves (2048^2: 65.7 -> 63.2 us per propagation) and hurts
+    // long ones (4096^2: 208.7 -> 221.9 us)
+    at[0].val.programmaticStreamSerializationAllowed = n_tiles <= 1024 ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, pass_kernel<LOGN, KIND, PAD, MID, IOM, X>, p);
 }
 
 // pipe_kernel.cuh: persistent, prefetching form of the same pass for the HBM-sized tile shapes
@@ -412,7 +451,10 @@ static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p)
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
     constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
-    if constexpr (pipe_supported(LOGN) && MID != MID_ASM_F64 &&
+#ifndef CWO_PIPE_FUSED
+#define CWO_PIPE_FUSED 0
+#endif
+    if constexpr (pipe_supported(LOGN) && MID != MID_ASM_F64 && (CWO_PIPE_FUSED || KIND != COL_FUSED) &&
                   (!ROWPASS || (KIND == ROW_FWD && IOM == IN_COMPLEX) || (KIND == ROW_INV && IOM == OUT_COMPLEX))) {
         if (p.use_pipe && (!ROWPASS || (p.use_tmap && p.rows % Tile<LOGN>::W == 0)))
             return launch_pipe<LOGN, KIND, PAD, MID, IOM>(n_tiles, s, p);

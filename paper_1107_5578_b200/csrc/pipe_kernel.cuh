@@ -115,7 +115,7 @@ template <int LOGN> struct PipeMidAsmSplit {
         const float* thl = reinterpret_cast<const float*>(P.tab_lane) + (size_t)plane * P.tab_plane_stride;
         if (!thy_) {
             thy = reinterpret_cast<const float*>(P.tab_point) + (size_t)plane * P.tab_plane_stride;
-            res_c = __ldg(&P.plane_resc[plane]);
+            if (P.plane_resc) res_c = __ldg(&P.plane_resc[plane]);
         }
         const float2 t = __ldg(reinterpret_cast<const float2*>(&thl[lane0]));     // lane0 is even
         thx[0] = t.x; thx[1] = t.y;
