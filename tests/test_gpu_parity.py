@@ -346,3 +346,77 @@ def test_host_pipeline_matches_oracle(api, oracle):
     torch.cuda.synchronize()
     for f, o, z in zip(fields, outs, zs):
         _assert_parity(o.numpy(), oracle.asm(f, cfg.pitch, cfg.pitch, cfg.lam, z), "host pipeline z=%g" % z)
+
+
+# ---------------------------------------------------------------- launch-structure variants --------------------
+
+@pytest.mark.parametrize("n", [1024, 2048, 4096])
+def test_asm_and_fresnel_without_pipeline_option(api, oracle, n):
+    """CWO_OPT_PIPELINE = 0 (one CTA per tile everywhere) computes the same propagations as the default."""
+    cfg = W.CONFIGS["c3"].scaled(n)
+    u1 = W.make_field(cfg)
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    plan.set_option(api.CWO_OPT_PIPELINE, 0)
+    d1 = _dev(u1); d2 = torch.empty_like(d1)
+    api.cwo_asm(plan, d1, d2, 0.03)
+    torch.cuda.synchronize()
+    _assert_parity(d2.cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, 0.03), "asm %d no pipeline" % n)
+    if n <= 2048:
+        m = n // 2
+        v1 = np.ascontiguousarray(u1[:m, :m])
+        planf = api.cwo_plan(m, m, 8e-6, 532e-9)
+        planf.set_option(api.CWO_OPT_PIPELINE, 0)
+        e1 = _dev(v1); e2 = torch.empty_like(e1)
+        z = 0.2 * m / 1024
+        api.cwo_fresnel_conv(planf, e1, e2, z)
+        torch.cuda.synchronize()
+        _assert_parity(e2.cpu().numpy(), oracle.fresnel_conv(v1, 8e-6, 8e-6, 532e-9, z), "fresnel %d no pipeline" % m)
+
+
+def test_stack_batching_edges(api, oracle):
+    """Batched stack launches: a batch remainder (5 planes, room for 3 per batch), the minimum workspace (one
+    plane in flight: unbatched launches) and the pipeline option off all give the planes of independent cwo_asm."""
+    n = 1024
+    cfg = W.CONFIGS["c4"].scaled(n)
+    u1 = W.make_field(cfg)
+    zs = [0.001, 0.004, -0.002, 0.03, 0.064]
+    ref = [oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, z) for z in zs]
+    f = 8 * n * n
+    for ws_planes, pipeline in ((4, 1), (2, 1), (17, 1), (4, 0)):
+        plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+        plan.set_option(api.CWO_OPT_PIPELINE, pipeline)
+        plan.set_workspace(torch.empty(ws_planes * f, dtype=torch.uint8, device="cuda"))
+        out = torch.empty((len(zs), n, n), dtype=torch.complex64, device="cuda")
+        arr = (api.ctypes.c_double * len(zs))(*zs)
+        plan.bind_stream()
+        rc = api.lib().cwo_propagate_stack(plan._h, _dev(u1).data_ptr(), arr, len(zs), out.data_ptr())
+        assert rc == 0
+        torch.cuda.synchronize()
+        for k in range(len(zs)):
+            _assert_parity(out[k].cpu().numpy(), ref[k], "stack ws=%d planes pipeline=%d plane %d" % (ws_planes, pipeline, k))
+    # below the minimum: refused, nothing enqueued
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    plan.set_workspace(torch.empty(f, dtype=torch.uint8, device="cuda"))
+    out = torch.empty((1, n, n), dtype=torch.complex64, device="cuda")
+    arr = (api.ctypes.c_double * 1)(0.01)
+    assert api.lib().cwo_propagate_stack(plan._h, _dev(u1).data_ptr(), arr, 1, out.data_ptr()) == api.CWO_EWORKSPACE
+
+
+def test_back_to_back_calls_on_a_side_stream(api, oracle):
+    """Programmatic dependent launch keeps stream order: alternating ASM / Fresnel calls with changing z, enqueued
+    back to back on a non-default stream without synchronising, each read its predecessor's output."""
+    n = 1024
+    cfg = W.CONFIGS["c3"].scaled(n)
+    u1 = W.make_field(cfg)
+    s = torch.cuda.Stream()
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    a = _dev(u1); b = torch.empty_like(a); c = torch.empty_like(a)
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        api.cwo_asm(plan, a, b, 0.01)
+        api.cwo_asm(plan, b, c, 0.02)          # semigroup: c = P(0.03) a
+        api.cwo_asm(plan, c, b, -0.03)         # b = a
+        api.cwo_fresnel_conv(plan, b, c, 0.4)
+    s.synchronize()
+    _assert_parity(b.cpu().numpy(), u1.astype(np.complex128), "chain back to the input")
+    _assert_parity(c.cpu().numpy(), oracle.fresnel_conv(u1, cfg.pitch, cfg.pitch, cfg.lam, 0.4), "fresnel after the chain")
