@@ -304,6 +304,8 @@ def run_cuda(args):
     plan, step, N = wl["plan"], wl["step"], wl["N"]
     if args.no_pipeline:
         plan.set_option(api.CWO_OPT_PIPELINE, 0)
+    if args.experiment:
+        plan.set_option(api.CWO_OPT_EXPERIMENT, args.experiment)
     NBUF = 3
     stream = torch.cuda.current_stream()
 
@@ -387,6 +389,8 @@ def run_cuda(args):
                            "bytes_per_step": int(wl["bytes_per_step"]), "propagations_per_step": wl["props_per_step"]},
                 "effective_gbs": eff, "pct_of_8TBs": 100.0 * eff / NOMINAL_HBM_GBS, "pct_of_measured_copy": 100.0 * eff / peak,
                 "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+        if args.experiment or args.no_pipeline:
+            line["not_a_benchmark"] = "experiment=%d no_pipeline=%d" % (args.experiment, int(args.no_pipeline))
         if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
             line["cpu_baseline"] = cpu_baseline(W.CONFIGS["c3"])
         print(json.dumps(line), flush=True)
@@ -403,6 +407,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pipeline", action="store_true",
                     help="CWO_OPT_PIPELINE = 0: one CTA per tile everywhere (comparison runs only)")
+    ap.add_argument("--experiment", type=int, default=0,
+                    help="CWO_OPT_EXPERIMENT bit mask (1: no global stores, 4: no global loads in the persistent kernels); "
+                         "results are wrong, the line is marked and is not a benchmark value")
     ap.add_argument("--workload", default="c3", choices=sorted(WORKLOADS),
                     help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()

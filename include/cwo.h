@@ -55,9 +55,13 @@ enum {
                                (the paper's Listing 8) */
     CWO_OPT_TIMING = 2,     /* value 1: bracket every pass kernel with a CUDA event pair on the plan's
                                stream (read with cwo_plan_timings); 0 (default): off */
-    CWO_OPT_PIPELINE = 3    /* value 1 (default): transform lengths 1024..4096 run as persistent CTAs that
-                               prefetch their next tiles (TMA bulk copies); 0: one CTA per tile everywhere.
-                               Same arithmetic either way. */
+    CWO_OPT_PIPELINE = 3,   /* value 1 (default): the row passes (and the depth stack's column passes) of transform
+                               lengths 1024..4096 run as persistent CTAs that prefetch their next tiles (TMA);
+                               0: one CTA per tile everywhere.  Same arithmetic either way. */
+    CWO_OPT_EXPERIMENT = 4  /* measurement aid, default 0.  Bit 0: the persistent kernels skip their global stores;
+                               bit 2: they skip their global loads (they transform whatever the buffers hold).
+                               RESULTS ARE WRONG with any bit set: it exists to time the on-chip part of a pass
+                               (DESIGN.md section 6). */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
 

@@ -21,6 +21,7 @@ struct cwo_plan_s {
     size_t ws_bytes;
     int gs_method;
     int pipeline;
+    int experiment;                 // CWO_OPT_EXPERIMENT bit mask
     int last_cuda_error;
     long long launches;
     float2* tw[MAX_LOGN + 2];       // fp32 twiddles per log2 length (lazily built)
@@ -161,6 +162,10 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
     }
     if (key == CWO_OPT_PIPELINE && (value == 0 || value == 1)) {
         p->pipeline = value;
+        return CWO_OK;
+    }
+    if (key == CWO_OPT_EXPERIMENT && value >= 0 && value <= 7) {
+        p->experiment = value;
         return CWO_OK;
     }
     if (key == CWO_OPT_TIMING && (value == 0 || value == 1)) {
@@ -397,11 +402,11 @@ static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int l
 static void row_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
     pp.rows = p->Ny; pp.pitch = p->Nx; pp.ly = p->Ny; pp.logwc = g.logwc;
-    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = getenv("CWO_DEBUG") ? atoi(getenv("CWO_DEBUG")) : 0;
+    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = p->experiment;
 }
 static void col_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
-    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = getenv("CWO_DEBUG") ? atoi(getenv("CWO_DEBUG")) : 0;
+    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = p->experiment;
 }
 
 static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float2* ws) {

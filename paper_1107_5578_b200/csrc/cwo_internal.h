@@ -32,7 +32,7 @@ struct PassParams {
     size_t out_plane_stride;  // same for `out`
     int tab_plane_stride;     // MID_ASM_SPLIT: floats between the planes' [theta_x | theta_y] tables
     const float* plane_resc;  // MID_ASM_SPLIT: res_c (= z/lambda) of every plane
-    int dbg;                  // experiment switches (CWO_DEBUG env): 1 no stores, 2 no transform, 4 no loads
+    int dbg;                  // CWO_OPT_EXPERIMENT bit mask (pipelined kernels): 1 no global stores, 4 no global loads
     int use_pipe;             // 1: use the pipelined form where it exists (CWO_OPT_PIPELINE)
     const float2* tw;         // forward twiddles exp(-i 2 pi m/n), m < n
     float out_scale;          // ROW_INV store

@@ -43,7 +43,6 @@ __device__ __forceinline__ void ws_store(float2* ws, int p, int row, int ly, int
 
 struct MidNone {
     __device__ __forceinline__ void operator()(float2 (&)[2][16]) const {}
-    __device__ __forceinline__ void slot(float2 (&)[16], int) const {}
     __device__ __forceinline__ void packed(PV&) const {}
 };
 
@@ -74,13 +73,6 @@ template <int LOGN> struct MidTables {
             const float2 a = cmul(make_float2(r0, i0), cmul(cx0, cy)), b = cmul(make_float2(r1, i1), cmul(cx1, cy));
             v.r[e] = pk_make(a.x, b.x); v.i[e] = pk_make(-a.y, -b.y);
         }
-    }
-    // one slot at a time (pp_core.cuh); lane pairs only
-    __device__ __forceinline__ void slot(float2 (&x)[16], int s) const {
-        using C = Tile<LOGN>;
-        const float2 cx = __ldg(&P.tab_lane[lane0 + s]);
-#pragma unroll
-        for (int e = 0; e < 16; ++e) x[e] = cconj(cmul(x[e], cmul(cx, __ldg(&P.tab_point[u[0] + e * C::Q]))));
     }
 };
 
@@ -118,30 +110,6 @@ template <int LOGN> struct MidAsmSplit {
                 __sincosf(6.283185307179586f * ph, &sn, &cs);
                 v[s][e] = cconj(cmul(v[s][e], make_float2(cs, sn)));
             }
-        }
-    }
-    // one slot at a time (pp_core.cuh); lane pairs only
-    __device__ __forceinline__ void slot(float2 (&x)[16], int s) const {
-        using C = Tile<LOGN>;
-        const float* thl = reinterpret_cast<const float*>(P.tab_lane);
-        const float* thp = reinterpret_cast<const float*>(P.tab_point);
-        const int lane = lane0 + s;
-        const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
-        const float thx = __ldg(&thl[lane]);
-        const float sx = P.res_a * (float)ks * (float)ks;
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int l = u[0] + e * C::Q;
-            const int ls = (l < C::N / 2) ? l : l - C::N;
-            const float sv = fmaf(P.res_b * (float)ls, (float)ls, sx);
-            const float om = 1.0f - sv;
-            const float r = 1.0f + om * rsqrtf(om);
-            const float res = __fdividef(P.res_c * sv * sv, 2.0f * r * r);
-            float ph = thx + __ldg(&thp[l]) - res;
-            ph -= rintf(ph);
-            float sn, cs;
-            __sincosf(6.283185307179586f * ph, &sn, &cs);
-            x[e] = cconj(cmul(x[e], make_float2(cs, sn)));
         }
     }
 };

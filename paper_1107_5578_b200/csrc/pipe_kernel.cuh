@@ -103,7 +103,7 @@ __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.w
 // order this thread's generic-proxy accesses to shared memory before later async-proxy (bulk copy) writes
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// Mid functors of the pipelined column passes: slot() only; tables that do not depend on the tile come
+// Mid functors with a packed() form (both slots of a thread, fft_packed.cuh); tables that do not depend on the tile come
 // from shared memory, the per-lane values are fetched when the functor is built (top of the tile).
 template <int LOGN> struct PipeMidAsmSplit {
     using C = Tile<LOGN>;
@@ -120,26 +120,6 @@ template <int LOGN> struct PipeMidAsmSplit {
         const float2 t = __ldg(reinterpret_cast<const float2*>(&thl[lane0]));     // lane0 is even
         thx[0] = t.x; thx[1] = t.y;
     }
-    __device__ __forceinline__ void slot(float2 (&x)[16], int s) const {
-        const int lane = lane0 + s;
-        const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
-        const float sx = P.res_a * (float)ks * (float)ks;
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int l = us + e * C::Q;
-            const int ls = (l < C::N / 2) ? l : l - C::N;
-            const float sv = fmaf(P.res_b * (float)ls, (float)ls, sx);
-            const float om = 1.0f - sv;
-            const float r = 1.0f + om * rsqrtf(om);
-            const float res = __fdividef(res_c * sv * sv, 2.0f * r * r);
-            float ph = thx[s] + thy[l] - res;
-            ph -= rintf(ph);
-            float sn, cs;
-            __sincosf(6.283185307179586f * ph, &sn, &cs);
-            x[e] = cconj(cmul(x[e], make_float2(cs, sn)));
-        }
-    }
-    __device__ __forceinline__ void operator()(float2 (&v)[2][16]) const { slot(v[0], 0); slot(v[1], 1); }
     // both slots in packed form (fft_packed.cuh): the phase is per sample, so this part stays scalar
     __device__ __forceinline__ void packed(PV& v) const {
         float sx[2];
@@ -396,7 +376,7 @@ pipe_kernel(const __grid_constant__ PassParams P) {
         const int wh = w0 >> 1;
         if constexpr (KIND == ROW_FWD) {
             sync();                                           // staged image retired
-            pp_run<LOGN, true, 0, M - 1, false, false>(v, us, wh, rgA, rgB, tws, MidNone(), sync);
+            pp_run<LOGN, true, 0, M - 1, false>(v, us, wh, rgA, rgB, tws, sync);
             // stage M-2 -> one plane per lane, read back unit pairs, last stage in unit-pair mapping
             constexpr int lns = L0 + 4 * (M - 2);
             sync();
@@ -435,7 +415,7 @@ pipe_kernel(const __grid_constant__ PassParams P) {
             lds_slot<LOGN>(v[0], us, wh, rgA);
             lds_slot<LOGN>(v[1], us, wh, rgB);
             sync();                                           // regions free again for pp_run
-            pp_run<LOGN, false, M + 1, 2 * M, true, false>(v, us, wh, rgA, rgB, tws, MidNone(), sync);
+            pp_run<LOGN, false, M + 1, 2 * M, true>(v, us, wh, rgA, rgB, tws, sync);
             if constexpr (L0 == 0) { unpermute<16>(v[0]); unpermute<16>(v[1]); }
         }
 

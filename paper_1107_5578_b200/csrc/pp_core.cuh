@@ -83,14 +83,12 @@ __device__ __forceinline__ void slot_small(float2 (&v)[16], int us, int lns, con
 // Runs the radix-16 stages SA..SB-1 of the concatenated list [forward stages 0..M-1 | inverse stages
 // M..2M-1] (forward stage s: Ns = 2^(L0+4s); inverse stage M+s: Ns = 2^(4s)), preceded by the small
 // forward radix (FWD_SMALL) and followed by the small inverse radix (INV_SMALL) when L0 > 0.
-// MERGE: the last forward stage, mid.slot() and the first inverse stage (no twiddles) form one block
-// (same 16 points per unit, no exchange).
 // In:  both slots hold the inputs of the first block (register e <-> point us + e*Q); the regions are
 //      free (callers put a barrier between their last use and this call).
 // Out: outputs of the last block; after a radix-16 block they are still in dft16's permuted order.
-template <int LOGN, bool FWD_SMALL, int SA, int SB, bool INV_SMALL, bool MERGE, class Mid, class SY>
+template <int LOGN, bool FWD_SMALL, int SA, int SB, bool INV_SMALL, class SY>
 __device__ __forceinline__ void pp_run(float2 (&v)[2][16], int us, int wh, float2* rgA, float2* rgB,
-                                       const float2* __restrict__ tw, const Mid& mid, const SY& sync) {
+                                       const float2* __restrict__ tw, const SY& sync) {
     using C = Tile<LOGN>;
     constexpr int L0 = C::L0, M = C::M;
     bool pendB = false;                 // slot B's inputs are still in (or on their way to) its region
@@ -107,10 +105,9 @@ __device__ __forceinline__ void pp_run(float2 (&v)[2][16], int us, int wh, float
     for (int s = SA; s < SB;) {
         const bool inv_half = s >= M;
         const int lns = inv_half ? 4 * (s - M) : L0 + 4 * s;
-        const bool merge = MERGE && (s == M - 1);
-        const int sn = s + (merge ? 2 : 1);
+        const int sn = s + 1;
         const bool has_next = (sn < SB) || (INV_SMALL && L0 > 0);
-        const int lns_out = merge ? 0 : lns;
+        const int lns_out = lns;
         const float2 w1 = tw[(us & ((1 << lns) - 1)) << (LOGN - lns - 4)];
 #pragma unroll
         for (int sl = 0; sl < 2; ++sl) {
@@ -121,11 +118,6 @@ __device__ __forceinline__ void pp_run(float2 (&v)[2][16], int us, int wh, float
                 apply_powers<16>(v[sl], 0, w);
             }
             dft16(v[sl]);
-            if (merge) {
-                unpermute<16>(v[sl]);
-                mid.slot(v[sl], sl);
-                dft16(v[sl]);
-            }
             if (sl == 0) {
                 if (pendB) { sync(); lds_slot<LOGN>(v[1], us, wh, rgB); }
                 if (has_next) sts_slot<LOGN, 4>(v[0], us, wh, lns_out, rgA);
