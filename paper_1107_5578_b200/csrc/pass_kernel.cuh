@@ -337,9 +337,30 @@ pass_kernel(const __grid_constant__ PassParams P) {
 #pragma unroll
                 for (int e = 0; e < NE; ++e) P.out[base + e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
             }
+        } else if constexpr (IOM == OUT_PHASOR_AMP) {
+            // GS constraints (S10), phase constraint then amplitude constraint (Listing 8 lines 11-13 / 15-16): keep
+            // u/|u| (1 where u == 0), replace the amplitude by that of the next plane.  The amplitudes of all the
+            // thread's samples are requested before the first is used.
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int row = lane0 + (C::PAIR ? s : 0);
+                if (row >= P.rows) continue;
+                const size_t base = (size_t)row * P.pitch + u[s];
+                float am[NE];
+#pragma unroll
+                for (int e = 0; e < NE; ++e) am[e] = P.out_amp[base + e * Q];
+#pragma unroll
+                for (int e = 0; e < NE; ++e) {
+                    const float2 x = v[s][e];                  // the sample is conj(x)
+                    const float m2 = x.x * x.x + x.y * x.y;
+                    float2 ph = make_float2(1.f, 0.f);
+                    if (m2 > 0.f) { const float r = rsqrtf(m2); ph = make_float2(x.x * r, -x.y * r); }
+                    P.out[base + e * Q] = make_float2(am[e] * ph.x, am[e] * ph.y);
+                }
+            }
         } else {
-            // GS constraints (S10) by a rolled loop over the thread's samples, staged through its own
-            // slots of the tile buffer (rsqrt / atan2f would otherwise be unrolled 32 times).
+            // OUT_PHASE, Eq.(25) P:L482 as atan2, by a rolled loop over the thread's samples staged through its own
+            // slots of the tile buffer (atan2f would otherwise be unrolled 32 times).
             __syncthreads();                               // tile buffer no longer being read
             float2* mine = sm + threadIdx.x;
 #pragma unroll
@@ -353,17 +374,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
                 if (row >= P.rows) continue;
                 const size_t a = (size_t)row * P.pitch + (s ? u[1] : u[0]) + e * Q;
                 const float2 x = mine[i * C::T];          // the sample is conj(x)
-                if constexpr (IOM == OUT_PHASOR_AMP) {
-                    // phase constraint then amplitude constraint (Listing 8 lines 11-13 / 15-16): keep
-                    // u/|u| (1 where u == 0), replace the amplitude by that of the next plane
-                    const float m2 = x.x * x.x + x.y * x.y;
-                    const float am = P.out_amp[a];
-                    float2 ph = make_float2(1.f, 0.f);
-                    if (m2 > 0.f) { const float r = rsqrtf(m2); ph = make_float2(x.x * r, -x.y * r); }
-                    P.out[a] = make_float2(am * ph.x, am * ph.y);
-                } else {   // OUT_PHASE: Eq.(25) P:L482 as atan2
-                    reinterpret_cast<float*>(P.out)[a] = atan2f(-x.y, x.x);
-                }
+                reinterpret_cast<float*>(P.out)[a] = atan2f(-x.y, x.x);
             }
         }
     } else {
