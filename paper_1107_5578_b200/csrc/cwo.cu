@@ -241,8 +241,11 @@ enum { ROW_FWD = 0, ROW_INV = 1, COL_FWD = 2, COL_FUSED = 3, COL_MIDINV = 4 };  
 #ifndef CWO_LOGW12
 #define CWO_LOGW12 1
 #endif
+#ifndef CWO_LOGW13
+#define CWO_LOGW13 1
+#endif
 static int tile_logw_host(int logn) {   // == fft_core.cuh tile_logw
-    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn == 12 ? CWO_LOGW12 : logn == 13 ? 1 : 0;
+    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn == 12 ? CWO_LOGW12 : logn == 13 ? CWO_LOGW13 : 0;
 }
 
 struct Geometry { int pad, logmx, logmy, mx, my, rb, logwc, wc; };
@@ -409,6 +412,11 @@ static void col_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = p->experiment;
 }
 
+// the inverse pass over 8192-point rows of complex fields runs on one-row tiles (fold_kernel.cuh) when the
+// workspace pairs columns
+static bool row_fold(cwo_plan_t p, const Geometry& g, bool complex_io) {
+    return p->pipeline && complex_io && g.logmx == 13 && g.logwc == 1;
+}
 static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float2* ws) {
     PassParams pp; row_params(p, g, pp);
     pp.in = io.in; pp.in_amp = io.in_amp; pp.in_phase = io.in_phase; pp.in_mode = io.in_mode; pp.out = ws;
@@ -418,6 +426,10 @@ static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float
 static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const float2* ws, float scale) {
     PassParams pp; row_params(p, g, pp);
     pp.in = ws; pp.out = (float2*)io.out; pp.out_mode = io.out_mode; pp.out_amp = io.out_amp; pp.out_scale = scale;
+    if (row_fold(p, g, io.out_mode == OUT_COMPLEX) && encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, g.logwc, 1)) {
+        pp.use_fold = 1;
+        return launch(p, g.logmx, ROW_INV, g.pad, MID_NONE, p->Ny, pp);
+    }
     pp.use_tmap = (p->pipeline && encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, g.logwc, g.rb)) ? 1 : 0;
     return launch(p, g.logmx, ROW_INV, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
 }

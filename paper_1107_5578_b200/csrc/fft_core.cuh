@@ -127,8 +127,11 @@ template <int R> __device__ __forceinline__ void unpermute(float2 (&v)[16]) {
 #ifndef CWO_LOGW12
 #define CWO_LOGW12 1
 #endif
+#ifndef CWO_LOGW13
+#define CWO_LOGW13 1
+#endif
 constexpr int tile_logw(int logn) {
-    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn == 12 ? CWO_LOGW12 : logn == 13 ? 1 : 0;
+    return logn <= 5 ? 5 : logn <= 9 ? 4 : logn == 10 ? 3 : logn == 11 ? 2 : logn == 12 ? CWO_LOGW12 : logn == 13 ? CWO_LOGW13 : 0;
 }
 template <int LOGN> struct Tile {
     static constexpr int N = 1 << LOGN, Q = N / 16;
@@ -138,7 +141,7 @@ template <int LOGN> struct Tile {
 #ifndef CWO_MINB
 #define CWO_MINB 2
 #endif
-    static constexpr int MINB = (LOGN <= 12 && T <= 256) ? CWO_MINB : 1;
+    static constexpr int MINB = (LOGN <= 13 && T <= 256) ? CWO_MINB : 1;
     static constexpr int L0 = LOGN & 3, M = LOGN >> 2; // n = 2^L0 * 16^M
     static constexpr size_t SMEM_BYTES = sizeof(float2) * (size_t)(N + N / 16) * W;
     // unit-pair variants: one plane per lane, 2 pad elements every 16 points, plane offsets staggered

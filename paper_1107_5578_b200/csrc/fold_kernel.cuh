@@ -1,0 +1,172 @@
+// fold_kernel.cuh -- pipelined INVERSE row pass (R') for transform length 2n = 8192, built on the n = 4096
+// tile of pipe_kernel.cuh: one row is FOLDED into the two slots of a thread.
+//
+// A tile of two 8192-point lanes no longer fits three times in shared memory, so the 8192-point passes of
+// pass_kernel.cuh run one 139 KB tile per SM with nothing overlapped.  One radix-2 step (decimation in time,
+// forward kernel on the conjugated data as everywhere, see pass_kernel.cuh) removes the problem:
+//       A = FFT_n(X[even]),  B = FFT_n(X[odd]);  y[x] = A[x] + w^x B[x],  y[x+n] = A[x] - w^x B[x],  w = exp(-i 2 pi/2n)
+// X[even], X[odd] are two ordinary n-point lanes with the SAME twiddles: exactly the lane pair (slot 0, slot 1)
+// of the 4096-point tile, and X[2k], X[2k+1] are neighbouring columns of the row, i.e. one planar 16-byte
+// element of the column-tiled workspace -- no unit-pair mapping is needed.  The tile is ONE row (64 KB, three
+// buffers); the radix-2 step runs in registers while the row is written to its row-major staging.
+// Zero padding (Fresnel): y[x+n] is not formed.
+// Measured (8192^2 ASM): 443 -> 280 us.  The mirrored forward pass (decimation in frequency) was built and
+// measured too and is NOT used: its workspace side writes 16-byte pieces, half a DRAM sector each, and scattered
+// partial-sector writes run at about half the rate of the 32-byte pieces the two-row tiles of pass R write
+// (641 us with TMA stores, 745 us with st.global, against 350 us).
+// Same producer / consumer-group / mbarrier structure as pipe_kernel.cuh; transform = pp_core.cuh.
+#pragma once
+#include "pipe_kernel.cuh"
+
+namespace cwo {
+
+// w32^e = exp(-i 2 pi e/32), e = 0..15: the twiddle of point x = us + e*Q (Q = n/16) is w^us * w32^e.
+// e is a compile-time constant after unrolling, so the table folds into immediates.
+__device__ __forceinline__ float2 w32_pow(int e) {
+    constexpr float c[16] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                             0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                             0.19509032201612826785f, 0.0f, -0.19509032201612826785f, -0.38268343236508977173f,
+                             -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                             -0.92387953251128675613f, -0.98078528040323044913f};
+    constexpr float sn[16] = {0.0f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                              0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                              0.98078528040323044913f, 1.0f, 0.98078528040323044913f, 0.92387953251128675613f,
+                              0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                              0.38268343236508977173f, 0.19509032201612826785f};
+    return make_float2(c[e], -sn[e]);
+}
+
+template <int LOGC> struct FoldCfg {
+    using C = Tile<LOGC>;
+    static constexpr int GROUPS = 2, NBUF = 3, GT = 256;
+    static constexpr int THREADS = GROUPS * GT + 128;
+    static constexpr size_t BUF = (C::SMEM_BYTES + 127) / 128 * 128;          // >= one row of 2n points (16 n bytes)
+    static constexpr size_t TW_OFF = NBUF * BUF + 64;                          // n-point twiddles, first Q entries
+    static constexpr size_t TW2_OFF = TW_OFF + sizeof(float2) * C::Q;          // 2n-point twiddles w^us, us < Q
+    static constexpr size_t SMEM = TW2_OFF + sizeof(float2) * C::Q;
+    static_assert(C::L0 == 0 && C::W == 2 && C::T == GT, "fold core: n = 16^m, two slots, 256 threads per tile");
+    static_assert(BUF >= sizeof(float2) * 2 * C::N, "row staging fits the tile buffer");
+};
+
+// Pass R': workspace -> IFFT_2n -> u2.
+// P.tw: the 2n-point twiddle table.  P.tmap: the workspace with boxes of ONE row (16 bytes x 256 column pairs).
+template <int LOGC, bool PAD>
+__global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(const __grid_constant__ PassParams P) {
+    using C = Tile<LOGC>;
+    using K = FoldCfg<LOGC>;
+    constexpr int Q = C::Q, N = C::N, M = C::M;
+    constexpr int NPR = PAD ? N : 2 * N;                    // points of a row that exist in the row-major field
+    constexpr int GR = N / 256;                             // TMA boxes (256 column pairs each) per row
+    extern __shared__ __align__(128) unsigned char smraw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smraw + K::NBUF * K::BUF);
+    uint64_t* staged = full + K::NBUF;
+    const int nt = (P.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int b = 0; b < K::NBUF; ++b) { mbar_init(&full[b], 1); mbar_init(&staged[b], K::GT); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    float2* tws = reinterpret_cast<float2*>(smraw + K::TW_OFF);
+    float2* tw2 = reinterpret_cast<float2*>(smraw + K::TW2_OFF);
+    for (int i = threadIdx.x; i < Q; i += K::THREADS) { tws[i] = __ldg(&P.tw[2 * i]); tw2[i] = __ldg(&P.tw[i]); }
+    asm volatile("griddepcontrol.wait;" ::: "memory");      // see pipe_kernel.cuh
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    __syncthreads();
+
+    if (threadIdx.x >= K::GROUPS * K::GT) {
+        // ================================ producer warp (one lane) ================================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 24;");
+        if (threadIdx.x != K::GROUPS * K::GT) return;
+        auto load = [&](int j) {                            // the row's 16-byte elements, one per column pair
+            const int b = j % K::NBUF, row = blockIdx.x + j * gridDim.x;
+            unsigned char* dst = smraw + b * K::BUF;
+            mbar_expect_tx(&full[b], 2 * N * 8);
+            for (int c = 0; c < GR; ++c) tma_load_2d(dst + (size_t)c * 256 * 16, &P.tmap, row * 4, c * 256, &full[b]);
+        };
+        auto store = [&](int j) {                           // one row of the row-major field
+            const int b = j % K::NBUF, row = blockIdx.x + j * gridDim.x;
+            const unsigned char* src = smraw + b * K::BUF;
+            unsigned char* dst = reinterpret_cast<unsigned char*>(P.out + (size_t)row * P.pitch);
+            for (uint32_t o = 0; o < NPR * 8u; o += 32768u) bulk_s2g(dst + o, src + o, 32768u);
+            bulk_commit();
+        };
+        for (int j = 0; j < nt && j < K::NBUF; ++j) load(j);
+        for (int j = 0; j < nt; ++j) {
+            mbar_wait_backoff(&staged[j % K::NBUF], (j / K::NBUF) & 1);
+            store(j);
+            if (j + K::NBUF < nt) { bulk_wait_read(); load(j + K::NBUF); }
+        }
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        return;
+    }
+
+    // ===================================== consumer groups =====================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
+    const int g = threadIdx.x >> 8, us = threadIdx.x & 255;
+    const SyncGroup sync{1 + g};
+    const float2 wb = tw2[us];                              // w^us
+#pragma unroll 1
+    for (int j = g; j < nt; j += K::GROUPS) {
+        const int b = j % K::NBUF;
+        float2* sm = reinterpret_cast<float2*>(smraw + b * K::BUF);
+        float2 v[2][16];
+        mbar_wait(&full[b], (j / K::NBUF) & 1);
+        // one planar element per column pair: (re X[2k], re X[2k+1], im X[2k], im X[2k+1]), k = us + e*Q;
+        // the column pass left conj(field) here (pass_kernel.cuh)
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float4 t4 = *reinterpret_cast<const float4*>(&sm[2 * (us + e * Q)]);
+            v[0][e] = make_float2(t4.x, t4.z); v[1][e] = make_float2(t4.y, t4.w);
+        }
+        sync();                                             // staged image retired
+        pp_run<LOGC, false, 0, M, false>(v, us, 0, sm, sm + PP<LOGC>::REGION, tws, sync);
+        unpermute<16>(v[0]); unpermute<16>(v[1]);
+        sync();                                             // nobody still reads the exchange regions
+        const float sc = P.out_scale;                       // conj completes the inverse transform
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 t = cmul(v[1][e], cmul(wb, w32_pow(e)));   // w^x B[x], x = us + e*Q
+            const float2 lo = cadd(v[0][e], t);
+            sm[us + e * Q] = make_float2(lo.x * sc, -lo.y * sc);
+            if constexpr (!PAD) {
+                const float2 hi = csub(v[0][e], t);
+                sm[N + us + e * Q] = make_float2(hi.x * sc, -hi.y * sc);
+            }
+        }
+        fence_proxy_async();
+        mbar_arrive(&staged[b]);
+    }
+}
+
+template <int LOGC, bool PAD>
+static cudaError_t launch_fold(int n_rows, cudaStream_t s, const PassParams& p) {
+    using K = FoldCfg<LOGC>;
+    static int n_sm = 0;
+    if (!n_sm) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+    }
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(fold_row_kernel<LOGC, PAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)K::SMEM);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    PassParams q = p;
+    q.n_tiles = n_rows;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(n_rows < n_sm ? n_rows : n_sm)); cfg.blockDim = dim3((unsigned)K::THREADS);
+    cfg.dynamicSmemBytes = K::SMEM; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, fold_row_kernel<LOGC, PAD>, q);
+}
+
+}  // namespace cwo

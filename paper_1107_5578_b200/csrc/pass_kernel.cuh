@@ -427,9 +427,17 @@ constexpr bool pipe_supported(int logn) { return logn >= 10 && logn <= 12; }
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p);
 
+// fold_kernel.cuh: pipelined inverse row pass of length 2n = 8192 on the n = 4096 tile (one row per tile)
+constexpr int FOLD_LOGN = 13;
+template <int LOGC, bool PAD>
+static cudaError_t launch_fold(int n_rows, cudaStream_t s, const PassParams& p);
+
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
     constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
+    if constexpr (LOGN == FOLD_LOGN && KIND == ROW_INV && IOM == OUT_COMPLEX) {
+        if (p.use_fold) return launch_fold<LOGN - 1, PAD>(n_tiles, s, p);                     // n_tiles = rows
+    }
 #ifndef CWO_PIPE_FUSED
 #define CWO_PIPE_FUSED 0
 #endif
