@@ -34,6 +34,8 @@ sys.path.insert(0, ROOT)
 
 METRIC = "propagations/sec (4096^2 ASM, new z per call); effective HBM GB/s for 48*N^2 algorithmic bytes"
 UNIT = "propagations/s"
+C3_DESC = ("c3: ASM 4096x4096 complex64 speckle field, lambda 633 nm, pitch 4 um, z cycling {0.01,0.1,0.5} m "
+           "(new z every call)")
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json's "~8 TB/s peak" (the target's denominator)
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 
@@ -156,7 +158,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "c3: ASM 4096x4096 complex field, lambda 633 nm, pitch 4 um, z cycling {0.01,0.1,0.5} m"},
+            "config": {"workload": C3_DESC, "parallelism": "host cores (oracle)", "bytes_per_step": 48 * cfg.N * cfg.N,
+                       "propagations_per_step": 1},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -208,6 +211,7 @@ def make_workload(name, rank, torch, api, W):
             bps = 48 * n2
             desc = ("%s: ASM %dx%d complex64 speckle field, lambda %g nm, pitch %g um, z cycling %s m (new z every call)"
                     % (name, N, N, base.lam * 1e9, base.pitch * 1e6, "{" + ",".join("%g" % z for z in zs) + "}"))
+            assert name != "c3" or desc == C3_DESC, desc
         else:
             kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2}       # R: 8 rd + 16 wr; C: 16 + 16; R': 16 rd + 8 wr
             bps = 80 * n2
