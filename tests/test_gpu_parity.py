@@ -76,7 +76,8 @@ def test_asm_square_sizes(api, oracle, n):
                        "asm %d z=%g" % (n, z))
 
 
-@pytest.mark.parametrize("shape", [(32, 1024), (2048, 64), (256, 4096), (8192, 32), (32, 16384), (16384, 32)])
+@pytest.mark.parametrize("shape", [(32, 1024), (2048, 64), (256, 4096), (8192, 32), (32, 16384), (16384, 32),
+                                   (1024, 4096), (4096, 1024), (2048, 1024), (1024, 8192), (8192, 2048)])
 def test_asm_non_square_and_unequal_pitch(api, oracle, shape):
     u1 = _rand(shape, 3)
     px, py, lam, z = 3e-6, 5e-6, 633e-9, 0.004
@@ -139,7 +140,7 @@ def test_fresnel_square_sizes(api, oracle, n):
                        oracle.fresnel_conv(u1, cfg.pitch, cfg.pitch, cfg.lam, zz), "fresnel %d z=%g" % (n, zz))
 
 
-@pytest.mark.parametrize("shape", [(16, 512), (1024, 32), (64, 2048)])
+@pytest.mark.parametrize("shape", [(16, 512), (1024, 32), (64, 2048), (512, 2048), (2048, 512), (1024, 4096), (4096, 1024)])
 def test_fresnel_non_square_and_unequal_pitch(api, oracle, shape):
     u1 = _rand(shape, 11)
     px, py, lam, z = 6e-6, 9e-6, 532e-9, 0.01
