@@ -17,6 +17,7 @@
 // This is the transform of S4/S6 in SURVEY.md section 8(a) (paper: "FFT", "IFFT").
 #pragma once
 #include <cuda_runtime.h>
+#include <stdint.h>
 
 namespace cwo {
 
@@ -150,14 +151,57 @@ template <int LOGN> struct Tile {
     static constexpr size_t SMEM_BYTES_X = sizeof(float2) * (size_t)W * (size_t)XPLANE;
 };
 
+// ---- mbarrier primitives (shared::cta) ------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_u32(b)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+
 // Barrier over the threads that share a tile: the whole CTA (one tile per CTA), or a named barrier over
 // one 256-thread group of a persistent CTA that keeps several tiles in flight (pipe_kernel.cuh).
+// An exchange between two stages needs two synchronisations: war() before the stores (everybody has loaded
+// the previous contents of the region; a thread announces that with consumed() right after its loads) and
+// raw() before the loads (everybody's stores are visible).  With plain barriers consumed() is empty.
 struct SyncCta {
+    static constexpr bool EARLY_WAR = false;   // a blocking barrier belongs right before the stores
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
+    __device__ __forceinline__ void consumed() const {}
+    __device__ __forceinline__ void war() const { __syncthreads(); }
+    __device__ __forceinline__ void raw() const { __syncthreads(); }
 };
 struct SyncGroup {
+    static constexpr bool EARLY_WAR = false;
     int id;
     __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 256;" ::"r"(id) : "memory"); }
+    __device__ __forceinline__ void consumed() const {}
+    __device__ __forceinline__ void war() const { (*this)(); }
+    __device__ __forceinline__ void raw() const { (*this)(); }
+};
+// Split-phase form on two mbarriers (arrival count = threads of the tile): consumed() arrives on the first one
+// a whole butterfly block before war() waits on it, so that wait is normally already satisfied and the stores
+// can be issued among the last butterflies.  Both barriers are used once per exchange; n counts the uses.
+struct SyncSplit {
+    static constexpr bool EARLY_WAR = true;    // the wait is normally satisfied: take it before the butterflies
+    uint64_t* bc; uint64_t* bp; mutable uint32_t nc, np;
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+    __device__ __forceinline__ void consumed() const { mbar_arrive(bc); }
+    __device__ __forceinline__ void war() const { mbar_wait(bc, nc & 1); ++nc; }
+    __device__ __forceinline__ void raw() const { mbar_arrive(bp); mbar_wait(bp, np & 1); ++np; }
 };
 
 // shared-memory index of (point p, lane w): one pad row of W elements every 16 points

@@ -134,8 +134,10 @@ template <int R> __device__ __forceinline__ void unpermute_p(PV& v) {
 
 // Twiddle (if lns > 0) and butterflies of one radix-2^LR stage; both slots are unit `us` (shared twiddles).
 // tw: shared-memory copy of the twiddle table (pipe_kernel.cuh).
-template <int LOGN, int LR>
-__device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const float2* tw) {
+// war: an exchange follows directly; its write-after-read synchronisation is taken here, between the twiddles
+// and the butterflies, so that the exchange's stores can be scheduled among the butterflies.
+template <int LOGN, int LR, class SY>
+__device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const float2* tw, const SY& sync, bool war) {
     using C = Tile<LOGN>;
     constexpr int R = 1 << LR, S = 16 / R;
 #pragma unroll
@@ -147,6 +149,7 @@ __device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const floa
 #pragma unroll
             for (int r = 1; r < R; ++r) mul_tw(v, i + r * S, w[r], w[r]);
         }
+        if (SY::EARLY_WAR && war && i == 0) sync.war();
         dftRp<R>(v, i);
     }
 }
@@ -162,7 +165,7 @@ __device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float
     constexpr int R = 1 << LR, S = 16 / R, H = C::W / 2;
     ulonglong2* rg = reinterpret_cast<ulonglong2*>(sm);
     const int wh = w0 >> 1;
-    sync();
+    if (!SY::EARLY_WAR) sync.war();                       // else taken by butterflies_p (war = true)
 #pragma unroll
     for (int i = 0; i < S; ++i) {
         const int j = us + i * C::Q;
@@ -183,7 +186,7 @@ __device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float
             }
         }
     }
-    sync();
+    sync.raw();
     static_assert(C::Q % 16 == 0, "Q multiple of 16");
     const ulonglong2* b = rg + (us + (us >> 4)) * H + wh;
 #pragma unroll
@@ -191,6 +194,7 @@ __device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float
         const ulonglong2 t = b[e * (C::Q + C::Q / 16) * H];
         v.r[e] = t.x; v.i[e] = t.y;
     }
+    sync.consumed();
 }
 
 // Forward and/or inverse transform of the tile held in registers (fft_core.cuh transform()).  `mid`
@@ -203,7 +207,7 @@ __device__ __forceinline__ void transform_p(PV& v, int us, int w0, float2* sm, c
     constexpr int L0 = C::L0, M = C::M;
     static_assert(!(HAS_FWD && HAS_INV) || M >= 2, "merged middle phase needs an exchange after it");
     if constexpr (HAS_FWD && L0 > 0) {
-        butterflies_p<LOGN, L0>(v, us, 0, tw);
+        butterflies_p<LOGN, L0>(v, us, 0, tw, sync, true);
         exchange_p<LOGN, L0>(v, us, w0, 0, sm, sync);
     }
     constexpr int NST = (HAS_FWD ? M : 0) + (HAS_INV ? M : 0);
@@ -212,24 +216,24 @@ __device__ __forceinline__ void transform_p(PV& v, int us, int w0, float2* sm, c
         const bool inv_half = HAS_FWD ? (s >= M) : true;
         const int sl = (HAS_FWD && inv_half) ? s - M : s;
         int lns = inv_half ? 4 * sl : L0 + 4 * sl;
+        const bool fwd_end = !inv_half && sl == M - 1;       // no exchange directly after these butterflies
+        const bool inv_end = inv_half && sl == M - 1 && L0 == 0;
         if (MID_FIRST && s == 0) mid.packed(v);
-        butterflies_p<LOGN, 4>(v, us, lns, tw);
-        if (sl == M - 1) {
-            if (!inv_half) {                                 // end of the forward transform
-                unpermute_p<16>(v);
-                if constexpr (!HAS_INV) break;
-                mid.packed(v);
-                butterflies_p<LOGN, 4>(v, us, 0, tw);        // first inverse stage, same phase
-                ++s; lns = 0;
-            } else if (L0 == 0) {                            // end of the inverse transform
-                unpermute_p<16>(v);
-                break;
-            }
+        butterflies_p<LOGN, 4>(v, us, lns, tw, sync, !fwd_end && !inv_end);
+        if (fwd_end) {                                       // end of the forward transform
+            unpermute_p<16>(v);
+            if constexpr (!HAS_INV) break;
+            mid.packed(v);
+            butterflies_p<LOGN, 4>(v, us, 0, tw, sync, true);   // first inverse stage, same phase
+            ++s; lns = 0;
+        } else if (inv_end) {                                // end of the inverse transform
+            unpermute_p<16>(v);
+            break;
         }
         exchange_p<LOGN, 4>(v, us, w0, lns, sm, sync);
     }
     if constexpr (HAS_INV && L0 > 0) {
-        butterflies_p<LOGN, L0>(v, us, 4 * M, tw);
+        butterflies_p<LOGN, L0>(v, us, 4 * M, tw, sync, false);
         unpermute_p<(1 << L0)>(v);
     }
 }

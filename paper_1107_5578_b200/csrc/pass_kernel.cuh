@@ -15,6 +15,9 @@
 // the register-pair format of the packed arithmetic (fft_packed.cuh), so no pass ever shuffles registers
 // to (de)interleave.  Wc == 1 (n = 16384) keeps interleaved (re, im).
 #pragma once
+#ifndef CWO_SPLIT_SYNC
+#define CWO_SPLIT_SYNC 1
+#endif
 #include "cwo_internal.h"
 #include "fft_core.cuh"
 #include "pp_core.cuh"
@@ -199,9 +202,22 @@ pass_kernel(const __grid_constant__ PassParams P) {
             }
         }
         typename PipeMidSelect<LOGN, KIND == COL_FWD ? MID_NONE : MID>::type mid(P, u, lane0, nullptr, 0);
-        if constexpr (KIND == COL_FWD) transform_p<LOGN, true, false, false>(pv, u[0], w0, sm, P.tw, mid, SyncCta());
-        else if constexpr (KIND == COL_FUSED) transform_p<LOGN, true, true, false>(pv, u[0], w0, sm, P.tw, mid, SyncCta());
-        else transform_p<LOGN, false, true, true>(pv, u[0], w0, sm, P.tw, mid, SyncCta());
+#if CWO_SPLIT_SYNC
+        // split-phase exchange synchronisation on two mbarriers behind the tile buffer (fft_core.cuh SyncSplit)
+        uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(sm) + C::SMEM_BYTES);
+        if (threadIdx.x == 0) {
+            mbar_init(&bars[0], C::T); mbar_init(&bars[1], C::T);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        __syncthreads();
+        const SyncSplit sy{&bars[0], &bars[1], 0u, 0u};
+        sy.consumed();                                     // the region starts free
+#else
+        const SyncCta sy;
+#endif
+        if constexpr (KIND == COL_FWD) transform_p<LOGN, true, false, false>(pv, u[0], w0, sm, P.tw, mid, sy);
+        else if constexpr (KIND == COL_FUSED) transform_p<LOGN, true, true, false>(pv, u[0], w0, sm, P.tw, mid, sy);
+        else transform_p<LOGN, false, true, true>(pv, u[0], w0, sm, P.tw, mid, sy);
 #pragma unroll
         for (int e = 0; e < NE; ++e) dst[((size_t)(u[0] + e * Q) * W + w0) >> 1] = make_ulonglong2(pv.r[e], pv.i[e]);
         return;
@@ -402,7 +418,7 @@ pass_kernel(const __grid_constant__ PassParams P) {
 
 template <int LOGN, int KIND, bool PAD, int MID, int IOM, bool X>
 static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
-    constexpr size_t smem = (X && KIND == ROW_FWD) ? Tile<LOGN>::SMEM_BYTES_X : Tile<LOGN>::SMEM_BYTES;
+    constexpr size_t smem = ((X && KIND == ROW_FWD) ? Tile<LOGN>::SMEM_BYTES_X : Tile<LOGN>::SMEM_BYTES) + 64;   // + two mbarriers
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(pass_kernel<LOGN, KIND, PAD, MID, IOM, X>,
