@@ -176,13 +176,16 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* b) {
 // one 256-thread group of a persistent CTA that keeps several tiles in flight (pipe_kernel.cuh).
 // An exchange between two stages needs two synchronisations: war() before the stores (everybody has loaded
 // the previous contents of the region; a thread announces that with consumed() right after its loads) and
-// raw() before the loads (everybody's stores are visible).  With plain barriers consumed() is empty.
+// raw() before the loads (everybody's stores are visible; raw_arrive() ... raw_wait() when there is work that
+// needs neither, such as the next stage's twiddle powers).  With plain barriers consumed() and raw_arrive() are empty.
 struct SyncCta {
     static constexpr bool EARLY_WAR = false;   // a blocking barrier belongs right before the stores
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
     __device__ __forceinline__ void consumed() const {}
     __device__ __forceinline__ void war() const { __syncthreads(); }
     __device__ __forceinline__ void raw() const { __syncthreads(); }
+    __device__ __forceinline__ void raw_arrive() const {}
+    __device__ __forceinline__ void raw_wait() const { __syncthreads(); }
 };
 struct SyncGroup {
     static constexpr bool EARLY_WAR = false;
@@ -191,6 +194,8 @@ struct SyncGroup {
     __device__ __forceinline__ void consumed() const {}
     __device__ __forceinline__ void war() const { (*this)(); }
     __device__ __forceinline__ void raw() const { (*this)(); }
+    __device__ __forceinline__ void raw_arrive() const {}
+    __device__ __forceinline__ void raw_wait() const { (*this)(); }
 };
 // Split-phase form on two mbarriers (arrival count = threads of the tile): consumed() arrives on the first one
 // a whole butterfly block before war() waits on it, so that wait is normally already satisfied and the stores
@@ -201,7 +206,9 @@ struct SyncSplit {
     __device__ __forceinline__ void operator()() const { __syncthreads(); }
     __device__ __forceinline__ void consumed() const { mbar_arrive(bc); }
     __device__ __forceinline__ void war() const { mbar_wait(bc, nc & 1); ++nc; }
-    __device__ __forceinline__ void raw() const { mbar_arrive(bp); mbar_wait(bp, np & 1); ++np; }
+    __device__ __forceinline__ void raw() const { raw_arrive(); raw_wait(); }
+    __device__ __forceinline__ void raw_arrive() const { mbar_arrive(bp); }
+    __device__ __forceinline__ void raw_wait() const { mbar_wait(bp, np & 1); ++np; }
 };
 
 // shared-memory index of (point p, lane w): one pad row of W elements every 16 points

@@ -160,7 +160,7 @@ __device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const floa
 // lns >= 4, and that of point us + e*Q is affine in e (Q is a multiple of 16): one address computation per
 // unit, immediate offsets per access.
 template <int LOGN, int LR, class SY>
-__device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float2* sm, const SY& sync) {
+__device__ __forceinline__ void exchange_store_p(const PV& v, int us, int w0, int lns, float2* sm, const SY& sync) {
     using C = Tile<LOGN>;
     constexpr int R = 1 << LR, S = 16 / R, H = C::W / 2;
     ulonglong2* rg = reinterpret_cast<ulonglong2*>(sm);
@@ -186,7 +186,13 @@ __device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float
             }
         }
     }
-    sync.raw();
+}
+template <int LOGN, class SY>
+__device__ __forceinline__ void exchange_load_p(PV& v, int us, int w0, const float2* sm, const SY& sync) {
+    using C = Tile<LOGN>;
+    constexpr int H = C::W / 2;
+    const ulonglong2* rg = reinterpret_cast<const ulonglong2*>(sm);
+    const int wh = w0 >> 1;
     static_assert(C::Q % 16 == 0, "Q multiple of 16");
     const ulonglong2* b = rg + (us + (us >> 4)) * H + wh;
 #pragma unroll
@@ -195,6 +201,80 @@ __device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float
         v.r[e] = t.x; v.i[e] = t.y;
     }
     sync.consumed();
+}
+template <int LOGN, int LR, class SY>
+__device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float2* sm, const SY& sync) {
+    exchange_store_p<LOGN, LR>(v, us, w0, lns, sm, sync);
+    sync.raw();
+    exchange_load_p<LOGN>(v, us, w0, sm, sync);
+}
+
+// radix-16 stage with the twiddle powers w[1..15] supplied (computed during the previous exchange)
+template <int LOGN, class SY>
+__device__ __forceinline__ void butterflies16_p(PV& v, int lns, const float2 (&w)[16], const SY& sync, bool war) {
+    if (lns > 0) {
+#pragma unroll
+        for (int r = 1; r < 16; ++r) mul_tw(v, r, w[r], w[r]);
+    }
+    if (SY::EARLY_WAR && war) sync.war();
+    dft16p(v);
+}
+template <int LOGN>
+__device__ __forceinline__ void stage_powers(int us, int lns, const float2* tw, float2 (&w)[16]) {
+    if (lns > 0) powers<16>(tw[(us & ((1 << lns) - 1)) << (LOGN - lns - 4)], w);
+}
+
+// transform_p for split-phase synchronisation (SyncSplit): the twiddle powers of stage s + 1 are formed inside
+// the exchange after stage s.  Otherwise as transform_p below.
+// Forward and/or inverse transform of the tile held in registers (fft_core.cuh transform()).  `mid`
+// (mid.packed(v), which must also conjugate) runs between the two, or first when MID_FIRST.  The last
+// forward stage, mid and the first inverse stage (no twiddles) form one compute phase without an exchange.
+template <int LOGN, bool HAS_FWD, bool HAS_INV, bool MID_FIRST, class Mid, class SY>
+__device__ __forceinline__ void transform_ahead_p(PV& v, int us, int w0, float2* sm, const float2* tw, const Mid& mid,
+                                            const SY& sync) {
+    using C = Tile<LOGN>;
+    constexpr int L0 = C::L0, M = C::M;
+    static_assert(!(HAS_FWD && HAS_INV) || M >= 2, "merged middle phase needs an exchange after it");
+    if constexpr (HAS_FWD && L0 > 0) {
+        butterflies_p<LOGN, L0>(v, us, 0, tw, sync, true);
+        exchange_p<LOGN, L0>(v, us, w0, 0, sm, sync);
+    }
+    constexpr int NST = (HAS_FWD ? M : 0) + (HAS_INV ? M : 0);
+    // Ns = 2^lns of radix-16 stage s of the list [forward 0..M-1 | inverse M..2M-1]
+    auto lns_of = [](int s) { return (HAS_FWD && s < M) ? L0 + 4 * s : 4 * (HAS_FWD ? s - M : s); };
+    float2 w[16];
+    stage_powers<LOGN>(us, lns_of(0), tw, w);
+#pragma unroll 1
+    for (int s = 0; s < NST; ++s) {
+        const bool inv_half = HAS_FWD ? (s >= M) : true;
+        const int sl = (HAS_FWD && inv_half) ? s - M : s;
+        int lns = lns_of(s);
+        const bool fwd_end = !inv_half && sl == M - 1;       // no exchange directly after these butterflies
+        const bool inv_end = inv_half && sl == M - 1 && L0 == 0;
+        if (MID_FIRST && s == 0) mid.packed(v);
+        butterflies16_p<LOGN>(v, lns, w, sync, !fwd_end && !inv_end);
+        if (fwd_end) {                                       // end of the forward transform
+            unpermute_p<16>(v);
+            if constexpr (!HAS_INV) break;
+            mid.packed(v);
+            butterflies16_p<LOGN>(v, 0, w, sync, true);      // first inverse stage (no twiddles), same phase
+            ++s; lns = 0;
+        } else if (inv_end) {                                // end of the inverse transform
+            unpermute_p<16>(v);
+            break;
+        }
+        // exchange; the next stage's twiddle powers are formed between publishing the stores and waiting for
+        // everybody else's (they need neither, and v is dead in between)
+        exchange_store_p<LOGN, 4>(v, us, w0, lns, sm, sync);
+        sync.raw_arrive();
+        if (s + 1 < NST) stage_powers<LOGN>(us, lns_of(s + 1), tw, w);
+        sync.raw_wait();
+        exchange_load_p<LOGN>(v, us, w0, sm, sync);
+    }
+    if constexpr (HAS_INV && L0 > 0) {
+        butterflies_p<LOGN, L0>(v, us, 4 * M, tw, sync, false);
+        unpermute_p<(1 << L0)>(v);
+    }
 }
 
 // Forward and/or inverse transform of the tile held in registers (fft_core.cuh transform()).  `mid`
@@ -206,6 +286,10 @@ __device__ __forceinline__ void transform_p(PV& v, int us, int w0, float2* sm, c
     using C = Tile<LOGN>;
     constexpr int L0 = C::L0, M = C::M;
     static_assert(!(HAS_FWD && HAS_INV) || M >= 2, "merged middle phase needs an exchange after it");
+    if constexpr (SY::EARLY_WAR) {
+        transform_ahead_p<LOGN, HAS_FWD, HAS_INV, MID_FIRST>(v, us, w0, sm, tw, mid, sync);
+        return;
+    }
     if constexpr (HAS_FWD && L0 > 0) {
         butterflies_p<LOGN, L0>(v, us, 0, tw, sync, true);
         exchange_p<LOGN, L0>(v, us, w0, 0, sm, sync);
