@@ -170,7 +170,7 @@ def run_reference(args):
 # workloads: c3 is the headline (BASELINE.json); the others time the same C-ABI calls on other configs
 # ------------------------------------------------------------------------------------------------------
 
-WORKLOADS = {"c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
+WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
              "c2": ("fresnel", 1024), "fresnel2048": ("fresnel", 2048), "fresnel4096": ("fresnel", 4096),
              "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c5": ("gs", 8192)}
 
@@ -181,7 +181,8 @@ def make_workload(name, rank, torch, api, W):
     NBUF = 3
     n2 = float(N) * N
     if op in ("asm", "fresnel"):
-        base = W.CONFIGS["c3"] if op == "asm" else (W.CONFIGS["c2"] if N <= 2048 else W.CONFIGS["c5"])
+        base = (W.CONFIGS["c1"] if name == "c1" else W.CONFIGS["c3"]) if op == "asm" else (
+            W.CONFIGS["c2"] if N <= 2048 else W.CONFIGS["c5"])
         zs = base.zs if op == "asm" else (base.zs[0], 1.07 * base.zs[0], 0.93 * base.zs[0])
         hosts = [W.field_c3(W.Config(name, op, N, base.lam, base.pitch, zs, index=base.index + 100 * (i + rank * NBUF)))
                  for i in range(NBUF)]
