@@ -421,3 +421,26 @@ def test_back_to_back_calls_on_a_side_stream(api, oracle):
     s.synchronize()
     _assert_parity(b.cpu().numpy(), u1.astype(np.complex128), "chain back to the input")
     _assert_parity(c.cpu().numpy(), oracle.fresnel_conv(u1, cfg.pitch, cfg.pitch, cfg.lam, 0.4), "fresnel after the chain")
+
+
+# ---------------------------------------------------------------- randomised sweep -------------------------------
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_shapes_and_parameters(api, oracle, seed):
+    """Seeded sweep over shapes (powers of two, Nx != Ny allowed), pitches, wavelengths and distances of both
+    signs, for both propagations, including in-place calls."""
+    r = np.random.default_rng(20240 + seed)
+    lx, ly = int(r.integers(5, 12)), int(r.integers(5, 12))
+    if lx + ly > 21:                      # keep the fp64 oracle to seconds
+        ly = 21 - lx
+    nx, ny = 1 << lx, 1 << ly
+    lam = float(r.choice([405e-9, 532e-9, 633e-9, 1064e-9]))
+    px, py = float(r.uniform(2.0, 12.0)) * lam * 2, float(r.uniform(2.0, 12.0)) * lam * 2
+    z = float(r.choice([-1, 1])) * float(r.uniform(0.002, 0.3))
+    u1 = _rand((ny, nx), 900 + seed)
+    inplace = bool(seed & 1)
+    _assert_parity(_gpu_asm(api, u1, px, py, lam, z, inplace=inplace), oracle.asm(u1, px, py, lam, z),
+                   "asm %dx%d px=%g py=%g lam=%g z=%g" % (ny, nx, px, py, lam, z))
+    if lx <= 10 and ly <= 10:
+        _assert_parity(_gpu_fresnel(api, u1, px, py, lam, z, inplace=inplace), oracle.fresnel_conv(u1, px, py, lam, z),
+                       "fresnel %dx%d px=%g py=%g lam=%g z=%g" % (ny, nx, px, py, lam, z))
