@@ -391,7 +391,7 @@ static encode_tiled_t get_encode_tiled() {
 }
 static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int logwc, int w_rows, int planes = 1) {
     encode_tiled_t enc = get_encode_tiled();
-    if (!enc || logwc < 1) return false;
+    if (!enc || (w_rows << logwc) < 2) return false;          // boxes are at least 16 bytes wide
     const int wc = 1 << logwc, groups = mx >> logwc;
     cuuint64_t dims[2] = {(cuuint64_t)ly * wc * 2, (cuuint64_t)groups * planes};   // planes stack in the outer dimension
     cuuint64_t strides[1] = {(cuuint64_t)ly * wc * 8};
@@ -420,6 +420,12 @@ static bool row_fold(cwo_plan_t p, const Geometry& g, bool complex_io) {
 static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float2* ws) {
     PassParams pp; row_params(p, g, pp);
     pp.in = io.in; pp.in_amp = io.in_amp; pp.in_phase = io.in_phase; pp.in_mode = io.in_mode; pp.out = ws;
+    // 16384-point rows into a column-major workspace: four rows per cluster, 32-byte pieces (cluster_kernel.cuh)
+    if (p->pipeline && io.in_mode == IN_COMPLEX && g.logmx == 14 && g.logwc == 0 && p->Ny % 4 == 0 &&
+        encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, 0, 4)) {
+        pp.use_cluster = 1;
+        return launch(p, g.logmx, ROW_FWD, g.pad, MID_NONE, p->Ny, pp);
+    }
     pp.use_tmap = (p->pipeline && encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, g.logwc, g.rb)) ? 1 : 0;
     return launch(p, g.logmx, ROW_FWD, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
 }

@@ -14,6 +14,7 @@ enum MidMode { MID_NONE = 0, MID_TABLES = 1, MID_ASM_SPLIT = 2, MID_ASM_F64 = 3 
 struct PassParams {
     CUtensorMap tmap;         // pipelined row passes: the column-tiled workspace as a 2-D tensor (see encode_ws_tmap)
     int use_tmap;             // 1: tmap is valid, the row pass moves its workspace side with TMA tensor copies
+    int use_cluster;          // 1: 16384-point forward row pass on 4-CTA clusters (cluster_kernel.cuh); tmap has 4-row boxes
     int use_fold;             // 1: 8192-point inverse row pass on one-row tiles (fold_kernel.cuh); tmap has one-row boxes
     const float2* in;
     float2* out;              // OUT_PHASE: float*

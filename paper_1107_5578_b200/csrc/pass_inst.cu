@@ -1,6 +1,7 @@
 // pass_inst.cu -- instantiates the pass kernels for ONE transform length; compiled once per
 // CWO_LOGN in [5, 14] (see build.py) so the ten lengths build in parallel.
 #include "fold_kernel.cuh"
+#include "cluster_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"

@@ -448,8 +448,16 @@ constexpr int FOLD_LOGN = 13;
 template <int LOGC, bool PAD>
 static cudaError_t launch_fold(int n_rows, cudaStream_t s, const PassParams& p);
 
+// cluster_kernel.cuh: forward row pass of 16384-point rows on 4-CTA clusters (32-byte workspace pieces)
+constexpr int CLUSTER_LOGN = 14;
+template <int LOGN, bool PAD>
+static cudaError_t launch_cluster_row_fwd(int n_rows, cudaStream_t s, const PassParams& p);
+
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
+    if constexpr (LOGN == CLUSTER_LOGN && KIND == ROW_FWD && IOM == IN_COMPLEX) {
+        if (p.use_cluster) return launch_cluster_row_fwd<LOGN, PAD>(n_tiles, s, p);           // n_tiles = rows
+    }
     constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
     if constexpr (LOGN == FOLD_LOGN && KIND == ROW_INV && IOM == OUT_COMPLEX) {
         if (p.use_fold) return launch_fold<LOGN - 1, PAD>(n_tiles, s, p);                     // n_tiles = rows
