@@ -42,15 +42,22 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, 1) cluster_row_fwd_kernel(const
     constexpr int Q = C::Q, N = C::N, T = C::T, NE = PAD ? 8 : 16, COLS = N / CLUSTER_ROWS, CPT = COLS / T;
     static_assert(sizeof(float2) * N <= C::SMEM_BYTES && COLS % T == 0, "staging fits the tile buffer");
     extern __shared__ float2 sm[];
-    const int row = blockIdx.x;
-    const uint32_t rank = cluster_ctarank();                // == row % 4: clusters are 4 consecutive CTAs
+    const uint32_t rank = cluster_ctarank();                // clusters are 4 consecutive CTAs
     const int u[2] = {(int)threadIdx.x, (int)threadIdx.x + Q / 2};
+    // Persistent over row quads (the grid is one wave of clusters): the TMA store of one quad reads the tile buffer
+    // while the next quad's rows are loaded from global memory.
+#pragma unroll 1
+    for (int row = blockIdx.x; row < P.n_tiles; row += gridDim.x) {
     float2 v[2][16];
 #pragma unroll
     for (int s = 0; s < 2; ++s) {
         const size_t base = (size_t)row * P.pitch + u[s];
 #pragma unroll
         for (int e = 0; e < 16; ++e) v[s][e] = (e < NE) ? P.in[base + e * Q] : make_float2(0.f, 0.f);
+    }
+    if (row != (int)blockIdx.x) {                           // the previous quad's store has read the tile buffer
+        if (threadIdx.x == 0) bulk_wait_read();
+        __syncthreads();
     }
     transform<LOGN, true, false>(v, u, 0, sm, P.tw, MidNone(), SyncCta());
     // register e of slot s <-> point (column) p = u[s] + e*Q of this row; stage as [owner p / COLS][p % COLS] = sm[p]
@@ -80,8 +87,9 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, 1) cluster_row_fwd_kernel(const
         for (int b = 0; b < COLS / 256; ++b)
             tma_store_2d(&P.tmap, sm + (size_t)b * 256 * CLUSTER_ROWS, row0 * 2, (int)rank * COLS + b * 256);
         bulk_commit();
-        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
+    }   // row quads
+    if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 template <int LOGN, bool PAD>
@@ -101,7 +109,17 @@ static cudaError_t launch_cluster_row_fwd(int n_rows, cudaStream_t s, const Pass
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = CLUSTER_ROWS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, cluster_row_fwd_kernel<LOGN, PAD>, p);
+    static int wave = 0;                                    // CTAs of the clusters that are resident at once
+    if (!wave) {
+        int nc = 0;
+        cudaError_t e = cudaOccupancyMaxActiveClusters(&nc, cluster_row_fwd_kernel<LOGN, PAD>, &cfg);
+        if (e != cudaSuccess) return e;
+        wave = (nc > 0 ? nc : 1) * CLUSTER_ROWS;
+    }
+    if (n_rows > wave) cfg.gridDim = dim3((unsigned)wave);
+    PassParams q = p;
+    q.n_tiles = n_rows;
+    return cudaLaunchKernelEx(&cfg, cluster_row_fwd_kernel<LOGN, PAD>, q);
 }
 
 }  // namespace cwo
