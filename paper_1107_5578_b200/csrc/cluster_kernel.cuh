@@ -10,6 +10,9 @@
 // [column][4 rows], one full 32-byte sector per column, and stores its quarter with TMA tensor copies (box
 // 32 B x 256 columns).  (Pushing the results with scattered 8-byte st.shared::cluster instead was measured
 // slower than the plain kernel: 1727 us.)  Loads and the transform are those of pass_kernel.cuh (ROW_FWD).
+// Pass 1514 -> 1024 us.  The mirrored inverse pass (TMA gather of 32-byte pieces, rows redistributed through
+// distributed shared memory) was built and measured as well and is not used: 8-byte GATHERS are not what bounds
+// pass R' (1056 -> 1130 us).
 #pragma once
 #include "pipe_kernel.cuh"
 
