@@ -444,3 +444,30 @@ def test_random_shapes_and_parameters(api, oracle, seed):
     if lx <= 10 and ly <= 10:
         _assert_parity(_gpu_fresnel(api, u1, px, py, lam, z, inplace=inplace), oracle.fresnel_conv(u1, px, py, lam, z),
                        "fresnel %dx%d px=%g py=%g lam=%g z=%g" % (ny, nx, px, py, lam, z))
+
+
+def test_asm_16384_square_plane_wave_and_roundtrip(api):
+    """Largest supported ASM (16384 x 16384, the cluster row kernel without padding), checked without the oracle:
+    a plane wave is an eigenfunction, u2 = H(k0, l0) u1 with H from Eq.(16) in double; z then -z returns the input."""
+    n, px, lam, z = 16384, 4e-6, 633e-9, 0.05
+    k0, l0 = 37, -1234
+    j = torch.arange(n, device="cuda", dtype=torch.float64)
+    phx = torch.remainder(k0 * j, n) * (2 * np.pi / n)
+    phy = torch.remainder(l0 * j, n) * (2 * np.pi / n)
+    u1 = torch.polar(torch.ones((n, n), device="cuda", dtype=torch.float32),
+                     (phy[:, None] + phx[None, :]).to(torch.float32)).contiguous()
+    del phx, phy
+    plan = api.cwo_plan(n, n, px, lam)
+    u2 = torch.empty_like(u1)
+    api.cwo_asm(plan, u1, u2, z)
+    torch.cuda.synchronize()
+    fx, fy = k0 / (n * px), l0 / (n * px)
+    w = 1.0 / lam ** 2 - (fx * fx + fy * fy)
+    ph = z * np.sqrt(w)
+    H = np.exp(2j * np.pi * (ph - np.floor(ph)))
+    err = torch.linalg.vector_norm(u2 - complex(H) * u1) / torch.linalg.vector_norm(u1)
+    assert float(err) <= REL_L2, "plane wave eigenfunction rel-L2 %.3e" % float(err)
+    api.cwo_asm(plan, u2, u2, -z)                       # in place, back
+    torch.cuda.synchronize()
+    err = torch.linalg.vector_norm(u2 - u1) / torch.linalg.vector_norm(u1)
+    assert float(err) <= REL_L2, "round trip rel-L2 %.3e" % float(err)
