@@ -2,6 +2,7 @@
 // CWO_LOGN in [5, 14] (see build.py) so the ten lengths build in parallel.
 #include "fold_kernel.cuh"
 #include "cluster_kernel.cuh"
+#include "prefetch_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"

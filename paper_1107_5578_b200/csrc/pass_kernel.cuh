@@ -453,8 +453,17 @@ constexpr int CLUSTER_LOGN = 14;
 template <int LOGN, bool PAD>
 static cudaError_t launch_cluster_row_fwd(int n_rows, cudaStream_t s, const PassParams& p);
 
+// prefetch_kernel.cuh: fused column pass of the padded 8192/16384-point transforms, persistent with the next tile
+// prefetched into a spare 64 KB buffer
+constexpr size_t PREFETCH_BYTES = 65536;
+template <int LOGN, int MID>
+static cudaError_t launch_colpref(int n_tiles, cudaStream_t s, const PassParams& p);
+
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
+    if constexpr (KIND == COL_FUSED && PAD && MID == MID_TABLES && LOGN >= 13) {
+        if (p.use_pipe && (size_t)p.ly * Tile<LOGN>::W * 8 <= PREFETCH_BYTES) return launch_colpref<LOGN, MID>(n_tiles, s, p);
+    }
     if constexpr (LOGN == CLUSTER_LOGN && KIND == ROW_FWD && IOM == IN_COMPLEX) {
         if (p.use_cluster) return launch_cluster_row_fwd<LOGN, PAD>(n_tiles, s, p);           // n_tiles = rows
     }
