@@ -205,6 +205,22 @@ void cwo_oracle_asm_naive(int ny, int nx, double px, double py, double lambda, d
     free(A);
 }
 
+/* the paper's own form of ASM: like every "convolution form" method it expands the calculation
+ * area to 2Nx x 2Ny with zeros to avoid the wrap-around of the circular convolution (Table 2
+ * P:L287-289).  u1 sits in the [0,Ny) x [0,Nx) corner of the zero array, Eq.(15)-(17) run on the 2N grid
+ * (so the frequency sampling is 1/(2 N p)), and the same corner is cropped.  The convolution is shift
+ * invariant, so the result does not depend on where in the big array the window sits. */
+int cwo_oracle_asm_pad2x(int ny, int nx, double px, double py, double lambda, double z, const zc* u1, zc* u2) {
+    int my = 2 * ny, mx = 2 * nx;
+    zc* a = (zc*)calloc((size_t)mx * my, sizeof(zc));
+    if (!a) return -1;
+    for (int r = 0; r < ny; ++r) memcpy(a + (size_t)r * mx, u1 + (size_t)r * nx, sizeof(zc) * nx);
+    int rc = cwo_oracle_asm(my, mx, px, py, lambda, z, a, a);
+    if (!rc) for (int r = 0; r < ny; ++r) memcpy(u2 + (size_t)r * nx, a + (size_t)r * mx, sizeof(zc) * nx);
+    free(a);
+    return rc;
+}
+
 /* 3-D diffraction = 2-D diffractions stacked along z (Listing 2):
  * out[k] = asm(u1, zs[k]).  Written as n independent calls on purpose. */
 int cwo_oracle_stack(int ny, int nx, double px, double py, double lambda, const double* zs, int n,

@@ -59,6 +59,7 @@ def lib():
     L.cwo_oracle_asm_transfer.argtypes = [_I, _I, _D, _D, _D, _D, _c128]
     L.cwo_oracle_asm.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_asm_naive.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_asm_pad2x.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_stack.argtypes = [_I, _I, _D, _D, _D, _f64, _I, _c128, _c128]
     L.cwo_oracle_fresnel_points.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _I, _i32, _i32, _c128]
     L.cwo_oracle_fresnel_direct.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
@@ -135,6 +136,14 @@ def asm(u1, px, py, lam, z, naive=False):
         lib().cwo_oracle_asm_naive(ny, nx, px, py, lam, z, u1, u2)
     else:
         _check(lib().cwo_oracle_asm(ny, nx, px, py, lam, z, u1, u2), "asm")
+    return u2
+
+
+def asm_pad2x(u1, px, py, lam, z):
+    """ASM on the zero-expanded 2Nx x 2Ny grid, cropped (the paper's own form)."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    _check(lib().cwo_oracle_asm_pad2x(ny, nx, px, py, lam, z, u1, u2), "asm_pad2x")
     return u2
 
 
