@@ -172,7 +172,8 @@ def run_reference(args):
 
 WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
              "c2": ("fresnel", 1024), "fresnel2048": ("fresnel", 2048), "fresnel4096": ("fresnel", 4096),
-             "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c5": ("gs", 8192)}
+             "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c5": ("gs", 8192),
+             "asm_pad2x_2048": ("asm_pad", 2048), "asm_pad2x_4096": ("asm_pad", 4096)}
 
 
 def make_workload(name, rank, torch, api, W):
@@ -180,6 +181,9 @@ def make_workload(name, rank, torch, api, W):
     op, N = WORKLOADS[name]
     NBUF = 3
     n2 = float(N) * N
+    pad2x = op == "asm_pad"                                  # cwo_asm on the zero-expanded grid
+    if pad2x:
+        op = "asm"
     if op in ("asm", "fresnel"):
         base = (W.CONFIGS["c1"] if name == "c1" else W.CONFIGS["c3"]) if op == "asm" else (
             W.CONFIGS["c2"] if N <= 2048 else W.CONFIGS["c5"])
@@ -190,6 +194,8 @@ def make_workload(name, rank, torch, api, W):
         u2 = [torch.empty_like(u1[0]) for _ in range(NBUF)]
         plan = api.cwo_plan(N, N, base.pitch, base.lam)
         call = api.cwo_asm if op == "asm" else api.cwo_fresnel_conv
+        if pad2x:
+            plan.set_option(api.CWO_OPT_ASM_PAD2X, 1)
         plan.ensure_workspace(api.CWO_OP_ASM if op == "asm" else api.CWO_OP_FRESNEL)
 
         def step(i):
@@ -207,7 +213,7 @@ def make_workload(name, rank, torch, api, W):
             f.begin = hp.start_after
             f.end = hp.join
             return f, 8 * n2, 8 * n2
-        if op == "asm":
+        if op == "asm" and not pad2x:
             kb = {0: 16 * n2, 3: 16 * n2, 1: 16 * n2}
             bps = 48 * n2
             desc = ("%s: ASM %dx%d complex64 speckle field, lambda %g nm, pitch %g um, z cycling %s m (new z every call)"
@@ -216,10 +222,11 @@ def make_workload(name, rank, torch, api, W):
         else:
             kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2}       # R: 8 rd + 16 wr; C: 16 + 16; R': 16 rd + 8 wr
             bps = 80 * n2
-            desc = ("%s: Fresnel convolution %dx%d complex64 speckle field (virtual %dx%d), lambda %g nm, pitch %g um, "
-                    "z cycling %s m (new z every call)" % (name, N, N, 2 * N, 2 * N, base.lam * 1e9, base.pitch * 1e6,
+            desc = ("%s: %s %dx%d complex64 speckle field (virtual %dx%d), lambda %g nm, pitch %g um, "
+                    "z cycling %s m (new z every call)" % (name, "zero-expanded ASM" if pad2x else "Fresnel convolution",
+                                                           N, N, 2 * N, 2 * N, base.lam * 1e9, base.pitch * 1e6,
                                                            "{" + ",".join("%.4g" % z for z in zs) + "}"))
-        ws = (24 if op == "asm" else 32) * n2             # u1 + u2 + workspace touched per step
+        ws = (24 if (op == "asm" and not pad2x) else 32) * n2   # u1 + u2 + workspace touched per step
         l2 = ("working set %.0f MB per step, rotating over 3 field pairs (%s the 126 MB L2); no flush"
               % (ws / 1e6, "larger than" if ws > 126e6 else "FITS in"))
         return dict(plan=plan, step=step, N=N, props_per_step=1, bytes_per_step=bps, kind_bytes=kb, e2e=e2e, desc=desc,

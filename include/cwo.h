@@ -58,6 +58,10 @@ enum {
     CWO_OPT_PIPELINE = 3,   /* value 1 (default): the row passes (and the depth stack's column passes) of transform
                                lengths 1024..4096 run as persistent CTAs that prefetch their next tiles (TMA);
                                0: one CTA per tile everywhere.  Same arithmetic either way. */
+    CWO_OPT_ASM_PAD2X = 5,  /* value 1: cwo_asm runs on the calculation area expanded to 2Nx x 2Ny with zeros and crops
+                               (the paper's own form of the method, Table 2: no wrap-around; frequency
+                               sampling 1/(2 N pitch)); needs Nx, Ny <= 8192 and a workspace of 16*Nx*Ny.  Default 0:
+                               circular Nx x Ny form.  cwo_propagate_stack and cwo_gs always use the circular form. */
     CWO_OPT_EXPERIMENT = 4  /* measurement aid, default 0.  Bit 0: the persistent kernels skip their global stores;
                                bit 2: they skip their global loads (they transform whatever the buffers hold).
                                RESULTS ARE WRONG with any bit set: it exists to time the on-chip part of a pass

@@ -26,6 +26,7 @@ CWO_OPT_GS_METHOD = 1
 CWO_OPT_TIMING = 2
 CWO_OPT_PIPELINE = 3
 CWO_OPT_EXPERIMENT = 4
+CWO_OPT_ASM_PAD2X = 5
 CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 
 EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",

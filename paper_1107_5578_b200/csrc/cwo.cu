@@ -22,6 +22,7 @@ struct cwo_plan_s {
     int gs_method;
     int pipeline;
     int experiment;                 // CWO_OPT_EXPERIMENT bit mask
+    int asm_pad2x;                  // CWO_OPT_ASM_PAD2X
     int last_cuda_error;
     long long launches;
     float2* tw[MAX_LOGN + 2];       // fp32 twiddles per log2 length (lazily built)
@@ -164,6 +165,11 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
         p->pipeline = value;
         return CWO_OK;
     }
+    if (key == CWO_OPT_ASM_PAD2X && (value == 0 || value == 1)) {
+        if (value && !(p->lognx + 1 <= MAX_LOGN && p->logny + 1 <= MAX_LOGN)) return CWO_EINVAL;
+        p->asm_pad2x = value;
+        return CWO_OK;
+    }
     if (key == CWO_OPT_EXPERIMENT && value >= 0 && value <= 7) {
         p->experiment = value;
         return CWO_OK;
@@ -190,7 +196,7 @@ extern "C" size_t cwo_plan_workspace_bytes(cwo_plan_t p, int op, int n) {
     if (!p) return 0;
     const size_t f = sizeof(float2) * (size_t)p->Nx * p->Ny;
     switch (op) {
-        case CWO_OP_ASM: return f;
+        case CWO_OP_ASM: return p->asm_pad2x ? 2 * f : f;
         case CWO_OP_FRESNEL: return 2 * f;
         case CWO_OP_STACK: {   // spectrum + the planes in flight: up to 16 planes per batch of launches (minimum 1)
             const int nb = n < 1 ? 1 : (n > STACK_BATCH ? STACK_BATCH : n);
@@ -250,9 +256,10 @@ static int tile_logw_host(int logn) {   // == fft_core.cuh tile_logw
 
 struct Geometry { int pad, logmx, logmy, mx, my, rb, logwc, wc; };
 
-static Geometry geometry(cwo_plan_t p, int method) {
+// pad2x: cwo_asm on the zero-expanded grid (CWO_OPT_ASM_PAD2X); the stack and GS keep the circular form
+static Geometry geometry(cwo_plan_t p, int method, bool pad2x = false) {
     Geometry g;
-    g.pad = (method == CWO_GS_ASM) ? 0 : 1;
+    g.pad = (method == CWO_GS_ASM && !pad2x) ? 0 : 1;
     g.logmx = p->lognx + g.pad; g.logmy = p->logny + g.pad;
     g.mx = 1 << g.logmx; g.my = 1 << g.logmy;
     g.rb = 1 << tile_logw_host(g.logmx);          // rows per row-pass tile
@@ -442,8 +449,9 @@ static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const
 
 // One propagation = pass R, pass C (fused), pass R'.  `ws` holds Ny rows x Mx columns in column-tile
 // order.  Fresnel: table set `set` must hold the spectra for this z.  ASM: tables (if split) at plane 0.
-static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, const PropIO& io, float2* ws) {
-    const Geometry g = geometry(p, method);
+static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, const PropIO& io, float2* ws,
+                      bool pad2x = false) {
+    const Geometry g = geometry(p, method, pad2x);
     int rc;
     if ((rc = ensure_twiddles(p, g.logmx, false)) != CWO_OK) return rc;
     if ((rc = ensure_twiddles(p, g.logmy, false)) != CWO_OK) return rc;
@@ -468,12 +476,13 @@ static bool aligned16(const void* q) { return q && !((uintptr_t)q & 15); }
 extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || !asm_sizes_ok(p)) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_ASM, 0)) return CWO_EWORKSPACE;
-    const Geometry g = geometry(p, CWO_GS_ASM);
+    const bool pad2x = p->asm_pad2x != 0;
+    const Geometry g = geometry(p, CWO_GS_ASM, pad2x);
     const bool split = asm_split_ok(p, g, &z, 1);
     int rc;
     if (split && (rc = build_asm_tables(p, g, &z, 1)) != CWO_OK) return rc;
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
-    return run_passes(p, CWO_GS_ASM, z, 0, split, io, (float2*)p->ws);
+    return run_passes(p, CWO_GS_ASM, z, 0, split, io, (float2*)p->ws, pad2x);
 }
 
 extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {

@@ -461,7 +461,7 @@ static cudaError_t launch_colpref(int n_tiles, cudaStream_t s, const PassParams&
 
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
-    if constexpr (KIND == COL_FUSED && PAD && MID == MID_TABLES && LOGN >= 13) {
+    if constexpr (KIND == COL_FUSED && PAD && MID != MID_ASM_F64 && LOGN >= 13) {
         if (p.use_pipe && (size_t)p.ly * Tile<LOGN>::W * 8 <= PREFETCH_BYTES) return launch_colpref<LOGN, MID>(n_tiles, s, p);
     }
     if constexpr (LOGN == CLUSTER_LOGN && KIND == ROW_FWD && IOM == IN_COMPLEX) {
@@ -511,6 +511,9 @@ static cudaError_t launch_pass_impl(int kind, int pad, int mid, int n_tiles, cud
         case COL_FUSED * 100 + 10 + MID_TABLES: return launch_iom<LOGN, COL_FUSED, true, MID_TABLES>(0, n_tiles, s, p);
         case COL_FUSED * 100 + MID_ASM_SPLIT: return launch_iom<LOGN, COL_FUSED, false, MID_ASM_SPLIT>(0, n_tiles, s, p);
         case COL_FUSED * 100 + MID_ASM_F64: return launch_iom<LOGN, COL_FUSED, false, MID_ASM_F64>(0, n_tiles, s, p);
+        // zero-expanded ASM (CWO_OPT_ASM_PAD2X): the Fresnel pad/crop addressing with the ASM transfer function
+        case COL_FUSED * 100 + 10 + MID_ASM_SPLIT: return launch_iom<LOGN, COL_FUSED, true, MID_ASM_SPLIT>(0, n_tiles, s, p);
+        case COL_FUSED * 100 + 10 + MID_ASM_F64: return launch_iom<LOGN, COL_FUSED, true, MID_ASM_F64>(0, n_tiles, s, p);
         case COL_MIDINV * 100 + MID_ASM_SPLIT: return launch_iom<LOGN, COL_MIDINV, false, MID_ASM_SPLIT>(0, n_tiles, s, p);
         case COL_MIDINV * 100 + MID_ASM_F64: return launch_iom<LOGN, COL_MIDINV, false, MID_ASM_F64>(0, n_tiles, s, p);
     }

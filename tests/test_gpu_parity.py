@@ -471,3 +471,55 @@ def test_asm_16384_square_plane_wave_and_roundtrip(api):
     torch.cuda.synchronize()
     err = torch.linalg.vector_norm(u2 - u1) / torch.linalg.vector_norm(u1)
     assert float(err) <= REL_L2, "round trip rel-L2 %.3e" % float(err)
+
+
+# ---------------------------------------------------------------- zero-expanded ASM --------------
+
+def _gpu_asm_pad2x(api, u1, px, py, lam, z, inplace=False):
+    ny, nx = u1.shape
+    plan = api.cwo_plan(nx, ny, px, lam)
+    if px != py:
+        plan.set_pitch_xy(px, py)
+    plan.set_option(api.CWO_OPT_ASM_PAD2X, 1)
+    d1 = _dev(u1)
+    d2 = d1 if inplace else torch.empty_like(d1)
+    api.cwo_asm(plan, d1, d2, z)
+    torch.cuda.synchronize()
+    return d2.cpu().numpy()
+
+
+@pytest.mark.parametrize("shape", [(32, 32), (64, 256), (512, 128), (1024, 1024), (2048, 512), (256, 4096), (2048, 2048)])
+def test_asm_pad2x_sizes(api, oracle, shape):
+    u1 = _rand(shape, 31)
+    px, py, lam = 4e-6, 5e-6, 633e-9
+    for z, inplace in ((0.01, False), (-0.004, True)):
+        _assert_parity(_gpu_asm_pad2x(api, u1, px, py, lam, z, inplace), oracle.asm_pad2x(u1, px, py, lam, z),
+                       "asm pad2x %s z=%g" % (shape, z))
+
+
+def test_asm_pad2x_c1_evanescent_and_option_scope(api, oracle):
+    cfg = W.CONFIGS["c1"]
+    u1 = W.make_field(cfg)
+    _assert_parity(_gpu_asm_pad2x(api, u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0]),
+                   oracle.asm_pad2x(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0]), "c1 pad2x")
+    # pitch < lambda / sqrt(2): evanescent bins on the expanded grid (fp64 per-sample path)
+    v1 = _rand((64, 64), 33)
+    _assert_parity(_gpu_asm_pad2x(api, v1, 0.3e-6, 0.3e-6, 633e-9, 5e-6), oracle.asm_pad2x(v1, 0.3e-6, 0.3e-6, 633e-9, 5e-6),
+                   "pad2x evanescent")
+    # the option changes cwo_asm only: the stack still gives the circular form; sizes above 8192 are refused
+    plan = api.cwo_plan(256, 256, cfg.pitch, cfg.lam)
+    plan.set_option(api.CWO_OPT_ASM_PAD2X, 1)
+    out = torch.empty((1, 256, 256), dtype=torch.complex64, device="cuda")
+    api.cwo_propagate_stack(plan, _dev(u1), [cfg.zs[0]], out)
+    torch.cuda.synchronize()
+    _assert_parity(out[0].cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0]), "stack stays circular")
+    big = api.cwo_plan(16384, 32, cfg.pitch, cfg.lam)
+    with pytest.raises(api.CwoError):
+        big.set_option(api.CWO_OPT_ASM_PAD2X, 1)
+
+
+def test_asm_pad2x_4096(api, oracle):
+    cfg = W.CONFIGS["c3"]
+    u1 = W.make_field(cfg)
+    _assert_parity(_gpu_asm_pad2x(api, u1, cfg.pitch, cfg.pitch, cfg.lam, 0.1), oracle.asm_pad2x(u1, cfg.pitch, cfg.pitch, cfg.lam, 0.1),
+                   "asm pad2x 4096")
