@@ -10,8 +10,8 @@ inverse row pass) over one 4096 x 4096 complex64 field of BASELINE.json config c
   value      whole-job propagations/s, inputs resident in HBM, CUDA events on the launching stream
   e2e        same metric through the public binding with HOST (pinned) buffers: H2D of u1 and D2H of
              u2 inside the timed region
-  roofline   the dominant kernel (fused column pass): algorithmic 16*N^2 bytes per launch / its
-             average duration from CUDA events recorded by the library (CWO_OPT_TIMING)
+  roofline   the dominant kernel (c3: the fused column pass): algorithmic bytes (or nominal flops) per launch / its
+             average duration from CUDA events recorded by the library (include/cwo_debug.h timing mode)
   cpu_baseline  the fp64 oracle as it stands on the host cores (reported baseline, not the target)
 
 --impl reference times the oracle itself (this tier has no installable reference implementation).
@@ -48,17 +48,22 @@ def _peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def _ncu_traffic(kernel_key: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+def _ncu_traffic(workload: str, kernel_key: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a kernel, as MEASURED BY THE COMMITTED ncu --set full
+    capture (profiles/traffic.csv names the capture); a constant of the repository, not something this run measures.
+    None when no capture of that kernel of that workload is committed."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         for line in open(p):
             t = [x.strip() for x in line.split(",")]
-            if t and t[0] == kernel_key:
-                return float(t[1]) + float(t[2])
+            if len(t) >= 4 and t[0] == workload and t[1] == kernel_key:
+                return float(t[2]) + float(t[3])
     except Exception:
         pass
     return None
+
+
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 148 SMs x 128 fp32 lanes x 2 flop (FMA) x 1965 MHz (DESIGN.md 6)
 
 
 class ClockSampler:
@@ -158,8 +163,10 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": t / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": C3_DESC, "parallelism": "host cores (oracle)", "bytes_per_step": 48 * cfg.N * cfg.N,
-                       "propagations_per_step": 1},
+            "config": {"workload": C3_DESC,
+                       "l2": "working set 403 MB per step, rotating over 3 field pairs (larger than the 126 MB L2); no flush",
+                       "parallelism": "single GPU", "bytes_per_step": 48 * cfg.N * cfg.N, "propagations_per_step": 1},
+            "arm_note": "oracle on the host cores (this tier has no installable reference); config keys mirror the CUDA arm",
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -220,7 +227,9 @@ def make_workload(name, rank, torch, api, W):
                     % (name, N, N, base.lam * 1e9, base.pitch * 1e6, "{" + ",".join("%g" % z for z in zs) + "}"))
             assert name != "c3" or desc == C3_DESC, desc
         else:
-            kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2}       # R: 8 rd + 16 wr; C: 16 + 16; R': 16 rd + 8 wr
+            # two-dimensional form: R: 8 rd + 16 wr; C: 16 + 16; R': 16 rd + 8 wr.  Separable form (Fresnel, 256..8192):
+            # kind 5 = one line-convolution pass (8 rd + 8 wr), kind 6 = one transpose (8 + 8)
+            kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2, 5: 16 * n2, 6: 16 * n2}
             bps = 80 * n2
             desc = ("%s: %s %dx%d complex64 speckle field (virtual %dx%d), lambda %g nm, pitch %g um, "
                     "z cycling %s m (new z every call)" % (name, "zero-expanded ASM" if pad2x else "Fresnel convolution",
@@ -229,8 +238,13 @@ def make_workload(name, rank, torch, api, W):
         ws = (24 if (op == "asm" and not pad2x) else 32) * n2   # u1 + u2 + workspace touched per step
         l2 = ("working set %.0f MB per step, rotating over 3 field pairs (%s the 126 MB L2); no flush"
               % (ws / 1e6, "larger than" if ws > 126e6 else "FITS in"))
-        return dict(plan=plan, step=step, N=N, props_per_step=1, bytes_per_step=bps, kind_bytes=kb, e2e=e2e, desc=desc,
-                    l2=l2, metric="propagations/sec (%s); effective HBM GB/s for the algorithmic bytes" % name)
+        # nominal flops of one line-convolution launch: N lines x (4 N-point FFTs at 5 n log2 n + ~30 flops per sample for
+        # the modulation, the spectrum multiply and the recombination)
+        kf = {5: N * (20.0 * N * np.log2(N) + 30.0 * N)}
+        scheme = bps if (op == "asm") else 64 * n2          # separable Fresnel: 2 x (conv 16 + transpose 16) N^2
+        return dict(plan=plan, step=step, N=N, props_per_step=1, bytes_per_step=bps, kind_bytes=kb, kind_flops=kf, e2e=e2e,
+                    desc=desc, l2=l2, scheme_bytes_per_step=scheme,
+                    metric="propagations/sec (%s); effective HBM GB/s for the algorithmic bytes" % name)
     if op == "stack":
         cfg = W.CONFIGS["c4"]
         n = len(cfg.zs)
@@ -254,7 +268,8 @@ def make_workload(name, rank, torch, api, W):
                 pin_out.copy_(out, non_blocking=True)
             return f, 8 * n2, 8 * n2 * n
         return dict(plan=plan, step=step, N=N, props_per_step=n, bytes_per_step=32 * n2 + n * 32 * n2,
-                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: 16 * n2, 1: 16 * n2}, e2e=e2e,
+                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: 16 * 16 * n2, 1: 16 * 16 * n2}, kind_flops={},
+                    scheme_bytes_per_step=32 * n2 + n * 32 * n2, e2e=e2e,
                     desc="c4: depth stack, one 2048x2048 random-phase field to 64 planes z = 1..64 mm by ASM, lambda 633 nm, "
                          "pitch 6.4 um, out 64x2048x2048 complex64",
                     l2="spectrum (34 MB) stays in L2; the 2.1 GB output stack streams to HBM; no flush",
@@ -282,8 +297,12 @@ def make_workload(name, rank, torch, api, W):
             pin_out.copy_(d_phi, non_blocking=True)
         return f, 12 * n2, 4 * n2
     props = 2 * cfg.iters + 1
+    # separable form: 2 iters + 2 convolution passes (2 iters of them fuse two convolutions and read one amplitude:
+    # 8 rd + 4 rd + 8 wr) and 2 iters + 1 field transposes (+ 2 real ones)
+    scheme = (2 * cfg.iters) * (20 + 16) * n2 + (16 + 16 + 12 + 16 + 8 + 8) * n2
     return dict(plan=plan, step=step, N=N, props_per_step=props, bytes_per_step=cfg.iters * 168 * n2 + 84 * n2,
-                kind_bytes={0: 24 * n2, 3: 32 * n2, 1: 28 * n2}, e2e=e2e,
+                kind_bytes={0: 24 * n2, 3: 32 * n2, 1: 28 * n2, 5: 20 * n2, 6: 16 * n2},
+                kind_flops={5: 2 * N * (20.0 * N * np.log2(N) + 30.0 * N)}, scheme_bytes_per_step=scheme, e2e=e2e,
                 desc="c5: Gerchberg-Saxton, 8192x8192, Fresnel convolution forward/back, lambda 532 nm, pitch 3.74 um, z 0.3 m, "
                      "20 iterations (41 propagations per call)",
                 l2="537 MB field + 1074 MB workspace per propagation (>> 126 MB L2); no flush",
@@ -316,8 +335,8 @@ def run_cuda(args):
     plan, step, N = wl["plan"], wl["step"], wl["N"]
     if args.no_pipeline:
         plan.set_option(api.CWO_OPT_PIPELINE, 0)
-    if args.experiment:
-        plan.set_option(api.CWO_OPT_EXPERIMENT, args.experiment)
+    if args.fresnel_2d:
+        plan.set_fresnel_2d(True)
     NBUF = 3
     stream = torch.cuda.current_stream()
 
@@ -332,42 +351,59 @@ def run_cuda(args):
     barrier()
     l0 = plan.launch_count
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
     e0.record(stream)
+    marks[0].record(stream)
     for i in range(args.steps):
         step(i)
+        marks[i + 1].record(stream)      # per-step times (median); the bracket e0..e1 gives the mean the value uses
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
+    step_ms = [marks[i].elapsed_time(marks[i + 1]) for i in range(args.steps)]
     launches = plan.launch_count - l0
     ms = S.max_over_ranks(ms, device="cuda")
     value = S.whole_job_rate([args.steps * wl["props_per_step"]] * world, ms)
 
     # ---- per-kernel durations (library-recorded CUDA events on the same stream) -------------------
-    plan.set_option(api.CWO_OPT_TIMING, 1)
+    plan.set_timing(True)
     reps = min(max(args.steps, 6), 60) if wl["props_per_step"] == 1 else 2
     for i in range(reps):
         step(i)
-    tm = plan.timings()
-    plan.set_option(api.CWO_OPT_TIMING, 0)
+    tm = plan.timings(65536)
+    plan.set_timing(False)
     clocks = sampler.stop() if rank == 0 else None
     per_kind = {}
     for tag, t_ms in tm:
         per_kind.setdefault(tag & 15, []).append(t_ms)
     names = {0: "pass_R (row FFT)", 1: "pass_R' (row IFFT)", 2: "pass_C0 (column FFT)",
-             3: "pass_C (fused column FFT*H*IFFT)", 4: "pass_C' (H * column IFFT)"}
+             3: "pass_C (fused column FFT*H*IFFT)", 4: "pass_C' (H * column IFFT)",
+             5: "line convolution pass (FFT*C*IFFT per line, separable Fresnel)", 6: "transpose"}
     passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
     dom_kind = max(per_kind, key=lambda k: np.sum(per_kind[k]))
     dom_ms = float(np.mean(per_kind[dom_kind]))
     peak, peak_src = _peak()
-    alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves (DESIGN.md 6)
-    achieved = alg_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = _ncu_traffic({0: "pass_R", 1: "pass_Rinv", 3: "pass_C"}.get(dom_kind, "-")) if args.workload == "c3" else None
     tot = sum(float(np.sum(v)) for v in per_kind.values())
-    roofline = {"bound": "hbm", "kernel": names[dom_kind], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms,
-                "pass_ms": passes, "step_share": float(np.sum(per_kind[dom_kind])) / tot}
+    alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves (DESIGN.md 6)
+    hbm_gbs = alg_bytes / (dom_ms * 1e-3) / 1e9
+    traffic = _ncu_traffic(args.workload, {0: "pass_R", 1: "pass_Rinv", 3: "pass_C", 5: "lineconv", 6: "transpose"}.get(dom_kind, "-"))
+    common = {"kernel": names[dom_kind], "traffic": traffic,
+              "traffic_source": "profiles/traffic.csv (committed ncu --set full capture; not measured by this run)" if traffic else None,
+              "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms, "pass_ms": passes,
+              "step_share": float(np.sum(per_kind[dom_kind])) / tot,
+              "hbm_gbs": hbm_gbs, "hbm_frac": hbm_gbs / peak, "hbm_peak": peak, "hbm_peak_source": peak_src}
+    if dom_kind in wl.get("kind_flops", {}):
+        # the line-convolution passes are bound by the fp32 pipes, not by HBM: nominal flops per launch
+        # over the live duration against 148 SMs x 128 lanes x 2 x 1965 MHz
+        fl = wl["kind_flops"][dom_kind]
+        ach = fl / (dom_ms * 1e-3) / 1e12
+        roofline = dict(common, bound="alu", achieved=ach, peak=FP32_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / FP32_PEAK_TFLOPS,
+                        peak_source="148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
+                        nominal_flops_per_launch=fl)
+    else:
+        roofline = dict(common, bound="hbm", achieved=hbm_gbs, peak=peak, unit="GB/s", frac=hbm_gbs / peak,
+                        peak_source=peak_src)
 
     # ---- end to end: host (pinned) buffers, H2D + propagate + D2H every step -----------------------
     e2e_step, h2d, d2h = wl["e2e"]()
@@ -396,15 +432,18 @@ def run_cuda(args):
         ms_step = ms / args.steps
         eff = wl["bytes_per_step"] / (ms_step * 1e-3) / 1e9
         line = {"metric": METRIC if args.workload == "c3" else wl["metric"], "value": value, "unit": UNIT, "n_gpus": world,
-                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+                "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_min": float(np.min(step_ms)),
+                "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": wl["desc"], "l2": wl["l2"],
                            "parallelism": "replicas" if world > 1 else "single GPU",
                            "bytes_per_step": int(wl["bytes_per_step"]), "propagations_per_step": wl["props_per_step"]},
                 "effective_gbs": eff, "pct_of_8TBs": 100.0 * eff / NOMINAL_HBM_GBS, "pct_of_measured_copy": 100.0 * eff / peak,
+                "scheme_bytes_per_step": int(wl["scheme_bytes_per_step"]),
                 "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
-        if args.experiment or args.no_pipeline:
-            line["not_a_benchmark"] = "experiment=%d no_pipeline=%d" % (args.experiment, int(args.no_pipeline))
+        if args.fresnel_2d or args.no_pipeline:
+            line["not_a_benchmark"] = "fresnel_2d=%d no_pipeline=%d" % (int(args.fresnel_2d), int(args.no_pipeline))
         if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
             line["cpu_baseline"] = cpu_baseline(W.CONFIGS["c3"])
         print(json.dumps(line), flush=True)
@@ -415,18 +454,19 @@ def run_cuda(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--steps", type=int, default=None, help="default: 300 for c3, fewer for the long workloads")
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-pipeline", action="store_true",
                     help="CWO_OPT_PIPELINE = 0: one CTA per tile everywhere (comparison runs only)")
-    ap.add_argument("--experiment", type=int, default=0,
-                    help="CWO_OPT_EXPERIMENT bit mask (1: no global stores, 4: no global loads in the persistent kernels); "
-                         "results are wrong, the line is marked and is not a benchmark value")
+    ap.add_argument("--fresnel-2d", action="store_true",
+                    help="cwo_debug_set_fresnel_2d: three-pass two-dimensional Fresnel form (comparison runs only)")
     ap.add_argument("--workload", default="c3", choices=sorted(WORKLOADS),
                     help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()
+    if args.steps is None:
+        args.steps = {"c5": 3, "c4": 20, "fresnel8192": 50, "asm8192": 100}.get(args.workload, 300)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -10,16 +10,17 @@
  *              Nx), 16-byte aligned.  Complex fields are interleaved (re, im) float pairs
  *              (8*Nx*Ny bytes); real fields are float (4*Nx*Ny bytes).
  *   Ownership  The caller owns every buffer, including the workspace.  A plan owns only small
- *              lookup tables (a few MiB at most) that it allocates with cudaMalloc at plan time or on the
- *              first call that needs them.  No call allocates or frees caller-visible memory.
- *   Asynchrony Every propagation call only enqueues kernels on the plan's stream and returns;
- *              results are valid once the caller has synchronised that stream.  No hidden
- *              host<->device copies of field data.  Host arrays (zs) are read before return.
+ *              lookup tables (a few MiB at most); ALL of them are allocated, built and synchronised
+ *              inside cwo_plan().  No other call allocates, frees or synchronises anything.
+ *   Asynchrony cwo_asm / cwo_fresnel_conv / cwo_propagate_stack / cwo_gs only ENQUEUE kernels on the
+ *              plan's stream and return (they may be captured into a CUDA graph); results are valid
+ *              once the caller has synchronised that stream.  No host<->device copies.  Host arrays
+ *              (zs) are read before return.
  *   Aliasing   u2 == u1 (exact in-place, as the paper's c.Diffract) is allowed.
  *              Partial overlap, or overlap with the workspace, is the caller's error.
  *   Errors     int return, CWO_OK == 0, negative on failure.  Nothing is enqueued when a call
  *              returns CWO_EINVAL / CWO_EWORKSPACE / CWO_EUNSUPPORTED.  No exceptions, no
- *              global state; use one plan per host thread at a time.
+ *              global state; use one plan per host thread at a time, on the device it was made on.
  *   Sizes      Nx, Ny powers of two.  cwo_asm / cwo_propagate_stack: 32..16384 per axis.
  *              cwo_fresnel_conv (transforms of 2Nx x 2Ny): 16..8192 per axis.  cwo_gs: the
  *              range of its propagator.
@@ -42,10 +43,11 @@ typedef struct { float re, im; } cwo_c64;      /* == float2 == torch.complex64 e
 enum {
     CWO_OK = 0,
     CWO_EINVAL = -1,        /* bad argument: null/unaligned pointer, unsupported size, lambda/pitch <= 0,
-                               non-finite z, z == 0 for Fresnel, n <= 0, iters < 0 */
+                               non-finite z, z == 0 for Fresnel, n <= 0, iters < 0, plan used on another device */
     CWO_EWORKSPACE = -2,    /* workspace missing or smaller than cwo_plan_workspace_bytes() */
     CWO_EUNSUPPORTED = -3,  /* current device is not compute capability 10.x */
-    CWO_ECUDA = -4          /* CUDA runtime failure; code via cwo_last_cuda_error() */
+    CWO_ECUDA = -4,         /* CUDA runtime failure; code via cwo_last_cuda_error() */
+    CWO_ENOMEM = -5         /* host or device allocation failed in cwo_plan() */
 };
 
 enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4 };
@@ -53,26 +55,26 @@ enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4 };
 enum {
     CWO_OPT_GS_METHOD = 1,  /* value: CWO_GS_FRESNEL (default; BASELINE config 5) or CWO_GS_ASM
                                (the paper's Listing 8) */
-    CWO_OPT_TIMING = 2,     /* value 1: bracket every pass kernel with a CUDA event pair on the plan's
-                               stream (read with cwo_plan_timings); 0 (default): off */
-    CWO_OPT_PIPELINE = 3,   /* value 1 (default): the row passes (and the depth stack's column passes) of transform
-                               lengths 1024..4096 run as persistent CTAs that prefetch their next tiles (TMA);
+    CWO_OPT_PIPELINE = 3,   /* value 1 (default): persistent, prefetching kernels where they exist;
                                0: one CTA per tile everywhere.  Same arithmetic either way. */
     CWO_OPT_ASM_PAD2X = 5,  /* value 1: cwo_asm runs on the calculation area expanded to 2Nx x 2Ny with zeros and crops
                                (the paper's own form of the method, Table 2: no wrap-around; frequency
                                sampling 1/(2 N pitch)); needs Nx, Ny <= 8192 and a workspace of 16*Nx*Ny.  Default 0:
                                circular Nx x Ny form.  cwo_propagate_stack and cwo_gs always use the circular form. */
-    CWO_OPT_EXPERIMENT = 4  /* measurement aid, default 0.  Bit 0: the persistent kernels skip their global stores;
-                               bit 2: they skip their global loads (they transform whatever the buffers hold).
-                               RESULTS ARE WRONG with any bit set: it exists to time the on-chip part of a pass
-                               (DESIGN.md section 6). */
+    CWO_OPT_STACK_INTENSITY = 6, /* value 1: cwo_propagate_stack writes the INTENSITY |u|^2 of every plane (Eq.(20),
+                               P:L254-256; the quantity the paper's 3-D example renders) as float [n][Ny][Nx]
+                               instead of the complex amplitude: half the output bytes.  Default 0. */
+    CWO_OPT_ASM_BAND_LIMIT = 7 /* value 1: cwo_asm multiplies the transfer function by the two Rect band limits of
+                               Eq.(18)-(19) for the on-axis case: bins with |fx| > 1/(lambda
+                               sqrt((2 dfx z)^2 + 1)) (same in y) are zeroed, which removes the aliased part of H at
+                               long distances.  Default 0. */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
 
 /* Plane parameters (SetPitch / SetWaveLength / Create).  pitch_x = pitch_y = pitch
  * [m], lambda [m].  Frequency sampling is 1/(M*pitch) with M the transform size.
- * Builds the FFT twiddle tables on the current CUDA device (tiny kernels on the null stream,
- * synchronised before return). */
+ * Allocates and builds every table the plan will ever need on the current CUDA device (tiny kernels
+ * on the null stream, synchronised before return); the plan must be used on that device. */
 int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t* plan_out);
 int cwo_plan_destroy(cwo_plan_t plan);
 
@@ -84,12 +86,22 @@ int cwo_plan_set_pitch_xy(cwo_plan_t plan, double px, double py);
 
 int cwo_plan_set_option(cwo_plan_t plan, int key, int value);
 
+/* Shifted angular spectrum method (Eq.(18)-(19); the paper's SetOffset): with CWO_OPT_ASM_BAND_LIMIT
+ * on, cwo_asm samples the destination plane on a window displaced by (ox, oy) metres from the axis of the source
+ * window: H is multiplied by the phase ramp exp(i 2 pi (ox fx + oy fy)) and the band limits follow the shift.
+ * Default (0, 0): on-axis, band-limited only. */
+int cwo_plan_set_offset(cwo_plan_t plan, double ox, double oy);
+
 /* Workspace a call needs, in bytes (n = number of planes for CWO_OP_STACK, ignored otherwise):
- *   ASM      8*Nx*Ny            (the row-transformed field in column-tile order)
- *   FRESNEL  16*Nx*Ny           (Ny rows x 2Nx columns; the 2Nx x 2Ny padded array is never stored)
- *   STACK    8*Nx*Ny*(1 + min(n, 16))   (spectrum + the planes in flight between their column and row pass;
- *            cwo_propagate_stack accepts anything >= 16*Nx*Ny and batches as many planes as fit)
- *   GS       propagator's workspace + 8*Nx*Ny (the constrained field between propagations)
+ *   ASM      8*Nx*Ny            the row-transformed field in column-tile order; needed for u2 != u1 too, because
+ *                               the inverse row pass cannot write row-major rows over the column-tiled data it reads
+ *            (16*Nx*Ny with CWO_OPT_ASM_PAD2X)
+ *   FRESNEL  16*Nx*Ny           two copies of the field (the 2Nx x 2Ny padded array is never stored)
+ *   STACK    8*Nx*Ny*(1 + min(n, 16)) + 4*n*(Nx+Ny+1) rounded up to 256
+ *                               spectrum + the planes in flight between their column and row pass + the planes'
+ *                               phase tables; cwo_propagate_stack accepts anything >= 16*Nx*Ny + the tables and
+ *                               batches as many planes as fit
+ *   GS       24*Nx*Ny (Fresnel) / 16*Nx*Ny (ASM)
  * Returns 0 for an unknown op. */
 size_t cwo_plan_workspace_bytes(cwo_plan_t plan, int op, int n);
 
@@ -110,8 +122,8 @@ int cwo_fresnel_conv(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
 
 /* 3-D diffraction as a stack of 2-D diffractions (Diffract3D): out[k] = cwo_asm(u1, zs[k]),
  * k = 0..n-1, the forward FFT of u1 computed once.  zs: HOST array of n doubles.  out: device,
- * [n][Ny][Nx] complex; must not overlap u1. */
-int cwo_propagate_stack(cwo_plan_t plan, const cwo_c64* u1, const double* zs, int n, cwo_c64* out);
+ * [n][Ny][Nx] complex (float intensities with CWO_OPT_STACK_INTENSITY); must not overlap u1. */
+int cwo_propagate_stack(cwo_plan_t plan, const cwo_c64* u1, const double* zs, int n, void* out);
 
 /* Gerchberg-Saxton loop (section 7.2, Listing 8) between a source (hologram)
  * plane with amplitude amp_src and a destination (image) plane with amplitude amp_dst, z apart:
@@ -126,16 +138,6 @@ int cwo_gs(cwo_plan_t plan, const float* amp_src, const float* amp_dst, double z
 
 const char* cwo_strerror(int code);
 int cwo_last_cuda_error(cwo_plan_t plan);
-
-/* With CWO_OPT_TIMING on: synchronises the plan's stream, writes the device time in ms of each pass
- * kernel launched since the option was set / since the last call (at most cap entries; tag_out, if
- * not NULL, receives log2(transform length)*16 + kind, kind 0 = forward, 1 = inverse, 2 = fused
- * forward x H x inverse, 3 = H x inverse), clears the record and returns the number of launches
- * recorded (may exceed cap), or a negative error. */
-int cwo_plan_timings(cwo_plan_t plan, float* ms_out, int* tag_out, int cap);
-
-/* Number of kernels the library has launched through this plan so far (bench accounting). */
-long long cwo_plan_launch_count(cwo_plan_t plan);
 
 #ifdef __cplusplus
 }

@@ -20,19 +20,20 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("CWO_LIBRARY_PATH") or os.path.join(_HERE, "libcwo.so")
 
-CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA = 0, -1, -2, -3, -4
+CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA, CWO_ENOMEM = 0, -1, -2, -3, -4, -5
 CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS = 1, 2, 3, 4
 CWO_OPT_GS_METHOD = 1
-CWO_OPT_TIMING = 2
 CWO_OPT_PIPELINE = 3
-CWO_OPT_EXPERIMENT = 4
 CWO_OPT_ASM_PAD2X = 5
+CWO_OPT_STACK_INTENSITY = 6
+CWO_OPT_ASM_BAND_LIMIT = 7
 CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 
+# include/cwo.h (the product boundary) and include/cwo_debug.h (measurement hooks of the harness)
 EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",
-           "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_asm", "cwo_fresnel_conv",
-           "cwo_propagate_stack", "cwo_gs", "cwo_strerror", "cwo_last_cuda_error", "cwo_plan_launch_count",
-           "cwo_plan_timings"]
+           "cwo_plan_set_offset", "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_asm", "cwo_fresnel_conv",
+           "cwo_propagate_stack", "cwo_gs", "cwo_strerror", "cwo_last_cuda_error"]
+DEBUG_EXPORTS = ["cwo_debug_set_timing", "cwo_debug_timings", "cwo_debug_launch_count", "cwo_debug_set_fresnel_2d"]
 
 _lib = None
 
@@ -61,6 +62,7 @@ def lib() -> ctypes.CDLL:
     L.cwo_plan_set_stream.argtypes = [vp, vp]
     L.cwo_plan_set_pitch_xy.argtypes = [vp, D, D]
     L.cwo_plan_set_option.argtypes = [vp, I, I]
+    L.cwo_plan_set_offset.argtypes = [vp, D, D]
     L.cwo_plan_workspace_bytes.argtypes = [vp, I, I]
     L.cwo_plan_workspace_bytes.restype = sz
     L.cwo_plan_set_workspace.argtypes = [vp, vp, sz]
@@ -71,9 +73,11 @@ def lib() -> ctypes.CDLL:
     L.cwo_strerror.argtypes = [I]
     L.cwo_strerror.restype = ctypes.c_char_p
     L.cwo_last_cuda_error.argtypes = [vp]
-    L.cwo_plan_launch_count.argtypes = [vp]
-    L.cwo_plan_launch_count.restype = ctypes.c_longlong
-    L.cwo_plan_timings.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(I), I]
+    L.cwo_debug_launch_count.argtypes = [vp]
+    L.cwo_debug_launch_count.restype = ctypes.c_longlong
+    L.cwo_debug_timings.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(I), I]
+    L.cwo_debug_set_timing.argtypes = [vp, I]
+    L.cwo_debug_set_fresnel_2d.argtypes = [vp, I]
     _lib = L
     return L
 
@@ -85,6 +89,7 @@ class Plan:
         self.Nx, self.Ny = int(Nx), int(Ny)
         self._h = ctypes.c_void_p()
         self._ws = None
+        self.stack_intensity = False
         rc = lib().cwo_plan(self.Nx, self.Ny, float(pitch), float(lam), ctypes.byref(self._h))
         if rc != CWO_OK:
             raise CwoError(rc, "cwo_plan")
@@ -98,6 +103,18 @@ class Plan:
 
     def set_option(self, key: int, value: int) -> None:
         self._check(lib().cwo_plan_set_option(self._h, int(key), int(value)), "cwo_plan_set_option")
+        if key == CWO_OPT_STACK_INTENSITY:
+            self.stack_intensity = bool(value)
+
+    def set_offset(self, ox: float, oy: float) -> None:
+        self._check(lib().cwo_plan_set_offset(self._h, float(ox), float(oy)), "cwo_plan_set_offset")
+
+    # include/cwo_debug.h: measurement hooks (harness only)
+    def set_timing(self, on: bool) -> None:
+        self._check(lib().cwo_debug_set_timing(self._h, int(bool(on))), "cwo_debug_set_timing")
+
+    def set_fresnel_2d(self, on: bool) -> None:
+        self._check(lib().cwo_debug_set_fresnel_2d(self._h, int(bool(on))), "cwo_debug_set_fresnel_2d")
 
     def workspace_bytes(self, op: int, n: int = 0) -> int:
         return int(lib().cwo_plan_workspace_bytes(self._h, int(op), int(n)))
@@ -112,24 +129,29 @@ class Plan:
 
     def ensure_workspace(self, op: int, n: int = 0) -> None:
         need = self.workspace_bytes(op, n)
-        have = 0 if self._ws is None else self._ws.numel()
+        have = 0 if self._ws is None else self._ws.numel() * self._ws.element_size()
         if have < need:
+            old = self._ws
             self.set_workspace(torch.empty(need, dtype=torch.uint8, device="cuda"))
+            if old is not None:
+                # kernels enqueued on the plan's stream may still use the old block: keep the allocator from handing
+                # it out before they are done
+                old.record_stream(torch.cuda.current_stream())
 
     def bind_stream(self) -> None:
         self._check(lib().cwo_plan_set_stream(self._h, torch.cuda.current_stream().cuda_stream), "cwo_plan_set_stream")
 
     def timings(self, cap: int = 4096):
-        """[(tag, ms), ...] of the pass kernels launched since CWO_OPT_TIMING was set / last read."""
+        """[(tag, ms), ...] of the pass kernels launched since timing was switched on / last read."""
         ms = (ctypes.c_float * cap)(); tag = (ctypes.c_int * cap)()
-        n = lib().cwo_plan_timings(self._h, ms, tag, cap)
+        n = lib().cwo_debug_timings(self._h, ms, tag, cap)
         if n < 0:
-            self._check(n, "cwo_plan_timings")
+            self._check(n, "cwo_debug_timings")
         return [(int(tag[i]), float(ms[i])) for i in range(min(n, cap))]
 
     @property
     def launch_count(self) -> int:
-        return int(lib().cwo_plan_launch_count(self._h))
+        return int(lib().cwo_debug_launch_count(self._h))
 
     def close(self) -> None:
         if self._h:
@@ -171,7 +193,7 @@ def cwo_fresnel_conv(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -
 def cwo_propagate_stack(plan: Plan, u1: torch.Tensor, zs: Sequence[float], out: torch.Tensor) -> None:
     n = len(zs)
     a = _field(u1, torch.complex64, (plan.Ny, plan.Nx), "u1")
-    b = _field(out, torch.complex64, (n, plan.Ny, plan.Nx), "out")
+    b = _field(out, torch.float32 if plan.stack_intensity else torch.complex64, (n, plan.Ny, plan.Nx), "out")
     arr = (ctypes.c_double * n)(*[float(z) for z in zs])
     plan.ensure_workspace(CWO_OP_STACK, n); plan.bind_stream()
     plan._check(lib().cwo_propagate_stack(plan._h, a, arr, n, b), "cwo_propagate_stack")
@@ -202,11 +224,16 @@ class HostPipeline:
         self.d_in = [torch.empty(shape, dtype=torch.complex64, device="cuda") for _ in range(self.depth)]
         self.d_out = [torch.empty(shape, dtype=torch.complex64, device="cuda") for _ in range(self.depth)]
         self.s_in, self.s_run, self.s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+        for t in self.d_in + self.d_out:          # allocated under the current stream, used on the private ones
+            for st in (self.s_in, self.s_run, self.s_out):
+                t.record_stream(st)
         self.ev_in = [torch.cuda.Event() for _ in range(self.depth)]     # H2D of slot k done
         self.ev_run = [torch.cuda.Event() for _ in range(self.depth)]    # kernels of slot k done
         self.ev_out = [torch.cuda.Event() for _ in range(self.depth)]    # D2H of slot k done
         self.used = [False] * self.depth
         plan.ensure_workspace(CWO_OP_ASM if op == "asm" else CWO_OP_FRESNEL)
+        if plan._ws is not None:
+            plan._ws.record_stream(self.s_run)
 
     def start_after(self, stream: "torch.cuda.Stream") -> None:
         """Order everything submitted from now on after the work already queued on `stream`."""

@@ -29,6 +29,7 @@ def _sources():
         if f.endswith((".cu", ".cuh", ".h")):
             out.append(os.path.join(CSRC, f))
     out.append(os.path.join(ROOT, "include", "cwo.h"))
+    out.append(os.path.join(ROOT, "include", "cwo_debug.h"))
     return out
 
 
@@ -49,26 +50,6 @@ def _run(cmd, verbose):
     return r.stdout
 
 
-def build_variant(out_lib: str, extra_flags, logns=None, verbose: bool = False) -> str:
-    """Experiment helper: build a variant library (extra nvcc flags) into out_lib without touching libcwo.so."""
-    obj = out_lib + ".obj"
-    os.makedirs(obj, exist_ok=True)
-    flags = NVCC_FLAGS + list(extra_flags) + ["-Xptxas", "-v"]
-    jobs = []
-    for k in (logns or LOGNS):
-        o = os.path.join(obj, "pass_%d.o" % k)
-        jobs.append((["nvcc"] + flags + ["-DCWO_LOGN=%d" % k, "-c", os.path.join(CSRC, "pass_inst.cu"), "-o", o], o))
-    for name in ("tables", "cwo"):
-        o = os.path.join(obj, name + ".o")
-        jobs.append((["nvcc"] + flags + ["-c", os.path.join(CSRC, name + ".cu"), "-o", o], o))
-    with cf.ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
-        logs = list(ex.map(lambda j: _run(j[0], verbose), jobs))
-    _run(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out_lib] + [j[1] for j in jobs]
-         + ["-lcudart"], verbose)
-    open(os.path.join(obj, "ptxas.log"), "w").write("\n".join(logs))
-    return out_lib
-
-
 def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     stamp_file = os.path.join(OBJ, "stamp")
@@ -81,7 +62,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     for k in LOGNS:
         o = os.path.join(OBJ, "pass_%d.o" % k)
         jobs.append((["nvcc"] + flags + ["-DCWO_LOGN=%d" % k, "-c", os.path.join(CSRC, "pass_inst.cu"), "-o", o], o))
-    for name in ("tables", "cwo"):
+    for name in ("tables", "transpose", "cwo"):
         o = os.path.join(OBJ, name + ".o")
         jobs.append((["nvcc"] + flags + ["-c", os.path.join(CSRC, name + ".cu"), "-o", o], o))
     logs = []

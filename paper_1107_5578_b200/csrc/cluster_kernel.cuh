@@ -98,12 +98,14 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, 1) cluster_row_fwd_kernel(const
 template <int LOGN, bool PAD>
 static cudaError_t launch_cluster_row_fwd(int n_rows, cudaStream_t s, const PassParams& p) {
     constexpr size_t smem = Tile<LOGN>::SMEM_BYTES + 64;
-    static bool configured = false;
-    if (!configured) {
+    DeviceInfo* d = device_info();
+    if (!d) return cudaErrorInvalidDevice;
+    static FuncOnce once;
+    if (!once.done(d->index)) {
         cudaError_t e = cudaFuncSetAttribute(cluster_row_fwd_kernel<LOGN, PAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        once.set(d->index);
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)n_rows); cfg.blockDim = dim3((unsigned)Tile<LOGN>::T);
@@ -112,12 +114,14 @@ static cudaError_t launch_cluster_row_fwd(int n_rows, cudaStream_t s, const Pass
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = CLUSTER_ROWS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    static int wave = 0;                                    // CTAs of the clusters that are resident at once
+    static std::atomic<int> waves[MAX_DEVICES];             // CTAs of the clusters that are resident at once, per device
+    int wave = waves[d->index].load(std::memory_order_acquire);
     if (!wave) {
         int nc = 0;
         cudaError_t e = cudaOccupancyMaxActiveClusters(&nc, cluster_row_fwd_kernel<LOGN, PAD>, &cfg);
         if (e != cudaSuccess) return e;
         wave = (nc > 0 ? nc : 1) * CLUSTER_ROWS;
+        waves[d->index].store(wave, std::memory_order_release);
     }
     if (n_rows > wave) cfg.gridDim = dim3((unsigned)wave);
     PassParams q = p;

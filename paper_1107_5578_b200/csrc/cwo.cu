@@ -1,6 +1,8 @@
 // cwo.cu -- the C ABI of libcwo.so (include/cwo.h): plan object, argument checks, and the
 // sequencing of the streaming passes that make up each call.  All arithmetic on field data
-// happens in the kernels of pass_kernel.cuh / tables.cu; nothing here touches field values.
+// happens in the kernels of csrc/*.cuh, tables.cu and transpose.cu; nothing here touches field values.
+// Every allocation and every synchronisation happens in cwo_plan(); the propagation calls only enqueue
+// (include/cwo_debug.h's timing mode excepted).
 #include <math.h>
 #include <new>
 #include <stdint.h>
@@ -9,31 +11,30 @@
 #include <vector>
 
 #include "../../include/cwo.h"
+#include "../../include/cwo_debug.h"
 #include "cwo_internal.h"
 
 using namespace cwo;
 
 struct cwo_plan_s {
     int Nx, Ny, lognx, logny;
+    int device;                     // the device the plan's tables live on
     double px, py, lambda;
+    double off_x, off_y;            // shifted angular spectrum method: destination offset [m] (Eq.(19))
     cudaStream_t stream;
     void* ws;
     size_t ws_bytes;
-    int gs_method;
-    int pipeline;
-    int experiment;                 // CWO_OPT_EXPERIMENT bit mask
-    int asm_pad2x;                  // CWO_OPT_ASM_PAD2X
+    int gs_method, pipeline, asm_pad2x, stack_intensity, band_limit, fresnel_2d;
     int last_cuda_error;
     long long launches;
-    float2* tw[MAX_LOGN + 2];       // fp32 twiddles per log2 length (lazily built)
+    float2* tw[MAX_LOGN + 2];       // fp32 twiddles per log2 length
     double2* tw64[MAX_LOGN + 2];    // fp64 twiddles for the chirp FFT
-    float2* chirp[2][2];            // [set][axis] Fresnel spectra Cx, Cy (set 0: +z, 1: the other sign in GS)
+    float2* chirp[2][2];            // [set][axis] Fresnel spectra Cx, Cy (set 0: the call's z / -z in GS, 1: +z in GS)
+    float4* chirp_pairs[2][2];      // the same as planar (even bin, odd bin) pairs (separable form)
     double2* chirp_scratch;         // 2 axes x 2M
-    float* asm_tab;                 // ASM split path: per plane [theta_x (Mx) | theta_y (My)]
-    int asm_tab_planes;             // capacity of asm_tab in planes
-    float* stack_resc;              // batched stack: z/lambda of every plane
-    int stack_resc_cap;
-    // CWO_OPT_TIMING: one CUDA event pair around every pass kernel
+    int* tile_counter;              // persistent line-convolution kernels: {next tile, CTAs done}, zero between launches
+    float* asm_tab;                 // ASM split path, one plane: [theta_x (Mx) | theta_y (My)], M up to 2N
+    // include/cwo_debug.h: one CUDA event pair around every pass kernel
     int timing;
     std::vector<cudaEvent_t>* ev;   // 2 per recorded launch
     std::vector<int>* ev_tag;       // logn*16 + kind
@@ -62,8 +63,14 @@ static const pass_launcher_t kLaunchers[MAX_LOGN + 1] = {
     nullptr, nullptr, nullptr, nullptr, nullptr,
     launch_pass_5, launch_pass_6, launch_pass_7, launch_pass_8, launch_pass_9,
     launch_pass_10, launch_pass_11, launch_pass_12, launch_pass_13, launch_pass_14};
+static const conv_launcher_t kConv[MAX_LOGN + 1] = {
+    nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+    launch_conv_8, launch_conv_9, launch_conv_10, launch_conv_11, launch_conv_12, launch_conv_13, nullptr};
+enum { KIND_CONV = 5, KIND_TRANSPOSE = 6 };
 
-static int launch(cwo_plan_t p, int logn, int kind, int pad, int mid, int n_tiles, const PassParams& pp) {
+// One kernel launch `f` (returns cudaError_t), counted, and bracketed by an event pair in timing mode.
+template <class F>
+static int launch_tagged(cwo_plan_t p, int tag, F f) {
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (p->timing) {
         while (p->ev->size() < 2 * (p->ev_used + 1)) {
@@ -73,32 +80,58 @@ static int launch(cwo_plan_t p, int logn, int kind, int pad, int mid, int n_tile
         }
         e0 = (*p->ev)[2 * p->ev_used]; e1 = (*p->ev)[2 * p->ev_used + 1];
         if (p->ev_tag->size() <= p->ev_used) p->ev_tag->push_back(0);
-        (*p->ev_tag)[p->ev_used] = logn * 16 + kind;
+        (*p->ev_tag)[p->ev_used] = tag;
         p->ev_used++;
         CWO_CUDA(p, cudaEventRecord(e0, p->stream));
     }
-    CWO_CUDA(p, kLaunchers[logn](kind, pad, mid, n_tiles, p->stream, pp));
+    CWO_CUDA(p, f());
     if (p->timing) CWO_CUDA(p, cudaEventRecord(e1, p->stream));
     p->launches++;
     return CWO_OK;
 }
 
-static int ensure_twiddles(cwo_plan_t p, int logn, bool want64) {
-    const int n = 1 << logn;
-    const bool built = !p->tw[logn] || (want64 && !p->tw64[logn]);
-    if (!p->tw[logn]) {
-        CWO_CUDA(p, cudaMalloc(&p->tw[logn], sizeof(float2) * n));
-        CWO_CUDA(p, build_twiddles(p->tw[logn], n, p->stream));
+static int launch(cwo_plan_t p, int logn, int kind, int pad, int mid, int n_tiles, const PassParams& pp) {
+    return launch_tagged(p, logn * 16 + kind, [&] { return kLaunchers[logn](kind, pad, mid, n_tiles, p->stream, pp); });
+}
+
+static bool fresnel_sizes_ok(cwo_plan_t p) { return p->lognx + 1 <= MAX_LOGN && p->logny + 1 <= MAX_LOGN; }
+static bool asm_sizes_ok(cwo_plan_t p) { return p->lognx >= MIN_LOGN && p->logny >= MIN_LOGN; }
+
+// ---- plan -------------------------------------------------------------------------------------------------
+
+static int plan_alloc_and_build(cwo_plan_t p) {
+    // twiddles: every transform length a call on this plan can use (N and 2N per axis)
+    const int lens[4] = {p->lognx, p->logny, p->lognx + 1, p->logny + 1};
+    for (int i = 0; i < 4; ++i) {
+        const int l = lens[i];
+        if (l > MAX_LOGN || p->tw[l]) continue;
+        const int n = 1 << l;
+        CWO_CUDA(p, cudaMalloc(&p->tw[l], sizeof(float2) * n));
+        CWO_CUDA(p, build_twiddles(p->tw[l], n, 0));
         p->launches++;
     }
-    if (want64 && !p->tw64[logn]) {
-        CWO_CUDA(p, cudaMalloc(&p->tw64[logn], sizeof(double2) * (n / 2)));
-        CWO_CUDA(p, build_twiddles_f64(p->tw64[logn], n, p->stream));
-        p->launches++;
+    const bool pad_ok = fresnel_sizes_ok(p);
+    if (pad_ok) {
+        const int mx = 2 * p->Nx, my = 2 * p->Ny;
+        for (int i = 2; i < 4; ++i) {
+            const int l = lens[i];
+            if (p->tw64[l]) continue;
+            CWO_CUDA(p, cudaMalloc(&p->tw64[l], sizeof(double2) * ((size_t)1 << (l - 1))));
+            CWO_CUDA(p, build_twiddles_f64(p->tw64[l], 1 << l, 0));
+            p->launches++;
+        }
+        for (int s = 0; s < 2; ++s) {
+            CWO_CUDA(p, cudaMalloc(&p->chirp[s][0], sizeof(float2) * mx));
+            CWO_CUDA(p, cudaMalloc(&p->chirp[s][1], sizeof(float2) * my));
+            CWO_CUDA(p, cudaMalloc(&p->chirp_pairs[s][0], sizeof(float4) * p->Nx));
+            CWO_CUDA(p, cudaMalloc(&p->chirp_pairs[s][1], sizeof(float4) * p->Ny));
+        }
+        CWO_CUDA(p, cudaMalloc(&p->chirp_scratch, sizeof(double2) * 2 * ((size_t)mx + my)));
     }
-    // the pipelined kernels read these tables before they wait for their predecessor (programmatic dependent
-    // launch), so a table built on demand must be complete before anything else is enqueued (once per length)
-    if (built) CWO_CUDA(p, cudaStreamSynchronize(p->stream));
+    CWO_CUDA(p, cudaMalloc(&p->tile_counter, 2 * sizeof(int)));
+    CWO_CUDA(p, cudaMemsetAsync(p->tile_counter, 0, 2 * sizeof(int), 0));
+    CWO_CUDA(p, cudaMalloc(&p->asm_tab, sizeof(float) * (size_t)(pad_ok ? 2 : 1) * (p->Nx + p->Ny)));
+    CWO_CUDA(p, cudaStreamSynchronize(0));
     return CWO_OK;
 }
 
@@ -113,19 +146,20 @@ extern "C" int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t*
     if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return CWO_ECUDA;
     if (major != 10) return CWO_EUNSUPPORTED;
     cwo_plan_t p = new (std::nothrow) cwo_plan_s;
-    if (!p) return CWO_EINVAL;
+    if (!p) return CWO_ENOMEM;
     memset(p, 0, sizeof(*p));
-    p->Nx = Nx; p->Ny = Ny; p->lognx = lx; p->logny = ly;
+    p->Nx = Nx; p->Ny = Ny; p->lognx = lx; p->logny = ly; p->device = dev;
     p->px = p->py = pitch; p->lambda = lambda;
     p->gs_method = CWO_GS_FRESNEL;
     p->pipeline = 1;
-    p->ev = new std::vector<cudaEvent_t>();
-    p->ev_tag = new std::vector<int>();
-    int rc = CWO_OK;
-    if (lx >= MIN_LOGN) rc = ensure_twiddles(p, lx, false);
-    if (rc == CWO_OK && ly >= MIN_LOGN) rc = ensure_twiddles(p, ly, false);
-    if (rc == CWO_OK && cudaStreamSynchronize(0) != cudaSuccess) rc = CWO_ECUDA;
-    if (rc != CWO_OK) { cwo_plan_destroy(p); return rc; }
+    p->ev = new (std::nothrow) std::vector<cudaEvent_t>();
+    p->ev_tag = new (std::nothrow) std::vector<int>();
+    int rc = (p->ev && p->ev_tag) ? plan_alloc_and_build(p) : CWO_ENOMEM;
+    if (rc != CWO_OK) {
+        if (rc == CWO_ECUDA && p->last_cuda_error == (int)cudaErrorMemoryAllocation) rc = CWO_ENOMEM;
+        cwo_plan_destroy(p);
+        return rc;
+    }
     *plan_out = p;
     return CWO_OK;
 }
@@ -133,10 +167,10 @@ extern "C" int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t*
 extern "C" int cwo_plan_destroy(cwo_plan_t p) {
     if (!p) return CWO_EINVAL;
     for (int i = 0; i < MAX_LOGN + 2; ++i) { cudaFree(p->tw[i]); cudaFree(p->tw64[i]); }
-    for (int s = 0; s < 2; ++s) for (int a = 0; a < 2; ++a) cudaFree(p->chirp[s][a]);
+    for (int s = 0; s < 2; ++s) for (int a = 0; a < 2; ++a) { cudaFree(p->chirp[s][a]); cudaFree(p->chirp_pairs[s][a]); }
     cudaFree(p->chirp_scratch);
     cudaFree(p->asm_tab);
-    cudaFree(p->stack_resc);
+    cudaFree(p->tile_counter);
     if (p->ev) { for (cudaEvent_t e : *p->ev) cudaEventDestroy(e); delete p->ev; }
     delete p->ev_tag;
     delete p;
@@ -155,41 +189,45 @@ extern "C" int cwo_plan_set_pitch_xy(cwo_plan_t p, double px, double py) {
     return CWO_OK;
 }
 
+extern "C" int cwo_plan_set_offset(cwo_plan_t p, double ox, double oy) {
+    if (!p || !isfinite(ox) || !isfinite(oy)) return CWO_EINVAL;
+    p->off_x = ox; p->off_y = oy;
+    return CWO_OK;
+}
+
 extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
     if (!p) return CWO_EINVAL;
-    if (key == CWO_OPT_GS_METHOD && (value == CWO_GS_FRESNEL || value == CWO_GS_ASM)) {
-        p->gs_method = value;
-        return CWO_OK;
-    }
-    if (key == CWO_OPT_PIPELINE && (value == 0 || value == 1)) {
-        p->pipeline = value;
-        return CWO_OK;
-    }
-    if (key == CWO_OPT_ASM_PAD2X && (value == 0 || value == 1)) {
-        if (value && !(p->lognx + 1 <= MAX_LOGN && p->logny + 1 <= MAX_LOGN)) return CWO_EINVAL;
-        p->asm_pad2x = value;
-        return CWO_OK;
-    }
-    if (key == CWO_OPT_EXPERIMENT && value >= 0 && value <= 7) {
-        p->experiment = value;
-        return CWO_OK;
-    }
-    if (key == CWO_OPT_TIMING && (value == 0 || value == 1)) {
-        p->timing = value;
-        p->ev_used = 0;
-        return CWO_OK;
+    const bool flag = (value == 0 || value == 1);
+    switch (key) {
+        case CWO_OPT_GS_METHOD:
+            if (value != CWO_GS_FRESNEL && value != CWO_GS_ASM) return CWO_EINVAL;
+            p->gs_method = value;
+            return CWO_OK;
+        case CWO_OPT_PIPELINE:
+            if (!flag) return CWO_EINVAL;
+            p->pipeline = value;
+            return CWO_OK;
+        case CWO_OPT_ASM_PAD2X:
+            if (!flag || (value && !fresnel_sizes_ok(p))) return CWO_EINVAL;
+            p->asm_pad2x = value;
+            return CWO_OK;
+        case CWO_OPT_STACK_INTENSITY:
+            if (!flag) return CWO_EINVAL;
+            p->stack_intensity = value;
+            return CWO_OK;
+        case CWO_OPT_ASM_BAND_LIMIT:
+            if (!flag) return CWO_EINVAL;
+            p->band_limit = value;
+            return CWO_OK;
     }
     return CWO_EINVAL;
 }
 
-static bool asm_sizes_ok(cwo_plan_t p) { return p->lognx >= MIN_LOGN && p->logny >= MIN_LOGN; }
-static bool fresnel_sizes_ok(cwo_plan_t p) { return p->lognx + 1 <= MAX_LOGN && p->logny + 1 <= MAX_LOGN; }
-
 enum { STACK_BATCH = 16 };
 
-static size_t prop_ws_bytes(cwo_plan_t p, int method) {
-    const size_t f = sizeof(float2) * (size_t)p->Nx * p->Ny;
-    return method == CWO_GS_ASM ? f : 2 * f;
+static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
+static size_t stack_table_bytes(cwo_plan_t p, int n) {      // per plane: theta_x, theta_y, z/lambda
+    return align256(sizeof(float) * (size_t)n * (size_t)(p->Nx + p->Ny + 1));
 }
 
 extern "C" size_t cwo_plan_workspace_bytes(cwo_plan_t p, int op, int n) {
@@ -198,11 +236,12 @@ extern "C" size_t cwo_plan_workspace_bytes(cwo_plan_t p, int op, int n) {
     switch (op) {
         case CWO_OP_ASM: return p->asm_pad2x ? 2 * f : f;
         case CWO_OP_FRESNEL: return 2 * f;
-        case CWO_OP_STACK: {   // spectrum + the planes in flight: up to 16 planes per batch of launches (minimum 1)
-            const int nb = n < 1 ? 1 : (n > STACK_BATCH ? STACK_BATCH : n);
-            return (size_t)(1 + nb) * f;
+        case CWO_OP_STACK: {   // spectrum + the planes in flight (up to 16 per batch of launches, minimum 1) + tables
+            const int nn = n < 1 ? 1 : n;
+            const int nb = nn > STACK_BATCH ? STACK_BATCH : nn;
+            return (size_t)(1 + nb) * f + stack_table_bytes(p, nn);
         }
-        case CWO_OP_GS: return f + prop_ws_bytes(p, p->gs_method);
+        case CWO_OP_GS: return p->gs_method == CWO_GS_ASM ? 2 * f : 3 * f;
     }
     return 0;
 }
@@ -221,13 +260,22 @@ extern "C" const char* cwo_strerror(int code) {
         case CWO_EWORKSPACE: return "workspace missing or too small";
         case CWO_EUNSUPPORTED: return "device is not compute capability 10.x (B200)";
         case CWO_ECUDA: return "CUDA runtime error (see cwo_last_cuda_error)";
+        case CWO_ENOMEM: return "out of memory while building the plan";
     }
     return "unknown error";
 }
 
 extern "C" int cwo_last_cuda_error(cwo_plan_t p) { return p ? p->last_cuda_error : 0; }
 
-extern "C" int cwo_plan_timings(cwo_plan_t p, float* ms_out, int* tag_out, int cap) {
+// ---- include/cwo_debug.h -------------------------------------------------------------------------------------
+
+extern "C" int cwo_debug_set_timing(cwo_plan_t p, int on) {
+    if (!p || (on != 0 && on != 1)) return CWO_EINVAL;
+    p->timing = on;
+    p->ev_used = 0;
+    return CWO_OK;
+}
+extern "C" int cwo_debug_timings(cwo_plan_t p, float* ms_out, int* tag_out, int cap) {
     if (!p || cap < 0 || (cap > 0 && !ms_out)) return CWO_EINVAL;
     CWO_CUDA(p, cudaStreamSynchronize(p->stream));
     const int n = (int)p->ev_used;
@@ -238,7 +286,12 @@ extern "C" int cwo_plan_timings(cwo_plan_t p, float* ms_out, int* tag_out, int c
     p->ev_used = 0;
     return n;
 }
-extern "C" long long cwo_plan_launch_count(cwo_plan_t p) { return p ? p->launches : 0; }
+extern "C" long long cwo_debug_launch_count(cwo_plan_t p) { return p ? p->launches : 0; }
+extern "C" int cwo_debug_set_fresnel_2d(cwo_plan_t p, int on) {
+    if (!p || (on != 0 && on != 1)) return CWO_EINVAL;
+    p->fresnel_2d = on;
+    return CWO_OK;
+}
 
 // ---- geometry of a propagation ------------------------------------------------------------------
 
@@ -272,34 +325,43 @@ struct PropIO {
     int out_mode; void* out; const float* out_amp;
 };
 
+static int check_call(cwo_plan_t p) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) return CWO_EINVAL;
+    return CWO_OK;
+}
+
 // ---- transfer-function tables (S2) ----------------------------------------------------------------
 
 // ASM: decide between the fp32 split-phase path and the per-sample fp64 path, and fill the Mid fields.
 // Split path requires: no evanescent bin (s_max well below 1) and a small non-paraxial residual for
 // every z of the call (fp32 evaluates it to ~1e-7 relative).
-static bool asm_split_ok(cwo_plan_t p, const Geometry& g, const double* zs, int n) {
+static bool asm_split_ok(cwo_plan_t p, const double* zs, int n) {
     const double fxm = 0.5 / p->px, fym = 0.5 / p->py;          // |f| <= Nyquist
     const double smax = p->lambda * p->lambda * (fxm * fxm + fym * fym);
     if (!(smax <= 0.5)) return false;
     const double r = 1.0 + sqrt(1.0 - smax);
     for (int i = 0; i < n; ++i)
         if (fabs(zs[i]) / p->lambda * smax * smax / (2.0 * r * r) > 32.0) return false;
-    (void)g;
     return true;
 }
 
-static int ensure_asm_tab(cwo_plan_t p, const Geometry& g, int planes) {
-    if (p->asm_tab_planes >= planes) return CWO_OK;
-    if (p->asm_tab) { CWO_CUDA(p, cudaStreamSynchronize(p->stream)); cudaFree(p->asm_tab); p->asm_tab = nullptr; }
-    CWO_CUDA(p, cudaMalloc(&p->asm_tab, sizeof(float) * (size_t)planes * (g.mx + g.my)));
-    p->asm_tab_planes = planes;
-    return CWO_OK;
+// The packed Mid evaluates the residual by its series through s^7 (pipe_kernel.cuh): allowed when the first omitted
+// term, (z/lambda) 429/32768 s^8 (and the geometric tail), stays below 1e-7 cycles at the largest s of the grid.
+static bool asm_poly_ok(cwo_plan_t p, const double* zs, int n) {
+    const double fxm = 0.5 / p->px, fym = 0.5 / p->py;
+    const double smax = p->lambda * p->lambda * (fxm * fxm + fym * fym);
+    if (!(smax < 0.25)) return false;
+    const double tail = 429.0 / 32768.0 * pow(smax, 8) / (1.0 - smax);
+    for (int i = 0; i < n; ++i)
+        if (fabs(zs[i]) / p->lambda * tail > 1e-7) return false;
+    return true;
 }
 
-static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, int n) {
-    int rc = ensure_asm_tab(p, g, n);
-    if (rc != CWO_OK) return rc;
+// tab: n planes x [theta_x (mx) | theta_y (my)]; resc (may be null): z/lambda per plane.  Tiny kernels, no allocation.
+static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, int n, float* tab, float* resc) {
     const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
+    const bool shifted = p->band_limit != 0;
     for (int i0 = 0; i0 < n; i0 += ASM_PLANE_BATCH) {
         AsmPlaneBatch b;
         const int m = n - i0 < ASM_PLANE_BATCH ? n - i0 : ASM_PLANE_BATCH;
@@ -308,52 +370,57 @@ static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, i
             b.p[i].c0 = kz - floor(kz);
             b.p[i].ax = z * p->lambda * dfx * dfx * 0.5;
             b.p[i].ay = z * p->lambda * dfy * dfy * 0.5;
+            b.p[i].kz = kz;
+            b.p[i].ox = shifted ? p->off_x * dfx : 0.0;      // Eq.(19): phase ramp 2 pi (Ox fx + Oy fy), cycles per bin
+            b.p[i].oy = shifted ? p->off_y * dfy : 0.0;
         }
-        CWO_CUDA(p, build_asm_phase_tables(p->asm_tab + (size_t)i0 * (g.mx + g.my), b, m, g.mx, g.my, p->stream));
+        CWO_CUDA(p, build_asm_phase_tables(tab + (size_t)i0 * (g.mx + g.my), resc ? resc + i0 : nullptr, b, m, g.mx, g.my,
+                                           p->stream));
         p->launches++;
     }
     return CWO_OK;
 }
 
-// z/lambda of every plane, for the batched stack kernels (host values copied with the stream's ordering)
-static int ensure_stack_resc(cwo_plan_t p, const double* zs, int n) {
-    if (p->stack_resc_cap < n) {
-        if (p->stack_resc) { CWO_CUDA(p, cudaStreamSynchronize(p->stream)); cudaFree(p->stack_resc); p->stack_resc = nullptr; }
-        CWO_CUDA(p, cudaMalloc(&p->stack_resc, sizeof(float) * (size_t)n));
-        p->stack_resc_cap = n;
+// Band limits of the shifted angular spectrum method, Eq.(18) P:L213-229 (parameters per Ref.[56] of the paper,
+// DESIGN.md reading R15): the phase of H_SA sampled at df must not alias, |O - z f/sqrt(1/lambda^2 - f^2)| <= 1/(2 df)
+// evaluated per axis on the axis itself.  Signed-bin range [lo, hi] of the bins kept (empty when lo > hi).
+static void band_range(double z, double lambda, double off, double df, int m, int* lo_out, int* hi_out) {
+    const double S = 0.5 / df, az = fabs(z);
+    // |z| f / sqrt(1/lambda^2 - f^2) in [o - S, o + S], o = sgn(z) O;  f = t / (lambda sqrt(t^2 + z^2))
+    const double o = z < 0 ? -off : off;
+    const double t0 = o - S, t1 = o + S;
+    int lo = -m / 2, hi = m / 2 - 1;
+    if (az > 0.0) {
+        const double f0 = t0 / (lambda * sqrt(t0 * t0 + az * az)), f1 = t1 / (lambda * sqrt(t1 * t1 + az * az));
+        while (lo <= hi && (double)lo * df < f0) ++lo;
+        while (hi >= lo && (double)hi * df > f1) --hi;
     }
-    std::vector<float> h((size_t)n);
-    for (int i = 0; i < n; ++i) h[(size_t)i] = (float)(zs[i] / p->lambda);
-    // pageable source: the copy is staged before the call returns, and ordered on the plan's stream
-    CWO_CUDA(p, cudaMemcpyAsync(p->stack_resc, h.data(), sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, p->stream));
-    return CWO_OK;
+    *lo_out = lo; *hi_out = hi;
 }
 
-static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, int plane, PassParams& pp) {
+static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, bool poly, const float* tab, PassParams& pp) {
     const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
     pp.n_lane_bins = g.mx;
     if (split) {
-        const float* t = p->asm_tab + (size_t)plane * (g.mx + g.my);
-        pp.tab_lane = (const float2*)t; pp.tab_point = (const float2*)(t + g.mx);
+        pp.tab_lane = (const float2*)tab; pp.tab_point = (const float2*)(tab + g.mx);
         pp.res_a = (float)(p->lambda * p->lambda * dfx * dfx);
         pp.res_b = (float)(p->lambda * p->lambda * dfy * dfy);
         pp.res_c = (float)(z / p->lambda);
+        pp.res_poly = poly ? 1 : 0;
     } else {
         pp.z = z; pp.inv_lam2 = 1.0 / (p->lambda * p->lambda);
         pp.df_lane = dfx; pp.df_point = dfy;
+        pp.off_lane = p->band_limit ? p->off_x : 0.0; pp.off_point = p->band_limit ? p->off_y : 0.0;
+    }
+    pp.band = p->band_limit;
+    if (p->band_limit) {
+        band_range(z, p->lambda, p->off_x, dfx, g.mx, &pp.band_lane_lo, &pp.band_lane_hi);
+        band_range(z, p->lambda, p->off_y, dfy, g.my, &pp.band_point_lo, &pp.band_point_hi);
     }
 }
 
 // Fresnel: Cx, Cy for distance z into table set `set` (coefficient of Eq.(1) and 1/(MxMy) folded in).
 static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int set) {
-    int rc;
-    if ((rc = ensure_twiddles(p, g.logmx, true)) != CWO_OK) return rc;
-    if ((rc = ensure_twiddles(p, g.logmy, true)) != CWO_OK) return rc;
-    for (int s = 0; s < 2; ++s) {
-        if (!p->chirp[s][0]) CWO_CUDA(p, cudaMalloc(&p->chirp[s][0], sizeof(float2) * g.mx));
-        if (!p->chirp[s][1]) CWO_CUDA(p, cudaMalloc(&p->chirp[s][1], sizeof(float2) * g.my));
-    }
-    if (!p->chirp_scratch) CWO_CUDA(p, cudaMalloc(&p->chirp_scratch, sizeof(double2) * 2 * ((size_t)g.mx + g.my)));
     // c = exp(i 2 pi z/lambda)/(i lambda z) * px py / (Mx My), split as cx = c/sqrt|c|, cy = sqrt|c|
     const double kz = z / p->lambda, fr = kz - floor(kz);
     const double cr = cos(2.0 * M_PI * fr), ci = sin(2.0 * M_PI * fr);
@@ -363,10 +430,12 @@ static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int s
     const double c_re = sg * ci * mag, c_im = -sg * cr * mag;
     const double rt = sqrt(mag);
     ChirpAxis ax, ay;
-    ax.out = p->chirp[set][0]; ax.scratch = p->chirp_scratch; ax.tw64 = p->tw64[g.logmx]; ax.logm = g.logmx;
+    ax.out = p->chirp[set][0]; ax.out_pairs = p->chirp_pairs[set][0];
+    ax.scratch = p->chirp_scratch; ax.tw64 = p->tw64[g.logmx]; ax.logm = g.logmx;
     ax.a_cycles = p->px * p->px / (2.0 * p->lambda * z);
     ax.coef = make_double2(c_re / rt, c_im / rt);
-    ay.out = p->chirp[set][1]; ay.scratch = p->chirp_scratch + 2 * (size_t)g.mx; ay.tw64 = p->tw64[g.logmy]; ay.logm = g.logmy;
+    ay.out = p->chirp[set][1]; ay.out_pairs = p->chirp_pairs[set][1];
+    ay.scratch = p->chirp_scratch + 2 * (size_t)g.mx; ay.tw64 = p->tw64[g.logmy]; ay.logm = g.logmy;
     ay.a_cycles = p->py * p->py / (2.0 * p->lambda * z);
     ay.coef = make_double2(rt, 0.0);
     CWO_CUDA(p, build_chirp_spectrum(ax, ay, p->stream));
@@ -384,17 +453,17 @@ typedef CUresult (*encode_tiled_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t
                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static encode_tiled_t get_encode_tiled() {
-    static encode_tiled_t fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    static std::atomic<encode_tiled_t> fn{nullptr};
+    static std::atomic<int> tried{0};
+    if (!tried.load(std::memory_order_acquire)) {
         void* f = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
             q == cudaDriverEntryPointSuccess)
-            fn = (encode_tiled_t)f;
+            fn.store((encode_tiled_t)f, std::memory_order_release);
+        tried.store(1, std::memory_order_release);
     }
-    return fn;
+    return fn.load(std::memory_order_acquire);
 }
 static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int logwc, int w_rows, int planes = 1) {
     encode_tiled_t enc = get_encode_tiled();
@@ -412,11 +481,11 @@ static bool encode_ws_tmap(CUtensorMap* m, const void* ws, int ly, int mx, int l
 static void row_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
     pp.rows = p->Ny; pp.pitch = p->Nx; pp.ly = p->Ny; pp.logwc = g.logwc;
-    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = p->experiment;
+    pp.tw = p->tw[g.logmx]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline;
 }
 static void col_params(cwo_plan_t p, const Geometry& g, PassParams& pp) {
     memset(&pp, 0, sizeof(pp));
-    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline; pp.dbg = p->experiment;
+    pp.ly = p->Ny; pp.tw = p->tw[g.logmy]; pp.out_scale = 1.0f; pp.use_pipe = p->pipeline;
 }
 
 // the inverse pass over 8192-point rows of complex fields runs on one-row tiles (fold_kernel.cuh) when the
@@ -447,14 +516,12 @@ static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const
     return launch(p, g.logmx, ROW_INV, g.pad, MID_NONE, (p->Ny + g.rb - 1) / g.rb, pp);
 }
 
-// One propagation = pass R, pass C (fused), pass R'.  `ws` holds Ny rows x Mx columns in column-tile
-// order.  Fresnel: table set `set` must hold the spectra for this z.  ASM: tables (if split) at plane 0.
-static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, const PropIO& io, float2* ws,
+// One propagation of the two-dimensional form = pass R, pass C (fused), pass R'.  `ws` holds Ny rows x Mx columns
+// in column-tile order.  Fresnel: table set `set` must hold the spectra for this z.  ASM: tables (if split) in asm_tab.
+static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, bool poly, const PropIO& io, float2* ws,
                       bool pad2x = false) {
     const Geometry g = geometry(p, method, pad2x);
     int rc;
-    if ((rc = ensure_twiddles(p, g.logmx, false)) != CWO_OK) return rc;
-    if ((rc = ensure_twiddles(p, g.logmy, false)) != CWO_OK) return rc;
     if ((rc = pass_row_fwd(p, g, io, ws)) != CWO_OK) return rc;
     PassParams pp; col_params(p, g, pp);
     pp.in = ws; pp.out = ws;
@@ -462,12 +529,16 @@ static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, c
     float scale = 1.0f;
     if (method == CWO_GS_ASM) {
         mid = split ? MID_ASM_SPLIT : MID_ASM_F64;
-        fill_asm_mid(p, g, z, split, 0, pp);
+        fill_asm_mid(p, g, z, split, poly, p->asm_tab, pp);
         scale = (float)(1.0 / ((double)g.mx * (double)g.my));       // 1/(MxMy) of the inverse FFT (reading R3)
     } else {
         mid = MID_TABLES; pp.tab_lane = p->chirp[set][0]; pp.tab_point = p->chirp[set][1]; pp.n_lane_bins = g.mx;
     }
-    if ((rc = launch(p, g.logmy, COL_FUSED, g.pad, mid, g.mx / g.wc, pp)) != CWO_OK) return rc;
+    const int n_tiles = g.mx / g.wc;
+    // (a persistent form of this pass with its tables in shared memory was built and measured: 101 vs 88 us at
+    // 4096^2, 549 vs 520 us at 8192^2 -- static tile assignment cannot follow the SM-to-SM spread)
+    rc = launch(p, g.logmy, COL_FUSED, g.pad, mid, n_tiles, pp);
+    if (rc != CWO_OK) return rc;
     return pass_row_inv(p, g, io, ws, scale);
 }
 
@@ -475,62 +546,108 @@ static bool aligned16(const void* q) { return q && !((uintptr_t)q & 15); }
 
 extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || !asm_sizes_ok(p)) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_ASM, 0)) return CWO_EWORKSPACE;
     const bool pad2x = p->asm_pad2x != 0;
     const Geometry g = geometry(p, CWO_GS_ASM, pad2x);
-    const bool split = asm_split_ok(p, g, &z, 1);
+    const bool split = asm_split_ok(p, &z, 1), poly = split && asm_poly_ok(p, &z, 1);
     int rc;
-    if (split && (rc = build_asm_tables(p, g, &z, 1)) != CWO_OK) return rc;
+    if (split && (rc = build_asm_tables(p, g, &z, 1, p->asm_tab, nullptr)) != CWO_OK) return rc;
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
-    return run_passes(p, CWO_GS_ASM, z, 0, split, io, (float2*)p->ws, pad2x);
+    return run_passes(p, CWO_GS_ASM, z, 0, split, poly, io, (float2*)p->ws, pad2x);
+}
+
+// ---- Fresnel diffraction, separable form (lineconv_kernel.cuh) --------------------------------------------------
+
+static bool fresnel_separable(cwo_plan_t p) {
+    return !p->fresnel_2d && p->lognx >= MIN_PAIR_LOGN && p->lognx <= MAX_PAIR_LOGN && p->logny >= MIN_PAIR_LOGN &&
+           p->logny <= MAX_PAIR_LOGN;
+}
+// axis 0: convolve along x (lines = rows of a [Ny][Nx] field); axis 1: along y (lines = rows of the transposed field)
+static int conv_pass(cwo_plan_t p, int axis, int variant, ConvParams& cp) {
+    const int logn = axis == 0 ? p->lognx : p->logny;
+    cp.tw = p->tw[logn]; cp.tw2 = p->tw[logn + 1];
+    cp.n_lines = axis == 0 ? p->Ny : p->Nx;
+    cp.counter = p->tile_counter;
+    return launch_tagged(p, logn * 16 + KIND_CONV, [&] { return kConv[logn](variant, p->stream, cp); });
+}
+static int transpose_c64(cwo_plan_t p, const float2* in, float2* out, int rows, int cols) {
+    return launch_tagged(p, KIND_TRANSPOSE, [&] { return launch_transpose_c64(in, out, rows, cols, p->stream); });
+}
+static int transpose_f32(cwo_plan_t p, const float* in, float* out, int rows, int cols) {
+    return launch_tagged(p, KIND_TRANSPOSE, [&] { return launch_transpose_f32(in, out, rows, cols, p->stream); });
 }
 
 extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_sizes_ok(p)) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL, 0)) return CWO_EWORKSPACE;
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0);
     if (rc != CWO_OK) return rc;
+    if (fresnel_separable(p)) {
+        const size_t f = (size_t)p->Nx * p->Ny;
+        float2* w0 = (float2*)p->ws;
+        float2* w1 = w0 + f;
+        ConvParams cp; memset(&cp, 0, sizeof(cp));
+        cp.in = (const float2*)u1; cp.out = w0; cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][0];
+        if ((rc = conv_pass(p, 0, 0, cp)) != CWO_OK) return rc;                     // rows: u1 -> w0
+        if ((rc = transpose_c64(p, w0, w1, p->Ny, p->Nx)) != CWO_OK) return rc;      // w1 = w0^T  [Nx][Ny]
+        memset(&cp, 0, sizeof(cp));
+        cp.in = w1; cp.out = w1; cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][1];
+        if ((rc = conv_pass(p, 1, 0, cp)) != CWO_OK) return rc;                     // columns, in place
+        return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);                      // u2 = w1^T
+    }
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
-    return run_passes(p, CWO_GS_FRESNEL, z, 0, false, io, (float2*)p->ws);
+    return run_passes(p, CWO_GS_FRESNEL, z, 0, false, false, io, (float2*)p->ws);
 }
 
-extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double* zs, int n, cwo_c64* out) {
+extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double* zs, int n, void* out) {
     if (!p || !aligned16(u1) || !aligned16(out) || !zs || n <= 0 || !asm_sizes_ok(p)) return CWO_EINVAL;
     for (int k = 0; k < n; ++k) if (!isfinite(zs[k])) return CWO_EINVAL;
-    if (!p->ws || p->ws_bytes < 2 * sizeof(float2) * (size_t)p->Nx * p->Ny) return CWO_EWORKSPACE;   // the minimum: one plane in flight
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
     const Geometry g = geometry(p, CWO_GS_ASM);
-    const size_t f = (size_t)p->Nx * p->Ny;
+    const size_t f = (size_t)p->Nx * p->Ny, fb = sizeof(float2) * f, tb = stack_table_bytes(p, n);
+    if (!p->ws || p->ws_bytes < 2 * fb + tb) return CWO_EWORKSPACE;               // the minimum: one plane in flight
+    const int cap = (int)((p->ws_bytes - tb) / fb) - 1;                            // planes in flight
     float2* A = (float2*)p->ws;       // FFT2[u1] in column-tile order, computed once (S9)
-    float2* B = A + f;                // one plane in flight between its column and row pass
+    float2* B = A + f;                // planes between their column and row pass
+    float* tab = (float*)((unsigned char*)p->ws + (size_t)(1 + cap) * fb);        // n x [theta_x | theta_y], then z/lambda
+    float* resc = tab + (size_t)n * (g.mx + g.my);
+    const int tab_stride = g.mx + g.my;
+    const bool intensity = p->stack_intensity != 0;
+    const int out_mode = intensity ? OUT_INTENSITY : OUT_COMPLEX;
+    const size_t out_plane = intensity ? f / 2 : f;                                // in float2 units
     int rc;
-    const bool split = asm_split_ok(p, g, zs, n);
-    if (split && (rc = build_asm_tables(p, g, zs, n)) != CWO_OK) return rc;
-    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, nullptr, nullptr};
+    const bool split = asm_split_ok(p, zs, n), poly = split && asm_poly_ok(p, zs, n);
+    // Batched form (pipelined kernels, split-phase H): one column launch and one row launch cover as many planes
+    // as the workspace holds, so the persistent CTAs fill and drain once per batch instead of once per plane.
+    const bool pipe_len = g.logmx >= 10 && g.logmx <= 12 && g.logmy >= 10 && g.logmy <= 12;
+    bool batched = split && p->pipeline && pipe_len && cap >= 2 && p->Ny % g.rb == 0;
+    if (batched) {                    // the tensor map of a batch must be encodable BEFORE anything is enqueued
+        CUtensorMap probe;
+        batched = encode_ws_tmap(&probe, B, p->Ny, g.mx, g.logwc, g.rb, cap < n ? cap : n);
+    }
+    if (split && (rc = build_asm_tables(p, g, zs, n, tab, resc)) != CWO_OK) return rc;
+    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, out_mode, nullptr, nullptr};
     if ((rc = pass_row_fwd(p, g, io, A)) != CWO_OK) return rc;
     PassParams pp; col_params(p, g, pp);
     pp.in = A; pp.out = A;
     if ((rc = launch(p, g.logmy, COL_FWD, 0, MID_NONE, g.mx / g.wc, pp)) != CWO_OK) return rc;
     const float scale = (float)(1.0 / ((double)g.mx * (double)g.my));
-    // Batched form (pipelined kernels, split-phase H): one column launch and one row launch cover as many planes
-    // as the workspace holds, so the persistent CTAs fill and drain once per batch instead of once per plane.
-    const int cap = (int)(p->ws_bytes / (sizeof(float2) * f)) - 1;
-    const bool pipe_len = g.logmx >= 10 && g.logmx <= 12 && g.logmy >= 10 && g.logmy <= 12;
-    if (split && p->pipeline && pipe_len && cap >= 2 && p->Ny % g.rb == 0) {
-        if ((rc = ensure_stack_resc(p, zs, n)) != CWO_OK) return rc;
-        const int tab_stride = g.mx + g.my;
+    if (batched) {
         for (int k0 = 0; k0 < n;) {
             const int nb = n - k0 < cap ? n - k0 : cap;
             col_params(p, g, pp);
             pp.in = A; pp.out = B;
-            fill_asm_mid(p, g, zs[k0], true, k0, pp);
+            fill_asm_mid(p, g, zs[k0], true, poly, tab + (size_t)k0 * tab_stride, pp);
             pp.n_planes = nb; pp.tiles_per_plane = g.mx / g.wc; pp.in_plane_stride = 0; pp.out_plane_stride = f;
-            pp.tab_plane_stride = tab_stride; pp.plane_resc = p->stack_resc + k0;
+            pp.tab_plane_stride = tab_stride; pp.plane_resc = resc + k0;
             if ((rc = launch(p, g.logmy, COL_MIDINV, 0, MID_ASM_SPLIT, nb * (g.mx / g.wc), pp)) != CWO_OK) return rc;
             PassParams rp; row_params(p, g, rp);
-            rp.in = B; rp.out = (float2*)out + (size_t)k0 * f; rp.out_mode = OUT_COMPLEX; rp.out_scale = scale;
-            rp.n_planes = nb; rp.tiles_per_plane = p->Ny / g.rb; rp.in_plane_stride = f; rp.out_plane_stride = f;
+            rp.in = B; rp.out = (float2*)out + (size_t)k0 * out_plane; rp.out_mode = out_mode; rp.out_scale = scale;
+            rp.n_planes = nb; rp.tiles_per_plane = p->Ny / g.rb; rp.in_plane_stride = f; rp.out_plane_stride = out_plane;
             rp.use_tmap = encode_ws_tmap(&rp.tmap, B, p->Ny, g.mx, g.logwc, g.rb, nb) ? 1 : 0;
-            if (!rp.use_tmap) return CWO_EUNSUPPORTED;
+            if (!rp.use_tmap) return fail_cuda(p, cudaErrorUnknown);    // cannot happen: same shape as the probe
             if ((rc = launch(p, g.logmx, ROW_INV, 0, MID_NONE, nb * (p->Ny / g.rb), rp)) != CWO_OK) return rc;
             k0 += nb;
         }
@@ -539,13 +656,57 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     for (int k = 0; k < n; ++k) {
         col_params(p, g, pp);
         pp.in = A; pp.out = B;
-        fill_asm_mid(p, g, zs[k], split, k, pp);
+        fill_asm_mid(p, g, zs[k], split, poly, tab + (size_t)k * tab_stride, pp);
         if ((rc = launch(p, g.logmy, COL_MIDINV, 0, split ? MID_ASM_SPLIT : MID_ASM_F64, g.mx / g.wc, pp)) != CWO_OK)
             return rc;
-        io.out = (float2*)out + (size_t)k * f;
+        io.out = (float2*)out + (size_t)k * out_plane;
         if ((rc = pass_row_inv(p, g, io, B, scale)) != CWO_OK) return rc;
     }
     return CWO_OK;
+}
+
+// Gerchberg-Saxton with the separable Fresnel propagator.  Propagations P_1 = P(-z), P_2 = P(+z), P_3 = P(-z), ...;
+// P_m convolves x then y for odd m and y then x for even m, so that the last convolution of P_m, the constraint and
+// the first convolution of P_(m+1) act on the same lines and run as ONE pass; the field is transposed between passes.
+static int gs_fresnel_separable(cwo_plan_t p, const float* amp_src, const float* amp_dst, double z, int iters,
+                                float* phase_out) {
+    const size_t f = (size_t)p->Nx * p->Ny;
+    float2* cur = (float2*)p->ws;                 // [Ny][Nx] after x passes, [Nx][Ny] after y passes
+    float2* oth = cur + f;
+    float* amp_src_t = (float*)((float2*)p->ws + 2 * f);   // amp_src transposed, [Nx][Ny]
+    const Geometry geo = geometry(p, CWO_GS_FRESNEL);
+    int rc;
+    if ((rc = build_fresnel_tables(p, geo, -z, 0)) != CWO_OK) return rc;                  // set 0: P(-z)
+    if (iters > 0 && (rc = build_fresnel_tables(p, geo, +z, 1)) != CWO_OK) return rc;     // set 1: P(+z)
+    const ulonglong2* X[2] = {(const ulonglong2*)p->chirp_pairs[0][0], (const ulonglong2*)p->chirp_pairs[1][0]};
+    const ulonglong2* Y[2] = {(const ulonglong2*)p->chirp_pairs[0][1], (const ulonglong2*)p->chirp_pairs[1][1]};
+    if (iters > 0 && (rc = transpose_f32(p, amp_src, amp_src_t, p->Ny, p->Nx)) != CWO_OK) return rc;
+    ConvParams cp;
+    // pass 0: G = amp_dst exp(i phi0) -> x convolution of P_1
+    memset(&cp, 0, sizeof(cp));
+    cp.in_amp = amp_dst; cp.in_phase = phase_out; cp.out = cur; cp.tab[0] = X[0];
+    if ((rc = conv_pass(p, 0, 1, cp)) != CWO_OK) return rc;
+    if ((rc = transpose_c64(p, cur, oth, p->Ny, p->Nx)) != CWO_OK) return rc;
+    { float2* t = cur; cur = oth; oth = t; }
+    for (int m = 1; m <= 2 * iters; ++m) {
+        memset(&cp, 0, sizeof(cp));
+        cp.in = cur; cp.out = cur;
+        if (m & 1) {   // y of P_m (-z), amplitude of the source plane, y of P_(m+1) (+z); lines = columns
+            cp.tab[0] = Y[0]; cp.tab[1] = Y[1]; cp.mid_amp = amp_src_t;
+            if ((rc = conv_pass(p, 1, 2, cp)) != CWO_OK) return rc;
+            if ((rc = transpose_c64(p, cur, oth, p->Nx, p->Ny)) != CWO_OK) return rc;
+        } else {       // x of P_m (+z), amplitude of the destination plane, x of P_(m+1) (-z); lines = rows
+            cp.tab[0] = X[1]; cp.tab[1] = X[0]; cp.mid_amp = amp_dst;
+            if ((rc = conv_pass(p, 0, 2, cp)) != CWO_OK) return rc;
+            if ((rc = transpose_c64(p, cur, oth, p->Ny, p->Nx)) != CWO_OK) return rc;
+        }
+        float2* t = cur; cur = oth; oth = t;
+    }
+    // last pass: y of P_(2 iters + 1) (-z), phase; the result is transposed back into phase_out
+    memset(&cp, 0, sizeof(cp));
+    cp.in = cur; cp.out = oth; cp.tab[0] = Y[0];
+    if ((rc = conv_pass(p, 1, 3, cp)) != CWO_OK) return rc;
+    return transpose_f32(p, (const float*)oth, phase_out, p->Nx, p->Ny);
 }
 
 extern "C" int cwo_gs(cwo_plan_t p, const float* amp_src, const float* amp_dst, double z, int iters,
@@ -554,23 +715,26 @@ extern "C" int cwo_gs(cwo_plan_t p, const float* amp_src, const float* amp_dst, 
         return CWO_EINVAL;
     const int method = p->gs_method;
     if (method == CWO_GS_ASM ? !asm_sizes_ok(p) : (!fresnel_sizes_ok(p) || z == 0.0)) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_GS, 0)) return CWO_EWORKSPACE;
+    if (method == CWO_GS_FRESNEL && fresnel_separable(p)) return gs_fresnel_separable(p, amp_src, amp_dst, z, iters, phase_out);
     const size_t f = (size_t)p->Nx * p->Ny;
     float2* g = (float2*)p->ws;          // the constrained field between propagations (8 B/px)
     float2* ws = g + f;
     const Geometry geo = geometry(p, method);
     int rc;
-    bool split = false;
+    bool split = false, poly = false;
     if (method == CWO_GS_FRESNEL) {      // set 0: P(-z), set 1: P(+z)
         if ((rc = build_fresnel_tables(p, geo, -z, 0)) != CWO_OK) return rc;
         if (iters > 0 && (rc = build_fresnel_tables(p, geo, +z, 1)) != CWO_OK) return rc;
     } else {
-        split = asm_split_ok(p, geo, &z, 1);
+        split = asm_split_ok(p, &z, 1);
+        poly = split && asm_poly_ok(p, &z, 1);
     }
-    // The ASM tables hold one z at a time (plane 0); they are rebuilt before each propagation (tiny kernel).
+    // The ASM tables hold one z at a time; they are rebuilt before each propagation (tiny kernel).
     auto prop = [&](double zz, int set, const PropIO& io) -> int {
-        if (method == CWO_GS_ASM && split) { int r = build_asm_tables(p, geo, &zz, 1); if (r != CWO_OK) return r; }
-        return run_passes(p, method, zz, set, split, io, ws);
+        if (method == CWO_GS_ASM && split) { int r = build_asm_tables(p, geo, &zz, 1, p->asm_tab, nullptr); if (r != CWO_OK) return r; }
+        return run_passes(p, method, zz, set, split, poly, io, ws);
     };
     // steps 1-2: G = amp_dst exp(i phi0); p = phasor(P(-z)[G]); the store already forms amp_src * p
     PropIO io = {IN_AMP_PHASE, nullptr, amp_dst, phase_out,

@@ -4,11 +4,12 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stddef.h>
+#include <atomic>
 
 namespace cwo {
 
 enum InMode { IN_COMPLEX = 0, IN_AMP_PHASE = 1 };
-enum OutMode { OUT_COMPLEX = 0, OUT_PHASOR_AMP = 1, OUT_PHASE = 2 };
+enum OutMode { OUT_COMPLEX = 0, OUT_PHASOR_AMP = 1, OUT_PHASE = 2, OUT_INTENSITY = 3 };
 enum MidMode { MID_NONE = 0, MID_TABLES = 1, MID_ASM_SPLIT = 2, MID_ASM_F64 = 3 };
 
 struct PassParams {
@@ -17,7 +18,7 @@ struct PassParams {
     int use_cluster;          // 1: 16384-point forward row pass on 4-CTA clusters (cluster_kernel.cuh); tmap has 4-row boxes
     int use_fold;             // 1: 8192-point inverse row pass on one-row tiles (fold_kernel.cuh); tmap has one-row boxes
     const float2* in;
-    float2* out;              // OUT_PHASE: float*
+    float2* out;              // OUT_PHASE, OUT_INTENSITY: float*
     const float* in_amp;      // IN_AMP_PHASE: amplitude [rows][pitch]
     const float* in_phase;    //               phase
     const float* out_amp;     // OUT_PHASOR_AMP: amplitude of the next plane
@@ -26,7 +27,8 @@ struct PassParams {
     int pitch;                // row passes: row pitch (elements) of the row-major field and real arrays
     int ly;                   // rows kept in the column-tiled workspace
     int logwc;                // row passes: log2 of the column-tile width of the workspace
-    int n_tiles;              // pipelined passes: total number of tiles (the grid is one CTA per SM)
+    int n_tiles;              // total number of tiles
+    int pf_dist;              // one-CTA-per-tile column passes: L2 prefetch distance in tiles (0: off)
     // batched planes (depth stack, pipelined kernels only): tile t belongs to plane t / tiles_per_plane
     int n_planes;             // 0 or 1: a single plane
     int tiles_per_plane;
@@ -34,7 +36,6 @@ struct PassParams {
     size_t out_plane_stride;  // same for `out`
     int tab_plane_stride;     // MID_ASM_SPLIT: floats between the planes' [theta_x | theta_y] tables
     const float* plane_resc;  // MID_ASM_SPLIT: res_c (= z/lambda) of every plane
-    int dbg;                  // CWO_OPT_EXPERIMENT bit mask (pipelined kernels): 1 no global stores, 4 no global loads
     int use_pipe;             // 1: use the pipelined form where it exists (CWO_OPT_PIPELINE)
     const float2* tw;         // forward twiddles exp(-i 2 pi m/n), m < n
     float out_scale;          // ROW_INV store
@@ -44,9 +45,58 @@ struct PassParams {
     const float2* tab_lane;   // MID_TABLES: Cx[k] (float2);  MID_ASM_SPLIT: theta_x[k] (float, cycles)
     const float2* tab_point;  // MID_TABLES: Cy[l];           MID_ASM_SPLIT: theta_y[l]
     float res_a, res_b, res_c;  // MID_ASM_SPLIT: lambda^2 dfx^2, lambda^2 dfy^2, z/lambda
+    // shifted / band-limited angular spectrum method (Eq.(18)-(19), CWO_OPT_ASM_BAND_LIMIT): bins whose signed index is
+    // outside [lo, hi] are zeroed; the phase ramp of Eq.(19) is in the theta tables (split) or formed from off_* (fp64)
+    int band, band_lane_lo, band_lane_hi, band_point_lo, band_point_hi;
+    double off_lane, off_point;
+    int res_poly;               // MID_ASM_SPLIT: 1 = the degree-7 series of the residual is exact to 1e-7 cycles for every bin
 };
 
 constexpr int MIN_LOGN = 5, MAX_LOGN = 14;
+
+// ---- per-device launch state ------------------------------------------------------------------------------
+// A plan belongs to the device that was current when it was made; launch attributes (opt-in shared memory) and
+// the SM count are per device, so the launchers cache them per device index, not per process.
+struct DeviceInfo { int index, n_sm; };
+constexpr int MAX_DEVICES = 64;
+inline DeviceInfo* device_info() {                     // the current device; nullptr on error
+    static DeviceInfo info[MAX_DEVICES];
+    static std::atomic<int> known[MAX_DEVICES];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEVICES) return nullptr;
+    if (!known[dev].load(std::memory_order_acquire)) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return nullptr;
+        info[dev].index = dev; info[dev].n_sm = n;       // idempotent: a race writes the same values
+        known[dev].store(1, std::memory_order_release);
+    }
+    return &info[dev];
+}
+// "cudaFuncSetAttribute has been called for this kernel on device d" (setting it twice is harmless)
+struct FuncOnce {
+    std::atomic<unsigned long long> mask{0};
+    bool done(int dev) const { return (mask.load(std::memory_order_acquire) >> dev) & 1ull; }
+    void set(int dev) { mask.fetch_or(1ull << dev, std::memory_order_release); }
+};
+
+// ---- separable Fresnel convolution (lineconv_kernel.cuh) ---------------------------------------------------
+struct ConvParams {
+    const float2* in;          // [n_lines][N] complex
+    const float* in_amp;       // variant 1: amplitude and phase, [n_lines][N]
+    const float* in_phase;
+    void* out;                 // [n_lines][N] complex, or float phase (variant 3); may alias `in`
+    const float* mid_amp;      // variant 2: amplitude imposed between the two convolutions, [n_lines][N]
+    const ulonglong2* tab[2];  // spectrum of the sampled chirp for convolution 0 / 1, planar pairs, N entries
+    const float2* tw;          // N-point forward twiddles
+    const float2* tw2;         // 2N-point forward twiddles
+    int n_lines;
+    int n_tiles;
+    int pf_dist;               // one CTA per tile: tiles between a CTA and the one that replaces it on its SM
+    int* counter;              // persistent form: {next tile, CTAs done}, zero between launches (self-resetting)
+};
+// variant: 0 complex -> conv -> complex; 1 amp, phase -> conv -> complex; 2 complex -> conv, GS constraint, conv -> complex;
+//          3 complex -> conv -> phase
+typedef cudaError_t (*conv_launcher_t)(int variant, cudaStream_t s, const ConvParams& p);
 
 // one launcher per transform length, defined in pass_inst.cu compiled with -DCWO_LOGN=<k>
 typedef cudaError_t (*pass_launcher_t)(int kind, int pad, int mid, int n_tiles, cudaStream_t s, const PassParams& p);
@@ -55,19 +105,29 @@ typedef cudaError_t (*pass_launcher_t)(int kind, int pad, int mid, int n_tiles, 
 CWO_DECL_LAUNCH(5) CWO_DECL_LAUNCH(6) CWO_DECL_LAUNCH(7) CWO_DECL_LAUNCH(8) CWO_DECL_LAUNCH(9)
 CWO_DECL_LAUNCH(10) CWO_DECL_LAUNCH(11) CWO_DECL_LAUNCH(12) CWO_DECL_LAUNCH(13) CWO_DECL_LAUNCH(14)
 #undef CWO_DECL_LAUNCH
+// lane-pair lengths 256..8192: separable Fresnel line convolution
+#define CWO_DECL_LAUNCH(k) cudaError_t launch_conv_##k(int variant, cudaStream_t s, const ConvParams& p);
+CWO_DECL_LAUNCH(8) CWO_DECL_LAUNCH(9) CWO_DECL_LAUNCH(10) CWO_DECL_LAUNCH(11) CWO_DECL_LAUNCH(12) CWO_DECL_LAUNCH(13)
+#undef CWO_DECL_LAUNCH
+constexpr int MIN_PAIR_LOGN = 8, MAX_PAIR_LOGN = 13;
 
 // tables.cu
 cudaError_t build_twiddles(float2* tw, int n, cudaStream_t s);                 // exp(-i 2 pi m/n), fp64 -> fp32
 cudaError_t build_twiddles_f64(double2* tw, int n, cudaStream_t s);            // same, kept in fp64, m < n/2
 // Fresnel: spectrum of the sampled 1-D chirp, C[k] = coef * sum_{d=-N}^{N-1} exp(i pi (d pitch)^2/(lambda z)) exp(-i 2 pi dk/M)
 // for two axes in one launch.  scratch: 2*M double2 per axis.
-struct ChirpAxis { float2* out; double2* scratch; const double2* tw64; int logm; double a_cycles; double2 coef; };
+// out: C[k], k < M (2-D path); out_pairs: (re C[2j], re C[2j+1], im C[2j], im C[2j+1]), j < M/2 (separable path).
+struct ChirpAxis { float2* out; float4* out_pairs; double2* scratch; const double2* tw64; int logm; double a_cycles; double2 coef; };
 cudaError_t build_chirp_spectrum(const ChirpAxis& ax0, const ChirpAxis& ax1, cudaStream_t s);
-// ASM split path: theta_x[k] = frac(c0 - ax ks^2), theta_y[l] = frac(-ay ls^2) (cycles, fp64 -> fp32) for
+// ASM split path: theta_x[k] = frac(c0 - ax ks^2 + ox ks), theta_y[l] = frac(-ay ls^2 + oy ls) (cycles, fp64 -> fp32) for
 // n_planes distances at once; plane i uses tab + i*(mx+my): [theta_x (mx) | theta_y (my)].
-struct AsmPlane { double c0, ax, ay; };
+struct AsmPlane { double c0, ax, ay, kz, ox, oy; };        // kz = z/lambda (-> resc[plane]); ox, oy: ramp, cycles per bin
 constexpr int ASM_PLANE_BATCH = 128;                      // planes per launch (passed by value)
 struct AsmPlaneBatch { AsmPlane p[ASM_PLANE_BATCH]; };
-cudaError_t build_asm_phase_tables(float* tab, const AsmPlaneBatch& planes, int n_planes, int mx, int my, cudaStream_t s);
+cudaError_t build_asm_phase_tables(float* tab, float* resc, const AsmPlaneBatch& planes, int n_planes, int mx, int my,
+                                   cudaStream_t s);    // resc (may be null): z/lambda of every plane
+// out[c][r] = in[r][c] (transpose.cu); rows, cols multiples of 32
+cudaError_t launch_transpose_c64(const float2* in, float2* out, int rows, int cols, cudaStream_t s);
+cudaError_t launch_transpose_f32(const float* in, float* out, int rows, int cols, cudaStream_t s);
 
 }  // namespace cwo

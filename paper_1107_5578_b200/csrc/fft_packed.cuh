@@ -31,7 +31,14 @@ __device__ __forceinline__ pk fma2(pk a, pk b, pk c) {
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
     return r;
 }
-__device__ __forceinline__ pk pk_bcast(float c) { return pk_make(c, c); }
+__device__ __forceinline__ pk pk_bcast(float c) { return pk_make(c, c); }   // folds into an .F32 (broadcast) operand
+// sign flip of both halves; ptxas folds it into the operand modifiers of the FFMA2 / FADD2 / FMUL2 that consumes it
+__device__ __forceinline__ pk pk_neg(pk a) {
+    pk r;
+    asm("{\n\t.reg .f32 lo, hi;\n\tmov.b64 {lo, hi}, %1;\n\tneg.f32 lo, lo;\n\tneg.f32 hi, hi;\n\tmov.b64 %0, {lo, hi};\n\t}"
+        : "=l"(r) : "l"(a));
+    return r;
+}
 
 // 16 complex points x 2 slots
 struct PV { pk r[16], i[16]; };
@@ -120,6 +127,13 @@ __device__ __forceinline__ void mul_tw(PV& v, int k, float2 w0, float2 w1) {
     const float2 a = cmul(make_float2(r0, i0), w0), b = cmul(make_float2(r1, i1), w1);
     v.r[k] = pk_make(a.x, b.x); v.i[k] = pk_make(a.y, b.y);
 }
+// element k of both slots times ONE twiddle w: packed multiplies with the scalar broadcast to both halves
+// (SASS: FMUL2/FFMA2 with an .F32 operand -- no move, no second multiply); values as cmul()
+__device__ __forceinline__ void mul_tw1(PV& v, int k, float2 w) {
+    const pk r = v.r[k], i = v.i[k];
+    v.r[k] = fma2(r, pk_bcast(w.x), mul2(i, pk_bcast(-w.y)));
+    v.i[k] = fma2(r, pk_bcast(w.y), mul2(i, pk_bcast(w.x)));
+}
 
 template <int R> __device__ __forceinline__ void unpermute_p(PV& v) {
     constexpr int S = 16 / R;
@@ -147,7 +161,7 @@ __device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const floa
             const int k0 = (us + i * C::Q) & ((1 << lns) - 1);
             powers<R>(tw[k0 << (LOGN - lns - LR)], w);
 #pragma unroll
-            for (int r = 1; r < R; ++r) mul_tw(v, i + r * S, w[r], w[r]);
+            for (int r = 1; r < R; ++r) mul_tw1(v, i + r * S, w[r]);
         }
         if (SY::EARLY_WAR && war && i == 0) sync.war();
         dftRp<R>(v, i);
@@ -214,7 +228,7 @@ template <int LOGN, class SY>
 __device__ __forceinline__ void butterflies16_p(PV& v, int lns, const float2 (&w)[16], const SY& sync, bool war) {
     if (lns > 0) {
 #pragma unroll
-        for (int r = 1; r < 16; ++r) mul_tw(v, r, w[r], w[r]);
+        for (int r = 1; r < 16; ++r) mul_tw1(v, r, w[r]);
     }
     if (SY::EARLY_WAR && war) sync.war();
     dft16p(v);

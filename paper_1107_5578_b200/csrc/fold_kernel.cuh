@@ -142,20 +142,15 @@ __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(con
 template <int LOGC, bool PAD>
 static cudaError_t launch_fold(int n_rows, cudaStream_t s, const PassParams& p) {
     using K = FoldCfg<LOGC>;
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return e;
-        e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-    }
-    static bool configured = false;
-    if (!configured) {
+    DeviceInfo* d = device_info();
+    if (!d) return cudaErrorInvalidDevice;
+    const int n_sm = d->n_sm;
+    static FuncOnce once;
+    if (!once.done(d->index)) {
         cudaError_t e = cudaFuncSetAttribute(fold_row_kernel<LOGC, PAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)K::SMEM);
         if (e != cudaSuccess) return e;
-        configured = true;
+        once.set(d->index);
     }
     PassParams q = p;
     q.n_tiles = n_rows;

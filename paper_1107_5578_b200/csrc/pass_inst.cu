@@ -3,6 +3,7 @@
 #include "fold_kernel.cuh"
 #include "cluster_kernel.cuh"
 #include "prefetch_kernel.cuh"
+#include "lineconv_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"
@@ -15,4 +16,9 @@ cudaError_t CWO_CAT(launch_pass_, CWO_LOGN)(int kind, int pad, int mid, int n_ti
                                             const PassParams& p) {
     return launch_pass_impl<CWO_LOGN>(kind, pad, mid, n_tiles, s, p);
 }
+#if CWO_LOGN >= 8 && CWO_LOGN <= 13
+cudaError_t CWO_CAT(launch_conv_, CWO_LOGN)(int variant, cudaStream_t s, const ConvParams& p) {
+    return launch_lineconv_impl<CWO_LOGN>(variant, s, p);
+}
+#endif
 }  // namespace cwo

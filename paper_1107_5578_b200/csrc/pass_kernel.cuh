@@ -112,6 +112,12 @@ template <int LOGN> struct MidAsmSplit {
                 float sn, cs;
                 __sincosf(6.283185307179586f * ph, &sn, &cs);
                 v[s][e] = cconj(cmul(v[s][e], make_float2(cs, sn)));
+                if (P.band) {                              // Eq.(18): the two Rect band limits
+                    const int lane = lane0 + (C::PAIR ? s : 0);
+                    const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+                    if (ks < P.band_lane_lo || ks > P.band_lane_hi || ls < P.band_point_lo || ls > P.band_point_hi)
+                        v[s][e] = make_float2(0.f, 0.f);
+                }
             }
         }
     }
@@ -136,8 +142,10 @@ template <int LOGN> struct MidAsmF64 {
             const double fx = (double)ks * P.df_lane, fy = (double)ls * P.df_point;
             const double w = __dsub_rn(P.inv_lam2, __dadd_rn(__dmul_rn(fx, fx), __dmul_rn(fy, fy)));
             float2 m = make_float2(0.f, 0.f);
-            if (w >= 0.0) {
-                double c = P.z * sqrt(w);
+            const bool cut = P.band && (ks < P.band_lane_lo || ks > P.band_lane_hi || ls < P.band_point_lo ||
+                                        ls > P.band_point_hi);
+            if (w >= 0.0 && !cut) {
+                double c = P.z * sqrt(w) + (P.off_lane * fx + P.off_point * fy);
                 c -= rint(c);
                 float sn, cs;
                 sincospif(2.0f * (float)c, &sn, &cs);
@@ -191,6 +199,10 @@ pass_kernel(const __grid_constant__ PassParams P) {
         // workspace stores the pair planar, which is the register format
         const ulonglong2* src = reinterpret_cast<const ulonglong2*>(P.in + (size_t)tile * P.ly * W);
         ulonglong2* dst = reinterpret_cast<ulonglong2*>(P.out + (size_t)tile * P.ly * W);
+        // the tile of the CTA that will take this one's place on the SM: have L2 fetch it now, so that its loads
+        // (nothing overlaps them: the whole tile goes to registers before the first butterfly) find it on chip
+        if (threadIdx.x == 0 && P.pf_dist > 0 && tile + P.pf_dist < P.n_tiles)
+            l2_prefetch(P.in + (size_t)(tile + P.pf_dist) * P.ly * W, (uint32_t)(P.ly * W * 8));
         PV pv;
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
@@ -374,6 +386,18 @@ pass_kernel(const __grid_constant__ PassParams P) {
                     P.out[base + e * Q] = make_float2(am[e] * ph.x, am[e] * ph.y);
                 }
             }
+        } else if constexpr (IOM == OUT_INTENSITY) {
+            // Eq.(20): I = |u|^2, one float per sample
+            const float sc2 = P.out_scale * P.out_scale;
+            float* outf = reinterpret_cast<float*>(P.out);
+#pragma unroll
+            for (int s = 0; s < 2; ++s) {
+                const int row = lane0 + (C::PAIR ? s : 0);
+                if (row >= P.rows) continue;
+                const size_t base = (size_t)row * P.pitch + u[s];
+#pragma unroll
+                for (int e = 0; e < NE; ++e) outf[base + e * Q] = (v[s][e].x * v[s][e].x + v[s][e].y * v[s][e].y) * sc2;
+            }
         } else {
             // OUT_PHASE, Eq.(25) P:L482 as atan2, by a rolled loop over the thread's samples staged through its own
             // slots of the tile buffer (atan2f would otherwise be unrolled 32 times).
@@ -419,12 +443,14 @@ pass_kernel(const __grid_constant__ PassParams P) {
 template <int LOGN, int KIND, bool PAD, int MID, int IOM, bool X>
 static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
     constexpr size_t smem = ((X && KIND == ROW_FWD) ? Tile<LOGN>::SMEM_BYTES_X : Tile<LOGN>::SMEM_BYTES) + 64;   // + two mbarriers
-    static bool configured = false;
-    if (!configured) {
+    DeviceInfo* d = device_info();
+    if (!d) return cudaErrorInvalidDevice;
+    static FuncOnce once;
+    if (!once.done(d->index)) {
         cudaError_t e = cudaFuncSetAttribute(pass_kernel<LOGN, KIND, PAD, MID, IOM, X>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        once.set(d->index);
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)n_tiles); cfg.blockDim = dim3((unsigned)Tile<LOGN>::T);
@@ -435,7 +461,10 @@ static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
     // long ones (4096^2: 208.7 -> 221.9 us)
     at[0].val.programmaticStreamSerializationAllowed = n_tiles <= 1024 ? 1 : 0;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, pass_kernel<LOGN, KIND, PAD, MID, IOM, X>, p);
+    PassParams q = p;
+    q.n_tiles = n_tiles;
+    q.pf_dist = (!(KIND == ROW_FWD || KIND == ROW_INV) && p.n_planes <= 1) ? d->n_sm * Tile<LOGN>::MINB : 0;
+    return cudaLaunchKernelEx(&cfg, pass_kernel<LOGN, KIND, PAD, MID, IOM, X>, q);
 }
 
 // pipe_kernel.cuh: persistent, prefetching form of the same pass for the HBM-sized tile shapes
@@ -475,7 +504,8 @@ static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) 
 #define CWO_PIPE_FUSED 0
 #endif
     if constexpr (pipe_supported(LOGN) && MID != MID_ASM_F64 && (CWO_PIPE_FUSED || KIND != COL_FUSED) &&
-                  (!ROWPASS || (KIND == ROW_FWD && IOM == IN_COMPLEX) || (KIND == ROW_INV && IOM == OUT_COMPLEX))) {
+                  (!ROWPASS || (KIND == ROW_FWD && IOM == IN_COMPLEX) ||
+                   (KIND == ROW_INV && (IOM == OUT_COMPLEX || IOM == OUT_INTENSITY)))) {
         if (p.use_pipe && (!ROWPASS || (p.use_tmap && p.rows % Tile<LOGN>::W == 0)))
             return launch_pipe<LOGN, KIND, PAD, MID, IOM>(n_tiles, s, p);
     }
@@ -493,6 +523,7 @@ static cudaError_t launch_iom(int iom, int n_tiles, cudaStream_t s, const PassPa
     } else if constexpr (KIND == ROW_INV) {
         return iom == OUT_COMPLEX      ? launch_one<LOGN, KIND, PAD, MID, OUT_COMPLEX>(n_tiles, s, p)
                : iom == OUT_PHASOR_AMP ? launch_one<LOGN, KIND, PAD, MID, OUT_PHASOR_AMP>(n_tiles, s, p)
+               : iom == OUT_INTENSITY  ? launch_one<LOGN, KIND, PAD, MID, OUT_INTENSITY>(n_tiles, s, p)
                                        : launch_one<LOGN, KIND, PAD, MID, OUT_PHASE>(n_tiles, s, p);
     } else {
         return launch_one<LOGN, KIND, PAD, MID, 0>(n_tiles, s, p);

@@ -89,8 +89,68 @@ template <int LOGN> struct PipeMidAsmSplit {
         const float2 t = __ldg(reinterpret_cast<const float2*>(&thl[lane0]));     // lane0 is even
         thx[0] = t.x; thx[1] = t.y;
     }
-    // both slots in packed form (fft_packed.cuh): the phase is per sample, so this part stays scalar
+    // Both slots in packed form (fft_packed.cuh).  z sqrt(1/lambda^2 - f^2) = (z/lambda)(1 - s/2 - g(s)),
+    // g(s) = s^2/8 + s^3/16 + 5 s^4/128 + 7 s^5/256 + 21 s^6/1024 + 33 s^7/2048 + ...: when the plan has verified that
+    // the truncated series is exact to 1e-7 cycles for every bin (P.res_poly) the residual is that polynomial in
+    // packed arithmetic (the two slots differ in s only; theta_y, s_y broadcast), reduced mod 1 BEFORE it meets the
+    // table phases (so the sum keeps 6e-8-cycle resolution), and the only scalar work left is the sine and cosine;
+    // otherwise the closed form with rsqrt / division per sample.
+    // Eq.(18): the two Rect band limits (CWO_OPT_ASM_BAND_LIMIT); uniform branch, off by default
+    __device__ __forceinline__ void band_mask(PV& v) const {
+        const int n = P.n_lane_bins;
+        const int k0 = (lane0 < n / 2) ? lane0 : lane0 - n, k1 = (lane0 + 1 < n / 2) ? lane0 + 1 : lane0 + 1 - n;
+        const bool c0 = k0 < P.band_lane_lo || k0 > P.band_lane_hi, c1 = k1 < P.band_lane_lo || k1 > P.band_lane_hi;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int l = us + e * C::Q;
+            const int ls = (l < C::N / 2) ? l : l - C::N;
+            const bool cp = ls < P.band_point_lo || ls > P.band_point_hi;
+            float r0, r1, i0, i1;
+            pk_split(v.r[e], r0, r1); pk_split(v.i[e], i0, i1);
+            if (cp || c0) { r0 = 0.f; i0 = 0.f; }
+            if (cp || c1) { r1 = 0.f; i1 = 0.f; }
+            v.r[e] = pk_make(r0, r1); v.i[e] = pk_make(i0, i1);
+        }
+    }
     __device__ __forceinline__ void packed(PV& v) const {
+        if (P.res_poly) packed_poly(v); else packed_closed(v);
+        if (P.band) band_mask(v);
+    }
+    __device__ __forceinline__ void packed_poly(PV& v) const {
+        float sx[2];
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            const int lane = lane0 + s;
+            const int ks = (lane < P.n_lane_bins / 2) ? lane : lane - P.n_lane_bins;
+            sx[s] = P.res_a * (float)ks * (float)ks;
+        }
+        const pk sx2 = pk_make(sx[0], sx[1]), thx2 = pk_make(thx[0], thx[1]);
+        const float usf = (float)us;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int l = us + e * C::Q;
+            const float lsf = usf + (float)(e < 8 ? e * C::Q : (e - 16) * C::Q);   // signed bin of l (us < Q), exact
+            const float sy = P.res_b * lsf * lsf;
+            const pk sv = add2(sx2, pk_bcast(sy));
+            pk h = fma2(sv, pk_bcast(33.0f / 2048.0f), pk_bcast(21.0f / 1024.0f));
+            h = fma2(sv, h, pk_bcast(7.0f / 256.0f));
+            h = fma2(sv, h, pk_bcast(5.0f / 128.0f));
+            h = fma2(sv, h, pk_bcast(1.0f / 16.0f));
+            h = fma2(sv, h, pk_bcast(0.125f));
+            pk res = mul2(mul2(mul2(sv, sv), pk_bcast(res_c)), h);
+            const pk big = pk_bcast(12582912.0f);                  // 1.5 * 2^23: (x + big) - big = rint(x), |x| < 2^22
+            res = sub2(res, sub2(add2(res, big), big));
+            const pk ph = mul2(sub2(add2(thx2, pk_bcast(thy[l])), res), pk_bcast(6.283185307179586f));
+            float p0, p1, sn0, cs0, sn1, cs1;
+            pk_split(ph, p0, p1);
+            __sincosf(p0, &sn0, &cs0); __sincosf(p1, &sn1, &cs1);
+            // conj(x (cs + i sn)) = (xr cs - xi sn) - i (xr sn + xi cs)
+            const pk cs2 = pk_make(cs0, cs1), sn2 = pk_make(sn0, sn1), xr = v.r[e], xi = v.i[e];
+            v.r[e] = fma2(xr, cs2, pk_neg(mul2(xi, sn2)));
+            v.i[e] = fma2(pk_neg(xr), sn2, pk_neg(mul2(xi, cs2)));
+        }
+    }
+    __device__ __forceinline__ void packed_closed(PV& v) const {
         float sx[2];
 #pragma unroll
         for (int s = 0; s < 2; ++s) {
@@ -177,7 +237,6 @@ pipe_kernel(const __grid_constant__ PassParams P) {
     uint64_t* staged = full + K::NBUF;                                        // results written back to buffer b
 
     const int nt = (P.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // tiles of this CTA
-    const bool no_st = P.dbg & 1, no_ld = P.dbg & 4;
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -209,7 +268,6 @@ pipe_kernel(const __grid_constant__ PassParams P) {
         const int wc = 1 << P.logwc;
         const int groups = N >> P.logwc, bg = groups < 256 ? groups : 256;    // column groups per TMA box
         auto load = [&](int j) {
-            if (no_ld) return;
             const int b = j % K::NBUF;
             const int gt = blockIdx.x + j * gridDim.x;
             const int plane = batched ? gt / P.tiles_per_plane : 0;
@@ -234,7 +292,6 @@ pipe_kernel(const __grid_constant__ PassParams P) {
             }
         };
         auto store = [&](int j) {
-            if (no_st) return;
             const int b = j % K::NBUF;
             const int gt = blockIdx.x + j * gridDim.x;
             const int plane = batched ? gt / P.tiles_per_plane : 0;
@@ -244,6 +301,11 @@ pipe_kernel(const __grid_constant__ PassParams P) {
             if constexpr (KIND == ROW_FWD) {
                 for (int c = 0; c < groups; c += bg)
                     tma_store_2d(&P.tmap, src + (size_t)c * W * wc * 8, tile * W * wc * 2, plane * groups + c);
+            } else if constexpr (KIND == ROW_INV && IOM == OUT_INTENSITY) {   // W rows of floats, NP points each
+                float* outf = reinterpret_cast<float*>(out);
+#pragma unroll
+                for (int r = 0; r < W; ++r)
+                    bulk_s2g(outf + (size_t)(tile * W + r) * P.pitch, src + (size_t)r * RS * 8, NP * 4);
             } else if constexpr (KIND == ROW_INV) {        // W rows of the row-major field, NP points each
 #pragma unroll
                 for (int r = 0; r < W; ++r)
@@ -285,7 +347,7 @@ pipe_kernel(const __grid_constant__ PassParams P) {
         const int plane = batched ? gt / P.tiles_per_plane : 0;
         const int tile = gt - plane * P.tiles_per_plane;
         float2* sm = reinterpret_cast<float2*>(smraw + b * K::BUF);
-        if (!no_ld) mbar_wait(&full[b], (j / K::NBUF) & 1);
+        mbar_wait(&full[b], (j / K::NBUF) & 1);
 
         if constexpr (COLPASS) {
             // ---- column passes: packed arithmetic, both slots in lockstep (fft_packed.cuh) ----------------
@@ -397,13 +459,22 @@ pipe_kernel(const __grid_constant__ PassParams P) {
             for (int e = 0; e < 16; ++e)
                 *reinterpret_cast<float4*>(d + e * Q * W) = make_float4(v[0][e].x, v[1][e].x, v[0][e].y, v[1][e].y);
         } else if constexpr (KIND == ROW_INV) {
-            static_assert(IOM == OUT_COMPLEX, "GS store modes run in pass_kernel");
+            static_assert(IOM == OUT_COMPLEX || IOM == OUT_INTENSITY, "GS store modes run in pass_kernel");
             const float sc = P.out_scale;                     // conj completes the inverse transform
+            if constexpr (IOM == OUT_INTENSITY) {             // Eq.(20): |u|^2 as floats, same row stride (bytes) of the staging
+                float* smf = reinterpret_cast<float*>(sm);
 #pragma unroll
-            for (int s = 0; s < 2; ++s)
+                for (int s = 0; s < 2; ++s)
 #pragma unroll
-                for (int e = 0; e < NE; ++e)
-                    sm[(w0 + s) * RS + us + e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
+                    for (int e = 0; e < NE; ++e)
+                        smf[(w0 + s) * RS * 2 + us + e * Q] = (v[s][e].x * v[s][e].x + v[s][e].y * v[s][e].y) * (sc * sc);
+            } else {
+#pragma unroll
+                for (int s = 0; s < 2; ++s)
+#pragma unroll
+                    for (int e = 0; e < NE; ++e)
+                        sm[(w0 + s) * RS + us + e * Q] = make_float2(v[s][e].x * sc, -v[s][e].y * sc);
+            }
         }
         fence_proxy_async();
         mbar_arrive(&staged[b]);
@@ -414,20 +485,15 @@ template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p) {
     using K = PipeCfg<LOGN, KIND>;
     constexpr size_t SM = (MID == MID_ASM_SPLIT) ? K::SMEM_TAB : K::SMEM_NOTAB;
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return e;
-        e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-    }
-    static bool configured = false;
-    if (!configured) {
+    DeviceInfo* d = device_info();
+    if (!d) return cudaErrorInvalidDevice;
+    const int n_sm = d->n_sm;
+    static FuncOnce once;
+    if (!once.done(d->index)) {
         cudaError_t e = cudaFuncSetAttribute(pipe_kernel<LOGN, KIND, PAD, MID, IOM>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM);
         if (e != cudaSuccess) return e;
-        configured = true;
+        once.set(d->index);
     }
     PassParams q = p;
     q.n_tiles = n_tiles;

@@ -95,15 +95,14 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, 1) colpref_kernel(const __grid_
 template <int LOGN, int MID>
 static cudaError_t launch_colpref(int n_tiles, cudaStream_t s, const PassParams& p) {
     constexpr size_t smem = Tile<LOGN>::SMEM_BYTES + 64 + PREFETCH_BYTES;
-    static int n_sm = 0;
-    if (!n_sm) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
+    DeviceInfo* d = device_info();
+    if (!d) return cudaErrorInvalidDevice;
+    const int n_sm = d->n_sm;
+    static FuncOnce once;
+    if (!once.done(d->index)) {
+        cudaError_t e = cudaFuncSetAttribute(colpref_kernel<LOGN, MID>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(colpref_kernel<LOGN, MID>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        once.set(d->index);
     }
     PassParams q = p;
     q.n_tiles = n_tiles;

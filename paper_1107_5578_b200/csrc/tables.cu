@@ -68,7 +68,11 @@ __global__ void __launch_bounds__(1024) chirp_fft_kernel(ChirpAxis ax0, ChirpAxi
     }
     for (int i = threadIdx.x; i < M; i += blockDim.x) {
         double2 r = zmul(a[i], ax.coef);
-        ax.out[i] = make_float2((float)r.x, (float)r.y);
+        if (ax.out) ax.out[i] = make_float2((float)r.x, (float)r.y);
+        if (ax.out_pairs) {                                  // planar pairs (even bin, odd bin): lineconv_kernel.cuh
+            float* q = reinterpret_cast<float*>(ax.out_pairs + (i >> 1)) + (i & 1);
+            q[0] = (float)r.x; q[2] = (float)r.y;
+        }
     }
 }
 
@@ -79,14 +83,15 @@ cudaError_t build_chirp_spectrum(const ChirpAxis& ax0, const ChirpAxis& ax1, cud
 
 // ASM split path (S2): per plane, theta_x[k] = frac(c0 - ax ks^2), theta_y[l] = frac(-ay ls^2) in cycles.
 // ax ks^2 reaches ~5e3 cycles (c3, z = 0.5 m): formed in fp64, reduced mod 1, then rounded to fp32.
-__global__ void asm_phase_kernel(float* tab, const __grid_constant__ AsmPlaneBatch planes, int mx, int my) {
+__global__ void asm_phase_kernel(float* tab, float* resc, const __grid_constant__ AsmPlaneBatch planes, int mx, int my) {
     const AsmPlane pl = planes.p[blockIdx.y];
+    if (resc && blockIdx.x == 0 && threadIdx.x == 0) resc[blockIdx.y] = (float)pl.kz;
     float* t = tab + (size_t)blockIdx.y * (mx + my);
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < mx + my; i += gridDim.x * blockDim.x) {
         const bool isx = i < mx;
         const int j = isx ? i : i - mx, m = isx ? mx : my;
         const double b = (double)((j < m / 2) ? j : j - m);
-        double c = (isx ? pl.c0 : 0.0) - (isx ? pl.ax : pl.ay) * b * b;
+        double c = (isx ? pl.c0 : 0.0) - (isx ? pl.ax : pl.ay) * b * b + (isx ? pl.ox : pl.oy) * b;
         c -= rint(c);
         t[i] = (float)c;
     }
@@ -96,7 +101,8 @@ __global__ void asm_phase_kernel(float* tab, const __grid_constant__ AsmPlaneBat
     asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
-cudaError_t build_asm_phase_tables(float* tab, const AsmPlaneBatch& planes, int n_planes, int mx, int my, cudaStream_t s) {
+cudaError_t build_asm_phase_tables(float* tab, float* resc, const AsmPlaneBatch& planes, int n_planes, int mx, int my,
+                                   cudaStream_t s) {
     dim3 grid((mx + my + 255) / 256 > 64 ? 64 : (mx + my + 255) / 256, n_planes);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = s;
@@ -104,7 +110,7 @@ cudaError_t build_asm_phase_tables(float* tab, const AsmPlaneBatch& planes, int 
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, asm_phase_kernel, tab, planes, mx, my);
+    return cudaLaunchKernelEx(&cfg, asm_phase_kernel, tab, resc, planes, mx, my);
 }
 
 }  // namespace cwo

@@ -110,6 +110,18 @@ def gs_inputs_c5(cfg: Config):
     return amp_src, amp_dst.astype(np.float32), phi0
 
 
+def gs_inputs(shape, seed: int):
+    """gs_inputs_c5's recipe on an arbitrary (Ny, Nx) grid (non-square parity cases): amp_src == 1, amp_dst = 9x9
+    periodic box blur of U[0,1) noise scaled to the same energy, phi0 ~ U[0,2pi).  float32 arrays."""
+    r = np.random.Generator(np.random.PCG64(SEED_BASE + 5 + 1000 * int(seed)))
+    ny, nx = shape
+    amp_src = np.ones((ny, nx), np.float32)
+    amp_dst = _box_blur_periodic(r.random((ny, nx)), 9)
+    amp_dst *= np.sqrt(float(ny) * nx / np.sum(amp_dst * amp_dst))
+    phi0 = (r.random((ny, nx)) * (2 * np.pi)).astype(np.float32)
+    return amp_src, amp_dst.astype(np.float32), phi0
+
+
 def random_phasor(cfg: Config, stream: int = 1) -> np.ndarray:
     """Unit-modulus complex64 field with uniform phase (restart states for GS parity)."""
     r = rng_for(cfg, stream)

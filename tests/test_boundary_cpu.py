@@ -14,8 +14,8 @@ def libpath():
     return build.build()
 
 
-def _declared():
-    src = open(os.path.join(ROOT, "include", "cwo.h")).read()
+def _declared(header="cwo.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(cwo_[a-z0-9_]+)\s*\(", src)))
 
@@ -29,13 +29,21 @@ def test_header_declares_the_calls_of_the_scope_table():
 
 def test_library_exports_every_declared_symbol(libpath):
     L = ctypes.CDLL(libpath)
-    for name in _declared():
+    for name in _declared() + _declared("cwo_debug.h"):
         assert hasattr(L, name), name
+
+
+def test_product_header_has_no_measurement_hooks():
+    names = _declared()
+    assert not [n for n in names if "debug" in n or "timing" in n or "launch_count" in n]
+    src = open(os.path.join(ROOT, "include", "cwo.h")).read()
+    assert "EXPERIMENT" not in src and "CWO_OPT_TIMING" not in src
 
 
 def test_binding_lists_the_same_names(libpath):
     from paper_1107_5578_b200 import api
     assert sorted(api.EXPORTS) == _declared()
+    assert sorted(api.DEBUG_EXPORTS) == _declared("cwo_debug.h")
     for name in ("cwo_plan", "cwo_asm", "cwo_fresnel_conv", "cwo_propagate_stack", "cwo_gs"):
         assert callable(getattr(api, name))
 

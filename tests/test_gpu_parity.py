@@ -147,6 +147,17 @@ def test_fresnel_non_square_and_unequal_pitch(api, oracle, shape):
     _assert_parity(_gpu_fresnel(api, u1, px, py, lam, z), oracle.fresnel_conv(u1, px, py, lam, z), "fresnel %s" % (shape,))
 
 
+@pytest.mark.parametrize("shape", [(8192, 32), (32, 8192), (8192, 64), (64, 8192), (4096, 64), (64, 4096), (8192, 256)])
+def test_fresnel_long_transforms_full_field(api, oracle, shape):
+    """The 8192- and 16384-point transforms of c5 / Fresnel 8192^2, compared element by element: one axis at full
+    length, the other short enough for the fp64 oracle (rows and columns both ways), at c5's pitch and wavelength."""
+    cfg = W.CONFIGS["c5"]
+    u1 = _rand(shape, 41 + shape[0] % 7)
+    for z in (cfg.zs[0], -cfg.zs[0]):
+        _assert_parity(_gpu_fresnel(api, u1, cfg.pitch, cfg.pitch, cfg.lam, z),
+                       oracle.fresnel_conv(u1, cfg.pitch, cfg.pitch, cfg.lam, z), "fresnel %s z=%g" % (shape, z))
+
+
 def test_fresnel_c2_full_and_inplace(api, oracle):
     cfg = W.CONFIGS["c2"]
     u1 = W.make_field(cfg)
@@ -171,17 +182,28 @@ def test_fresnel_2048_and_4096(api, oracle):
 
 
 def test_fresnel_c5_size_sampled(api, oracle):
-    # 8192^2 -> virtual 16384^2: spot-check against the direct sum (the oracle's plain definition)
+    # 8192^2 -> virtual 16384^2 in the launch configuration bench.py --workload c5 / fresnel8192 times: 256 outputs
+    # against the direct sum of Eq.(1) (the oracle's plain definition), covering every row and column phase mod 8,
+    # both crop edges and the corners; rel-L2 and max-abs gates as everywhere
     cfg = W.CONFIGS["c5"]
     n = cfg.N
     r = np.random.default_rng(2)
     u1 = W.random_phasor(cfg)
     got = _gpu_fresnel(api, u1, cfg.pitch, cfg.pitch, cfg.lam, -cfg.zs[0])
-    ms = np.concatenate([[0, n - 1, 0, n - 1], r.integers(0, n, 8)])
-    ns = np.concatenate([[0, n - 1, n - 1, 0], r.integers(0, n, 8)])
+    edge = np.array([0, 1, 2, 3, n - 4, n - 3, n - 2, n - 1])
+    ms = np.concatenate([[0, n - 1, 0, n - 1], edge, r.integers(0, n, 8), r.integers(0, n, 236)])
+    ns = np.concatenate([[0, n - 1, n - 1, 0], r.integers(0, n, 8), edge, r.integers(0, n, 236)])
+    ms[20:84] = (ms[20:84] // 8) * 8 + np.arange(64) % 8          # every x mod 8 ...
+    ns[20:84] = (ns[20:84] // 8) * 8 + np.arange(64) // 8         # ... with every y mod 8
+    assert ms.size == 256
+    oracle.set_threads(oracle.max_threads())          # 256 direct sums over 8192^2 terms
     ref = oracle.fresnel_points(u1, cfg.pitch, cfg.pitch, cfg.lam, -cfg.zs[0], ms, ns)
+    oracle.set_threads(min(8, oracle.max_threads()))
     err = np.abs(got[ns, ms] - ref)
-    assert np.linalg.norm(err) / np.linalg.norm(ref) <= REL_L2, (err, np.abs(ref))
+    # the peak of |u2| is not known from samples: every |u1| is 1 and the operator is ~unitary, so the sample
+    # maximum is a lower bound of the peak (a stricter gate than the definition's)
+    assert np.linalg.norm(err) / np.linalg.norm(ref) <= REL_L2, (err.max(), np.abs(ref).max())
+    assert err.max() <= MAX_ABS * np.abs(ref).max(), (err.max(), np.abs(ref).max())
 
 
 # ---------------------------------------------------------------- stack ---------------------------------------
@@ -206,7 +228,8 @@ def test_stack_c4_full_size_sampled_planes(api, oracle):
     out = torch.empty((len(cfg.zs), cfg.N, cfg.N), dtype=torch.complex64, device="cuda")
     api.cwo_propagate_stack(plan, _dev(u1), cfg.zs, out)
     torch.cuda.synchronize()
-    for k in (0, 17, 63):
+    # every plane of the second 16-plane batch of launches (positions 0..15), and the first / last plane of the call
+    for k in [0] + list(range(16, 32)) + [63]:
         _assert_parity(out[k].cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[k]), "c4 plane %d" % k)
     # every plane carries the input's energy (unitary H, no evanescent bins)
     e = torch.linalg.vector_norm(out.reshape(len(cfg.zs), -1), dim=1).cpu().numpy()
@@ -216,8 +239,8 @@ def test_stack_c4_full_size_sampled_planes(api, oracle):
 # ---------------------------------------------------------------- GS ------------------------------------------
 
 def _gs_gpu(api, method, amp_src, amp_dst, phi, pitch, lam, z, iters):
-    n = amp_src.shape[0]
-    plan = api.cwo_plan(n, n, pitch, lam)
+    ny, nx = amp_src.shape
+    plan = api.cwo_plan(nx, ny, pitch, lam)
     plan.set_option(api.CWO_OPT_GS_METHOD, method)
     ph = _dev(phi.astype(np.float32))
     api.cwo_gs(plan, _dev(amp_src), _dev(amp_dst), z, iters, ph)
@@ -242,14 +265,57 @@ def test_gs_kinoform_and_restart_parity(api, oracle, method, n):
     assert th.min() >= -np.pi - 1e-6 and th.max() <= np.pi + 1e-6
     # restart parity along the oracle's trajectory: from the image-plane phase of
     # iteration t, one init + one loop pass on both sides
-    for t in range(6):
+    for t in range(20):
         p, G = oracle.gs_iter(method, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z, want_G=True)
-        if t in (0, 1, 5):
+        if t in (0, 1, 5, 10, 19):
             phi_t = np.angle(G).astype(np.float32)
             th = _gs_gpu(api, method, amp_src, amp_dst, phi_t, cfg.pitch, cfg.lam, z, 1)
             pr = oracle.gs_init(method, amp_dst, phi_t, cfg.pitch, cfg.pitch, cfg.lam, z)
             pr = oracle.gs_iter(method, amp_src, amp_dst, pr, cfg.pitch, cfg.pitch, cfg.lam, z)
             assert _phasor_rel_l2(th, pr) <= REL_L2, "restart at t=%d" % t
+
+
+@pytest.mark.parametrize("method", [0, 1])
+@pytest.mark.parametrize("shape", [(2048, 2048), (4096, 64), (64, 4096), (8192, 64), (64, 8192)])
+def test_gs_restart_parity_long_transforms(api, oracle, method, shape):
+    """The GS load / store modes (amp * exp(i phi) load, phasor x amplitude store, atan2 store) on the tile shapes of
+    the 4096- .. 16384-point transforms, full field: kinoform (iters = 0) and one-iteration restart from the
+    oracle's state after its first loop pass."""
+    cfg = W.CONFIGS["c5"]
+    ny, nx = shape
+    z = cfg.zs[0] * max(shape) / 8192
+    amp_src, amp_dst, phi0 = W.gs_inputs(shape, 7)
+    th = _gs_gpu(api, method, amp_src, amp_dst, phi0, cfg.pitch, cfg.lam, z, 0)
+    p = oracle.gs_init(method, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z)
+    assert _phasor_rel_l2(th, p) <= REL_L2, "kinoform %s" % (shape,)
+    # a phasor is ill-conditioned where the field is nearly zero (error e at amplitude a moves it by e/a): the
+    # maximum is only bounded loosely
+    assert np.max(np.abs(np.exp(1j * th.astype(np.float64)) - p)) <= 5e-2
+    p, G = oracle.gs_iter(method, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z, want_G=True)
+    phi_t = np.angle(G).astype(np.float32)
+    th = _gs_gpu(api, method, amp_src, amp_dst, phi_t, cfg.pitch, cfg.lam, z, 1)
+    pr = oracle.gs_init(method, amp_dst, phi_t, cfg.pitch, cfg.pitch, cfg.lam, z)
+    pr = oracle.gs_iter(method, amp_src, amp_dst, pr, cfg.pitch, cfg.pitch, cfg.lam, z)
+    assert _phasor_rel_l2(th, pr) <= REL_L2, "restart %s" % (shape,)
+
+
+def test_gs_20_iteration_drift_reported(api, oracle, capsys):
+    """the end-to-end phasor difference after 20 iterations is REPORTED, not gated at the
+    single-propagation bar (fp32 and fp64 trajectories separate at near-zero amplitudes); only a loose sanity bound."""
+    lines = []
+    for method, n in ((0, 512), (1, 512)):
+        cfg = W.CONFIGS["c5"].scaled(n)
+        z = cfg.zs[0] * n / 8192
+        amp_src, amp_dst, phi0 = W.gs_inputs_c5(cfg)
+        th = _gs_gpu(api, method, amp_src, amp_dst, phi0, cfg.pitch, cfg.lam, z, 20)
+        ref = oracle.gs(method, amp_src, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z, 20)
+        d = np.exp(1j * th.astype(np.float64)) - np.exp(1j * ref)
+        rel, mx = np.linalg.norm(d) / np.sqrt(d.size), np.abs(d).max()
+        lines.append("GS drift after 20 iterations, %s %d^2: phasor rel-L2 %.3e, max %.3e"
+                     % ("Fresnel" if method == 0 else "ASM", n, rel, mx))
+        assert rel < 5e-2
+    with capsys.disabled():
+        print("\n" + "\n".join(lines))
 
 
 def test_gs_error_curve_matches_oracle(api, oracle):
@@ -293,11 +359,15 @@ def test_gs_c5_full_size(api, oracle):
     api.cwo_gs(plan, d_src, d_dst, z, 0, th0)
     torch.cuda.synchronize()
     r = np.random.default_rng(3)
-    ms = r.integers(0, n, 6); ns = r.integers(0, n, 6)
+    ms = r.integers(0, n, 32); ns = r.integers(0, n, 32)
     G0 = (amp_dst.astype(np.float64) * np.exp(1j * phi0.astype(np.float64)))
     ref = oracle.fresnel_points(G0, cfg.pitch, cfg.pitch, cfg.lam, -z, ms, ns)
     got = np.exp(1j * th0.cpu().numpy()[ns, ms].astype(np.float64))
-    assert np.max(np.abs(got - ref / np.abs(ref))) < 2e-4
+    pref = ref / np.abs(ref)
+    # phasors: an error e of the field at amplitude a moves the phasor by e/a, so weigh by the sample's amplitude
+    wgt = np.minimum(1.0, np.abs(ref) / np.abs(ref).max() * 4)
+    assert np.linalg.norm((got - pref) * wgt) / np.linalg.norm(pref * wgt) <= REL_L2
+    assert np.max(np.abs(got - pref) * wgt) <= MAX_ABS
     e0 = recon_error(th0)
     th = _dev(phi0.copy())
     api.cwo_gs(plan, d_src, d_dst, z, cfg.iters, th)
@@ -386,7 +456,8 @@ def test_stack_batching_edges(api, oracle):
     for ws_planes, pipeline in ((4, 1), (2, 1), (17, 1), (4, 0)):
         plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
         plan.set_option(api.CWO_OPT_PIPELINE, pipeline)
-        plan.set_workspace(torch.empty(ws_planes * f, dtype=torch.uint8, device="cuda"))
+        tables = plan.workspace_bytes(api.CWO_OP_STACK, len(zs)) - (1 + len(zs)) * f      # the planes' phase tables
+        plan.set_workspace(torch.empty(ws_planes * f + tables, dtype=torch.uint8, device="cuda"))
         out = torch.empty((len(zs), n, n), dtype=torch.complex64, device="cuda")
         arr = (api.ctypes.c_double * len(zs))(*zs)
         plan.bind_stream()
@@ -516,6 +587,21 @@ def test_asm_pad2x_c1_evanescent_and_option_scope(api, oracle):
     big = api.cwo_plan(16384, 32, cfg.pitch, cfg.lam)
     with pytest.raises(api.CwoError):
         big.set_option(api.CWO_OPT_ASM_PAD2X, 1)
+
+
+def test_asm_pad2x_toggled_on_one_plan(api, oracle):
+    """circular -> zero-expanded -> circular on ONE plan (the per-z tables double in size with the option)."""
+    u1 = _rand((512, 1024), 35)
+    px, lam, z = 4e-6, 633e-9, 0.02
+    plan = api.cwo_plan(1024, 512, px, lam)
+    d1 = _dev(u1); d2 = torch.empty_like(d1)
+    for pad in (0, 1, 0, 1):
+        plan.set_option(api.CWO_OPT_ASM_PAD2X, pad)
+        for zz in (z, -0.5 * z):
+            api.cwo_asm(plan, d1, d2, zz)
+            torch.cuda.synchronize()
+            ref = (oracle.asm_pad2x if pad else oracle.asm)(u1, px, px, lam, zz)
+            _assert_parity(d2.cpu().numpy(), ref, "pad=%d z=%g" % (pad, zz))
 
 
 def test_asm_pad2x_4096(api, oracle):
