@@ -146,6 +146,29 @@ template <int R> __device__ __forceinline__ void unpermute_p(PV& v) {
         for (int q = 0; q < R; ++q) { v.r[i + q * S] = tr[i + perm<R>(q) * S]; v.i[i + q * S] = ti[i + perm<R>(q) * S]; }
 }
 
+// w32^e = exp(-i 2 pi e/32), e = 0..15: the twiddle of point x = us + e*Q (Q = n/16) is w^us * w32^e.
+// e is a compile-time constant after unrolling, so the table folds into immediates.
+__device__ __forceinline__ float2 w32_pow(int e) {
+    constexpr float c[16] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                             0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                             0.19509032201612826785f, 0.0f, -0.19509032201612826785f, -0.38268343236508977173f,
+                             -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                             -0.92387953251128675613f, -0.98078528040323044913f};
+    constexpr float sn[16] = {0.0f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                              0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                              0.98078528040323044913f, 1.0f, 0.98078528040323044913f, 0.92387953251128675613f,
+                              0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                              0.38268343236508977173f, 0.19509032201612826785f};
+    return make_float2(c[e], -sn[e]);
+}
+
+// w16^i = exp(-i 2 pi i/16), i = 0..7 (compile-time index after unrolling: folds into immediates)
+__device__ __forceinline__ float2 w16_pow(int i) {
+    constexpr float c[8] = {1.0f, CWO_C16, CWO_C8, CWO_S16, 0.0f, -CWO_S16, -CWO_C8, -CWO_C16};
+    constexpr float sn[8] = {0.0f, CWO_S16, CWO_C8, CWO_C16, 1.0f, CWO_C16, CWO_C8, CWO_S16};
+    return make_float2(c[i], -sn[i]);
+}
+
 // Twiddle (if lns > 0) and butterflies of one radix-2^LR stage; both slots are unit `us` (shared twiddles).
 // tw: shared-memory copy of the twiddle table (pipe_kernel.cuh).
 // war: an exchange follows directly; its write-after-read synchronisation is taken here, between the twiddles
@@ -158,8 +181,14 @@ __device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const floa
     for (int i = 0; i < S; ++i) {
         if (lns > 0) {
             float2 w[16];
-            const int k0 = (us + i * C::Q) & ((1 << lns) - 1);
-            powers<R>(tw[k0 << (LOGN - lns - LR)], w);
+            if (LR == 1 && lns == LOGN - 1) {
+                // last stage of n = 2 * 16^m: the twiddle of unit us + i Q is w^us w16^i (Q = n/16), so that only the
+                // first Q table entries are ever read (the shared-memory copy of the table holds just those)
+                w[1] = i == 0 ? tw[us] : cmul(tw[us], w16_pow(i));
+            } else {
+                const int k0 = (us + i * C::Q) & ((1 << lns) - 1);
+                powers<R>(tw[k0 << (LOGN - lns - LR)], w);
+            }
 #pragma unroll
             for (int r = 1; r < R; ++r) mul_tw1(v, i + r * S, w[r]);
         }

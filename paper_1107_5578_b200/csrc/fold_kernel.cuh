@@ -20,22 +20,6 @@
 
 namespace cwo {
 
-// w32^e = exp(-i 2 pi e/32), e = 0..15: the twiddle of point x = us + e*Q (Q = n/16) is w^us * w32^e.
-// e is a compile-time constant after unrolling, so the table folds into immediates.
-__device__ __forceinline__ float2 w32_pow(int e) {
-    constexpr float c[16] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
-                             0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
-                             0.19509032201612826785f, 0.0f, -0.19509032201612826785f, -0.38268343236508977173f,
-                             -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
-                             -0.92387953251128675613f, -0.98078528040323044913f};
-    constexpr float sn[16] = {0.0f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
-                              0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
-                              0.98078528040323044913f, 1.0f, 0.98078528040323044913f, 0.92387953251128675613f,
-                              0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
-                              0.38268343236508977173f, 0.19509032201612826785f};
-    return make_float2(c[e], -sn[e]);
-}
-
 template <int LOGC> struct FoldCfg {
     using C = Tile<LOGC>;
     static constexpr int GROUPS = 2, NBUF = 3, GT = 256;

@@ -55,10 +55,7 @@ template <int LOGN> struct ConvCfg {
     static constexpr bool PREFETCH = (C::MINB == 1);
     static constexpr size_t BAR_OFF = C::SMEM_BYTES;
     static constexpr size_t TW_OFF = BAR_OFF + 64;
-    // stage twiddles in shared memory when the table is small (n = 16^m: first n/16 entries); with a small radix
-    // (n = 2^L0 16^m) the table would be 16^m entries, and those lengths read it from global memory (L2)
-    static constexpr bool TW_SHARED = (C::L0 == 0) || LOGN <= 11;
-    static constexpr int NTW = TW_SHARED ? PP<LOGN>::NTW : 0;
+    static constexpr int NTW = PP<LOGN>::NTW_P;            // stage twiddles, copied to shared memory once per CTA
     static constexpr size_t PF_OFF = (TW_OFF + sizeof(float2) * NTW + 127) / 128 * 128;
     static constexpr size_t PF_BYTES = sizeof(float2) * (size_t)C::N * (C::W / 2);
     static constexpr size_t SMEM = PREFETCH ? PF_OFF + PF_BYTES : PF_OFF;
@@ -82,7 +79,7 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = threadIdx.x; i < K::NTW; i += C::T) tws[i] = __ldg(&P.tw[i]);
-    const float2* tw = K::TW_SHARED ? tws : P.tw;
+    const float2* tw = tws;
     const int us = threadIdx.x / H, hl = threadIdx.x % H, w0 = 2 * hl;
     const float2 wb = __ldg(&P.tw2[us]);                    // w^us; w^(us + e Q) = wb w32^e
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -133,7 +130,7 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
             }
         } else {
 #pragma unroll
-            for (int e = 0; e < 16; ++e) x[e] = P.in[base + e * Q];
+            for (int e = 0; e < 16; ++e) x[e] = __ldcs(&P.in[base + e * Q]);   // streamed: keep L1 for the tables
         }
 
 #pragma unroll 1
@@ -180,7 +177,7 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
         if constexpr (OUT == CONV_OUT_COMPLEX) {
             float2* out = reinterpret_cast<float2*>(P.out);
 #pragma unroll
-            for (int e = 0; e < 16; ++e) out[base + e * Q] = x[e];
+            for (int e = 0; e < 16; ++e) __stcs(&out[base + e * Q], x[e]);
         } else {
             // Eq.(25) P:L482 as atan2, by a rolled loop (atan2f would otherwise be unrolled 16 times)
             __syncthreads();

@@ -203,11 +203,16 @@ pass_kernel(const __grid_constant__ PassParams P) {
         // (nothing overlaps them: the whole tile goes to registers before the first butterfly) find it on chip
         if (threadIdx.x == 0 && P.pf_dist > 0 && tile + P.pf_dist < P.n_tiles)
             l2_prefetch(P.in + (size_t)(tile + P.pf_dist) * P.ly * W, (uint32_t)(P.ly * W * 8));
+        // stage twiddles: copied to shared memory behind the exchange buffer (the first stage has none, so the copy is
+        // covered by it); read from global memory they are evicted from L1 by the tile traffic and every stage
+        // would begin with an L2 round trip
+        float2* tws = reinterpret_cast<float2*>(reinterpret_cast<unsigned char*>(sm) + C::SMEM_BYTES + 64);
+        for (int i = threadIdx.x; i < PP<LOGN>::NTW_P; i += C::T) tws[i] = __ldg(&P.tw[i]);
         PV pv;
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             if (e < NE) {
-                const ulonglong2 t2 = src[((size_t)(u[0] + e * Q) * W + w0) >> 1];
+                const ulonglong2 t2 = __ldcs(&src[((size_t)(u[0] + e * Q) * W + w0) >> 1]);   // streamed: keep L1 for the tables
                 pv.r[e] = t2.x; pv.i[e] = t2.y;
             } else {
                 pv.r[e] = pv.i[e] = 0ull;
@@ -225,13 +230,14 @@ pass_kernel(const __grid_constant__ PassParams P) {
         const SyncSplit sy{&bars[0], &bars[1], 0u, 0u};
         sy.consumed();                                     // the region starts free
 #else
+        __syncthreads();
         const SyncCta sy;
 #endif
-        if constexpr (KIND == COL_FWD) transform_p<LOGN, true, false, false>(pv, u[0], w0, sm, P.tw, mid, sy);
-        else if constexpr (KIND == COL_FUSED) transform_p<LOGN, true, true, false>(pv, u[0], w0, sm, P.tw, mid, sy);
-        else transform_p<LOGN, false, true, true>(pv, u[0], w0, sm, P.tw, mid, sy);
+        if constexpr (KIND == COL_FWD) transform_p<LOGN, true, false, false>(pv, u[0], w0, sm, tws, mid, sy);
+        else if constexpr (KIND == COL_FUSED) transform_p<LOGN, true, true, false>(pv, u[0], w0, sm, tws, mid, sy);
+        else transform_p<LOGN, false, true, true>(pv, u[0], w0, sm, tws, mid, sy);
 #pragma unroll
-        for (int e = 0; e < NE; ++e) dst[((size_t)(u[0] + e * Q) * W + w0) >> 1] = make_ulonglong2(pv.r[e], pv.i[e]);
+        for (int e = 0; e < NE; ++e) __stcs(&dst[((size_t)(u[0] + e * Q) * W + w0) >> 1], make_ulonglong2(pv.r[e], pv.i[e]));
         return;
     }
     float2 v[2][16];
@@ -442,7 +448,14 @@ pass_kernel(const __grid_constant__ PassParams P) {
 
 template <int LOGN, int KIND, bool PAD, int MID, int IOM, bool X>
 static cudaError_t launch_x(int n_tiles, cudaStream_t s, const PassParams& p) {
-    constexpr size_t smem = ((X && KIND == ROW_FWD) ? Tile<LOGN>::SMEM_BYTES_X : Tile<LOGN>::SMEM_BYTES) + 64;   // + two mbarriers
+    // + two mbarriers + (packed column passes) the stage twiddles
+    constexpr bool PACKED = !(KIND == ROW_FWD || KIND == ROW_INV) && Tile<LOGN>::PAIR && MID != MID_ASM_F64 && LOGN >= 8;
+    constexpr size_t smem = ((X && KIND == ROW_FWD) ? Tile<LOGN>::SMEM_BYTES_X : Tile<LOGN>::SMEM_BYTES) + 64 +
+                            (PACKED ? sizeof(float2) * PP<LOGN>::NTW_P : 0)
+#ifdef CWO_FORCE_SMEM
+                            + (PACKED ? CWO_FORCE_SMEM : 0)
+#endif
+        ;
     DeviceInfo* d = device_info();
     if (!d) return cudaErrorInvalidDevice;
     static FuncOnce once;

@@ -206,7 +206,9 @@ template <int LOGN, int KIND> struct PipeCfg {
     static constexpr size_t BUF_RAW = (KIND == ROW_FWD && C::SMEM_BYTES_X > C::SMEM_BYTES) ? C::SMEM_BYTES_X : C::SMEM_BYTES;
     static constexpr size_t BUF = (BUF_RAW + 127) / 128 * 128;
     static constexpr size_t TW_OFF = NBUF * BUF + 64;                       // after the mbarriers
-    static constexpr size_t TW_BYTES = sizeof(float2) * PP<LOGN>::NTW;
+    // full-length stage twiddles, then (packed row passes) the half-length ones, tw_h[i] = tw_n[2i]
+    static constexpr int NTW_H = PP<LOGN - 1>::NTW_P;
+    static constexpr size_t TW_BYTES = sizeof(float2) * (PP<LOGN>::NTW + NTW_H);
     static constexpr size_t TAB_OFF = TW_OFF + TW_BYTES;                    // ASM: theta_y[l] (float, N entries)
     static constexpr size_t TAB_BYTES = sizeof(float) * C::N;
     static constexpr size_t SMEM_NOTAB = TAB_OFF, SMEM_TAB = TAB_OFF + TAB_BYTES;
@@ -248,6 +250,9 @@ pipe_kernel(const __grid_constant__ PassParams P) {
     float2* tws = reinterpret_cast<float2*>(smraw + K::TW_OFF);
     float* thy = reinterpret_cast<float*>(smraw + K::TAB_OFF);
     for (int i = threadIdx.x; i < PP<LOGN>::NTW; i += K::THREADS) tws[i] = __ldg(&P.tw[i]);
+    float2* twh = tws + PP<LOGN>::NTW;
+    if constexpr (KIND == ROW_FWD || KIND == ROW_INV)
+        for (int i = threadIdx.x; i < K::NTW_H; i += K::THREADS) twh[i] = __ldg(&P.tw[2 * i]);
     const bool batched = P.n_planes > 1;
     if constexpr (MID == MID_ASM_SPLIT) {
         const float* thp = reinterpret_cast<const float*>(P.tab_point);
@@ -379,8 +384,82 @@ pipe_kernel(const __grid_constant__ PassParams P) {
             mbar_arrive(&staged[b]);
             continue;
         }
-        // ---- row passes: scalar arithmetic, the two slots half a stage apart (pp_core.cuh) --------------
         static_assert(COLPASS || KIND == ROW_FWD || KIND == ROW_INV, "kind");
+        if constexpr (!PAD) {
+            // ---- unpadded row passes: packed arithmetic on (even bins, odd bins) lane pairs ------------------------
+            // One radix-2 step splits a row of n = 2h points into two h-point lanes with the same twiddles
+            // (rowfft scheme: forward a = x[m] + x[m+h], b = (x[m] - x[m+h]) w^m, X[2j] = FFT_h(a)[j], X[2j+1] =
+            // FFT_h(b)[j]; inverse x[m] = A[m] + w^-m B[m], x[m+h] = A[m] - w^-m B[m]).  (X[2j], X[2j+1]) is one planar
+            // 16-byte element of the column-tiled workspace = the register pair: half the butterfly instructions of
+            // the scalar form, no unit-pair mapping.  The tile's W rows are the W lane pairs of Tile<LOGN-1>.
+            using CH = Tile<LOGN - 1>;
+            static_assert(CH::T == K::GT && CH::W == 2 * W && CH::SMEM_BYTES <= K::BUF, "half-length tile shape");
+            constexpr int QH = CH::Q, H = CH::N;
+            const int hus = t / W, hr = t % W;                // unit and row of this thread
+            const float2 wb = tws[hus];                       // w^us (n-point table); w^(us + e QH) = wb w32^e
+            float2 tq[8];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) tq[e] = e == 0 ? wb : cmul(wb, w32_pow(e));
+            PV pv;
+            if constexpr (KIND == ROW_FWD) {
+                const float2* x = sm + hr * RS + hus;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const float2 lo = x[e * QH], hi = x[H + e * QH];
+                    const float2 a = cadd(lo, hi), d = csub(lo, hi);
+                    const float2 bb = e < 8 ? cmul(d, tq[e]) : cmul_mi(cmul(d, tq[e - 8]));
+                    pv.r[e] = pk_make(a.x, bb.x); pv.i[e] = pk_make(a.y, bb.y);
+                }
+                sync();                                       // staged image retired: the buffer is the exchange buffer now
+                transform_p<LOGN - 1, true, false, false>(pv, hus, 2 * hr, sm, twh, MidNone(), sync);
+                sync();                                       // nobody still reads the exchange image
+                // [x/Wc][row][x%Wc]: the pair (2j, 2j+1), j = hus + e QH, of row hr
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const int x2 = 2 * (hus + e * QH);
+                    float2* d = sm + ((((x2 >> P.logwc) * W + hr) << P.logwc) + (x2 & ((1 << P.logwc) - 1)));
+                    *reinterpret_cast<ulonglong2*>(d) = make_ulonglong2(pv.r[e], pv.i[e]);
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const int x2 = 2 * (hus + e * QH);
+                    const float2* d = sm + ((((x2 >> P.logwc) * W + hr) << P.logwc) + (x2 & ((1 << P.logwc) - 1)));
+                    const ulonglong2 q2 = *reinterpret_cast<const ulonglong2*>(d);
+                    pv.r[e] = q2.x; pv.i[e] = q2.y;           // conj(field): see the column store
+                }
+                sync();                                       // staged image retired
+                transform_p<LOGN - 1, false, true, false>(pv, hus, 2 * hr, sm, twh, MidNone(), sync);
+                sync();                                       // nobody still reads the exchange image
+                const float sc = P.out_scale;                 // conj completes the inverse transform
+                if constexpr (IOM == OUT_INTENSITY) {
+                    float* y = reinterpret_cast<float*>(sm) + hr * RS * 2 + hus;
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        float ar, br, ai, bi;
+                        pk_split(pv.r[e], ar, br); pk_split(pv.i[e], ai, bi);
+                        const float2 m = cmul(make_float2(br, bi), e < 8 ? tq[e] : cmul_mi(tq[e - 8]));
+                        const float2 lo = make_float2(ar + m.x, ai + m.y), hi = make_float2(ar - m.x, ai - m.y);
+                        y[e * QH] = (lo.x * lo.x + lo.y * lo.y) * (sc * sc);
+                        y[H + e * QH] = (hi.x * hi.x + hi.y * hi.y) * (sc * sc);
+                    }
+                } else {
+                    float2* y = sm + hr * RS + hus;
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        float ar, br, ai, bi;
+                        pk_split(pv.r[e], ar, br); pk_split(pv.i[e], ai, bi);
+                        const float2 m = cmul(make_float2(br, bi), e < 8 ? tq[e] : cmul_mi(tq[e - 8]));
+                        y[e * QH] = make_float2((ar + m.x) * sc, -(ai + m.y) * sc);
+                        y[H + e * QH] = make_float2((ar - m.x) * sc, -(ai - m.y) * sc);
+                    }
+                }
+            }
+            fence_proxy_async();
+            mbar_arrive(&staged[b]);
+            continue;
+        }
+        // ---- padded row passes: scalar arithmetic, the two slots half a stage apart (pp_core.cuh) --------
         float2 v[2][16];
 
         // ---- registers <- staged tile ------------------------------------------------------------

@@ -24,6 +24,8 @@ template <int LOGN> struct PP {
     static constexpr int REGION = (Tile<LOGN>::N + Tile<LOGN>::N / 16) * (Tile<LOGN>::W / 2);   // elements
     // twiddles a CTA keeps in shared memory: indices < N/16 for radix-16 stages, < 16^M for the small inverse radix
     static constexpr int NTW = Tile<LOGN>::L0 == 0 ? Tile<LOGN>::Q : (1 << (4 * Tile<LOGN>::M));
+    // the packed transforms (fft_packed.cuh) form the last radix-2 twiddles from the first Q entries
+    static constexpr int NTW_P = Tile<LOGN>::L0 <= 1 ? Tile<LOGN>::Q : (1 << (4 * Tile<LOGN>::M));
 };
 
 // outputs of a radix-2^LR stage with Ns = 2^lns, one slot, Stockham order.  The padded index of
