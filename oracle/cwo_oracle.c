@@ -24,6 +24,11 @@
  *                              form, Gaussian-beam closed form, adjoint identity
  *   fresnel_point      pinned: equals fresnel_direct / closed forms (it IS Eq.(1) discretised)
  *   stack              pinned: equals n independent asm calls + semigroup
+ *   stack_intensity    pinned: |stack|^2 element by element, sum = input energy (Parseval, no evanescent bin)
+ *   asm_shifted        pinned: band covers the grid and O = 0 -> asm; plane wave inside the band -> H ramp u1 with
+ *                              the band edge of Ref.[56]'s closed form typed in the test, outside -> exactly 0;
+ *                              O = a whole number of pitches -> circular shift of asm (sign of the ramp);
+ *                              z -> -z mirrors the band; the mask only removes energy
  *   gs                 pinned: iters=0 kinoform identity, error non-increasing with the
  *                              unitary ASM propagator (Fienup), fixed point on a
  *                              consistent pair, step-by-step restatement in numpy
@@ -228,6 +233,56 @@ int cwo_oracle_stack(int ny, int nx, double px, double py, double lambda, const 
     for (int k = 0; k < n; ++k)
         if (cwo_oracle_asm(ny, nx, px, py, lambda, zs[k], u1, out + (size_t)k * nx * ny)) return -1;
     return 0;
+}
+
+/* Intensity of every plane of the stack, Eq.(20): I = |u|^2 (what the paper's 3-D example stores for
+ * rendering).  Written as the stack followed by the absolute square. */
+int cwo_oracle_stack_intensity(int ny, int nx, double px, double py, double lambda, const double* zs, int n,
+                               const zc* u1, double* out) {
+    size_t f = (size_t)nx * ny;
+    zc* plane = (zc*)malloc(sizeof(zc) * f);
+    if (!plane) return -1;
+    for (int k = 0; k < n; ++k) {
+        if (cwo_oracle_asm(ny, nx, px, py, lambda, zs[k], u1, plane)) { free(plane); return -1; }
+        for (size_t i = 0; i < f; ++i) {
+            double re = creal(plane[i]), im = cimag(plane[i]);
+            out[(size_t)k * f + i] = re * re + im * im;
+        }
+    }
+    free(plane);
+    return 0;
+}
+
+/* ---- shifted (band-limited) angular spectrum method: Eq.(18)-(19), P:L213-229 ---------------------------------
+ * u2 = IDFT2[ DFT2[u1] . H_SA . Rect((m1-cx)/wx) . Rect((n1-cy)/wy) ],
+ * H_SA = H_A exp(i 2 pi (Ox fx + Oy fy))                  (Eq.(19); the "i" is missing in the extracted text, D-R15)
+ * The paper refers to its Ref.[56] for cx, wx, cy, wy.  D-R15: they are the bins where the phase of H_SA,
+ * sampled at the pitch df of the frequency grid, is not aliased -- its local frequency |d(phase)/df| / 2 pi =
+ * |O - z f / sqrt(1/lambda^2 - f^2)| must not exceed 1/(2 df) -- evaluated per axis ON that axis (the other
+ * frequency 0), which is what makes the limit a product of two Rects.  A bin with f^2 >= 1/lambda^2 is outside. */
+static int shifted_keep(double f, double df, double off, double lambda, double z) {
+    double inv_lam2 = 1.0 / (lambda * lambda);
+    double w = inv_lam2 - f * f;
+    if (w <= 0.0) return 0;
+    return fabs(off - z * f / sqrt(w)) <= 0.5 / df;
+}
+
+int cwo_oracle_asm_shifted(int ny, int nx, double px, double py, double lambda, double z, double ox, double oy,
+                           const zc* u1, zc* u2) {
+    size_t n = (size_t)nx * ny;
+    double dfx = 1.0 / ((double)nx * px), dfy = 1.0 / ((double)ny * py);
+    if (u2 != u1) memcpy(u2, u1, sizeof(zc) * n);
+    if (cwo_oracle_fft2d(ny, nx, u2, -1)) return -1;
+    #pragma omp parallel for num_threads(g_threads) schedule(static)
+    for (int l = 0; l < ny; ++l)
+        for (int k = 0; k < nx; ++k) {
+            double fx = signed_bin(k, nx) * dfx, fy = signed_bin(l, ny) * dfy;
+            zc h = 0;
+            if (shifted_keep(fx, dfx, ox, lambda, z) && shifted_keep(fy, dfy, oy, lambda, z))
+                h = asm_H(k, l, nx, ny, px, py, lambda, z) * cis_cycles(ox * fx + oy * fy);
+            u2[(size_t)l * nx + k] *= h;
+        }
+    return cwo_oracle_fft2d(ny, nx, u2, +1);
 }
 
 /* ---- Fresnel diffraction, convolution form: Eq.(1)-(6), P:L98-135 ------------ */

@@ -61,6 +61,8 @@ def lib():
     L.cwo_oracle_asm_naive.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_asm_pad2x.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_stack.argtypes = [_I, _I, _D, _D, _D, _f64, _I, _c128, _c128]
+    L.cwo_oracle_stack_intensity.argtypes = [_I, _I, _D, _D, _D, _f64, _I, _c128, _f64]
+    L.cwo_oracle_asm_shifted.argtypes = [_I, _I, _D, _D, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_fresnel_points.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _I, _i32, _i32, _c128]
     L.cwo_oracle_fresnel_direct.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_fresnel_conv.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
@@ -154,6 +156,23 @@ def stack(u1, px, py, lam, zs):
     out = np.empty((zs.size, ny, nx), np.complex128)
     _check(lib().cwo_oracle_stack(ny, nx, px, py, lam, zs, zs.size, u1, out), "stack")
     return out
+
+
+def stack_intensity(u1, px, py, lam, zs):
+    """|Diffract3D|^2, Eq.(20) P:L254-256 on every plane of the stack."""
+    u1 = _z(u1); zs = _d(zs)
+    ny, nx = u1.shape
+    out = np.empty((zs.size, ny, nx), np.float64)
+    _check(lib().cwo_oracle_stack_intensity(ny, nx, px, py, lam, zs, zs.size, u1, out), "stack_intensity")
+    return out
+
+
+def asm_shifted(u1, px, py, lam, z, ox=0.0, oy=0.0):
+    """Shifted (band-limited) angular spectrum method, Eq.(18)-(19) P:L213-229; (ox, oy) = destination offset [m]."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    _check(lib().cwo_oracle_asm_shifted(ny, nx, px, py, lam, z, ox, oy, u1, u2), "asm_shifted")
+    return u2
 
 
 def fresnel_conv(u1, px, py, lam, z):
