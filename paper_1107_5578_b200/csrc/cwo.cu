@@ -382,19 +382,19 @@ static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, i
 }
 
 // Band limits of the shifted angular spectrum method, Eq.(18) P:L213-229 (parameters per Ref.[56] of the paper,
-// DESIGN.md reading R15): the phase of H_SA sampled at df must not alias, |O - z f/sqrt(1/lambda^2 - f^2)| <= 1/(2 df)
-// evaluated per axis on the axis itself.  Signed-bin range [lo, hi] of the bins kept (empty when lo > hi).
+// DESIGN.md reading R15): a bin is kept when the phase of H_SA sampled at df is not aliased,
+// |O - z f/sqrt(1/lambda^2 - f^2)| <= 1/(2 df), evaluated per axis on the axis itself.  The kept bins form an
+// interval (the left side is monotone in f): signed-bin range [lo, hi], empty when lo > hi.
+static bool band_keep(double f, double df, double off, double lambda, double z) {
+    const double inv_lam2 = 1.0 / (lambda * lambda);
+    const double w = inv_lam2 - f * f;
+    if (w <= 0.0) return false;
+    return fabs(off - z * f / sqrt(w)) <= 0.5 / df;
+}
 static void band_range(double z, double lambda, double off, double df, int m, int* lo_out, int* hi_out) {
-    const double S = 0.5 / df, az = fabs(z);
-    // |z| f / sqrt(1/lambda^2 - f^2) in [o - S, o + S], o = sgn(z) O;  f = t / (lambda sqrt(t^2 + z^2))
-    const double o = z < 0 ? -off : off;
-    const double t0 = o - S, t1 = o + S;
     int lo = -m / 2, hi = m / 2 - 1;
-    if (az > 0.0) {
-        const double f0 = t0 / (lambda * sqrt(t0 * t0 + az * az)), f1 = t1 / (lambda * sqrt(t1 * t1 + az * az));
-        while (lo <= hi && (double)lo * df < f0) ++lo;
-        while (hi >= lo && (double)hi * df > f1) --hi;
-    }
+    while (lo <= hi && !band_keep((double)lo * df, df, off, lambda, z)) ++lo;
+    while (hi >= lo && !band_keep((double)hi * df, df, off, lambda, z)) --hi;
     *lo_out = lo; *hi_out = hi;
 }
 

@@ -609,3 +609,119 @@ def test_asm_pad2x_4096(api, oracle):
     u1 = W.make_field(cfg)
     _assert_parity(_gpu_asm_pad2x(api, u1, cfg.pitch, cfg.pitch, cfg.lam, 0.1), oracle.asm_pad2x(u1, cfg.pitch, cfg.pitch, cfg.lam, 0.1),
                    "asm pad2x 4096")
+
+
+# ---------------------------------------------------------------- shifted / band-limited ASM ---------
+
+def _gpu_asm_shifted(api, u1, px, py, lam, z, ox=0.0, oy=0.0):
+    ny, nx = u1.shape
+    plan = api.cwo_plan(nx, ny, px, lam)
+    if px != py:
+        plan.set_pitch_xy(px, py)
+    plan.set_option(api.CWO_OPT_ASM_BAND_LIMIT, 1)
+    plan.set_offset(ox, oy)
+    d1 = _dev(u1); d2 = torch.empty_like(d1)
+    api.cwo_asm(plan, d1, d2, z)
+    torch.cuda.synchronize()
+    return d2.cpu().numpy()
+
+
+@pytest.mark.parametrize("shape", [(64, 64), (128, 32), (256, 512), (1024, 1024), (512, 4096), (2048, 2048), (32, 16384)])
+def test_asm_band_limited_and_shifted(api, oracle, shape):
+    """Eq.(18)-(19): the band limit cuts part of the grid (z chosen so that the edge is at ~1/3 of the Nyquist
+    frequency of the longer axis), on axis and with an offset of a non-integer number of pitches, both signs of z.
+    Scalar tiles (< 256 points), lane-pair tiles and the single-lane 16384-point tile."""
+    ny, nx = shape
+    px, py, lam = 4e-6, 5e-6, 633e-9
+    n = max(nx, ny)
+    p = px if nx >= ny else py
+    z = n * p * p / lam * 1.5                            # band edge = Nyquist / 3 along the longer axis
+    u1 = _rand(shape, 51)
+    for zz, ox, oy in ((z, 0.0, 0.0), (-z, 0.0, 0.0), (z, 37.3 * px, -11.6 * py)):
+        ref = oracle.asm_shifted(u1, px, py, lam, zz, ox, oy)
+        assert np.linalg.norm(ref) < 0.9 * np.linalg.norm(u1)            # the band really removes something
+        _assert_parity(_gpu_asm_shifted(api, u1, px, py, lam, zz, ox, oy), ref, "shifted asm %s z=%g O=(%g,%g)" % (shape, zz, ox, oy))
+
+
+def test_asm_band_limited_fp64_path_and_option_off(api, oracle):
+    # pitch < lambda / sqrt(2): the per-sample fp64 transfer function (evanescent bins) with the band limit and the ramp
+    u1 = _rand((64, 64), 53)
+    d, lam, z = 0.3e-6, 633e-9, 2e-5
+    _assert_parity(_gpu_asm_shifted(api, u1, d, d, lam, z, 3.2 * d, -1.5 * d), oracle.asm_shifted(u1, d, d, lam, z, 3.2 * d, -1.5 * d),
+                   "shifted asm, fp64 path")
+    # the offset has no effect while the option is off
+    plan = api.cwo_plan(64, 64, 4e-6, lam)
+    plan.set_offset(1e-4, 1e-4)
+    d1 = _dev(u1); d2 = torch.empty_like(d1)
+    api.cwo_asm(plan, d1, d2, 0.01)
+    torch.cuda.synchronize()
+    _assert_parity(d2.cpu().numpy(), oracle.asm(u1, 4e-6, 4e-6, lam, 0.01), "option off")
+
+
+# ---------------------------------------------------------------- intensity stack (SURVEY 8(f) f4) --------------------
+
+@pytest.mark.parametrize("n,pipeline", [(256, 1), (1024, 1), (1024, 0), (2048, 1)])
+def test_stack_intensity(api, oracle, n, pipeline):
+    """CWO_OPT_STACK_INTENSITY: float |u|^2 planes (Eq.(20)) from the batched and the unbatched launches."""
+    cfg = W.CONFIGS["c4"].scaled(n)
+    u1 = W.make_field(cfg)
+    zs = [0.001, 0.0047, -0.002, 0.064, 0.03]
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    plan.set_option(api.CWO_OPT_PIPELINE, pipeline)
+    plan.set_option(api.CWO_OPT_STACK_INTENSITY, 1)
+    out = torch.empty((len(zs), n, n), dtype=torch.float32, device="cuda")
+    api.cwo_propagate_stack(plan, _dev(u1), zs, out)
+    torch.cuda.synchronize()
+    ref = oracle.stack_intensity(u1, cfg.pitch, cfg.pitch, cfg.lam, zs)
+    got = out.cpu().numpy().astype(np.float64)
+    for k in range(len(zs)):
+        rel = np.linalg.norm(got[k] - ref[k]) / np.linalg.norm(ref[k])
+        mx = np.max(np.abs(got[k] - ref[k])) / np.max(ref[k])
+        # |u|^2 doubles the relative error of u: bars 2 x (2e-5, 1e-4)
+        assert rel <= 2 * REL_L2 and mx <= 2 * MAX_ABS, "intensity plane %d: %.3e %.3e" % (k, rel, mx)
+
+
+# ---------------------------------------------------------------- the calls only enqueue: CUDA graph capture ----------
+
+def test_calls_capture_into_a_cuda_graph_and_replay(api, oracle):
+    """include/cwo.h: every propagation call only enqueues kernels on the plan's stream (no allocation, no
+    synchronisation, no copy), so a sequence of calls can be captured into a CUDA graph and replayed on new data."""
+    n = 512
+    cfg = W.CONFIGS["c3"].scaled(n)
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    for op in (api.CWO_OP_ASM, api.CWO_OP_FRESNEL, api.CWO_OP_GS, api.CWO_OP_STACK):
+        plan.ensure_workspace(op, 3)
+    amp_src, amp_dst, phi0 = W.gs_inputs((n, n), 3)
+    a = torch.empty((n, n), dtype=torch.complex64, device="cuda")
+    b = torch.empty_like(a); c = torch.empty_like(a)
+    st = torch.empty((3, n, n), dtype=torch.complex64, device="cuda")
+    d_src, d_dst, d_phi = _dev(amp_src), _dev(amp_dst), _dev(phi0)
+    zs = [0.002, 0.004, -0.003]
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        # warm-up outside the capture (lazy module loading is not capturable)
+        api.cwo_asm(plan, a, b, 0.01); api.cwo_fresnel_conv(plan, b, c, 0.4)
+        api.cwo_propagate_stack(plan, a, zs, st); api.cwo_gs(plan, d_src, d_dst, 0.02, 1, d_phi)
+        s.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            api.cwo_asm(plan, a, b, 0.01)
+            api.cwo_fresnel_conv(plan, b, c, 0.4)
+            api.cwo_propagate_stack(plan, a, zs, st)
+            api.cwo_gs(plan, d_src, d_dst, 0.02, 2, d_phi)
+    for seed in (61, 62):
+        u1 = _rand((n, n), seed)
+        a.copy_(_dev(u1)); d_phi.copy_(_dev(phi0))
+        g.replay()
+        torch.cuda.synchronize()
+        ref_b = oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, 0.01)
+        _assert_parity(b.cpu().numpy(), ref_b, "graph: asm")
+        _assert_parity(c.cpu().numpy(), oracle.fresnel_conv(b.cpu().numpy(), cfg.pitch, cfg.pitch, cfg.lam, 0.4), "graph: fresnel")
+        ref_s = oracle.stack(u1, cfg.pitch, cfg.pitch, cfg.lam, zs)
+        for k in range(3):
+            _assert_parity(st[k].cpu().numpy(), ref_s[k], "graph: stack %d" % k)
+        p = oracle.gs_init(0, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, 0.02)
+        for _ in range(2):
+            p = oracle.gs_iter(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, 0.02)
+        assert _phasor_rel_l2(d_phi.cpu().numpy(), p) <= 5 * REL_L2     # two iterations: drift allowance (SURVEY G5)
