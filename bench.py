@@ -179,7 +179,7 @@ def run_reference(args):
 
 WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
              "c2": ("fresnel", 1024), "fresnel2048": ("fresnel", 2048), "fresnel4096": ("fresnel", 4096),
-             "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c5": ("gs", 8192),
+             "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c4_intensity": ("stack_i", 2048), "c5": ("gs", 8192),
              "asm_pad2x_2048": ("asm_pad", 2048), "asm_pad2x_4096": ("asm_pad", 4096)}
 
 
@@ -245,13 +245,17 @@ def make_workload(name, rank, torch, api, W):
         return dict(plan=plan, step=step, N=N, props_per_step=1, bytes_per_step=bps, kind_bytes=kb, kind_flops=kf, e2e=e2e,
                     desc=desc, l2=l2, scheme_bytes_per_step=scheme,
                     metric="propagations/sec (%s); effective HBM GB/s for the algorithmic bytes" % name)
-    if op == "stack":
+    if op in ("stack", "stack_i"):
         cfg = W.CONFIGS["c4"]
         n = len(cfg.zs)
         host = W.make_field(cfg)
         u1 = torch.from_numpy(host).cuda()
-        out = torch.empty((n, N, N), dtype=torch.complex64, device="cuda")
+        inten = op == "stack_i"              # float |u|^2 planes (CWO_OPT_STACK_INTENSITY), half the output
+        odt = torch.float32 if inten else torch.complex64
+        out = torch.empty((n, N, N), dtype=odt, device="cuda")
         plan = api.cwo_plan(N, N, cfg.pitch, cfg.lam)
+        if inten:
+            plan.set_option(api.CWO_OPT_STACK_INTENSITY, 1)
         plan.ensure_workspace(api.CWO_OP_STACK, n)
 
         def step(i):
@@ -259,19 +263,20 @@ def make_workload(name, rank, torch, api, W):
 
         def e2e():
             pin_in = torch.from_numpy(host).pin_memory()
-            pin_out = torch.empty((n, N, N), dtype=torch.complex64).pin_memory()
+            pin_out = torch.empty((n, N, N), dtype=odt).pin_memory()
             d_in = torch.empty_like(u1)
 
             def f(i):
                 d_in.copy_(pin_in, non_blocking=True)
                 api.cwo_propagate_stack(plan, d_in, cfg.zs, out)
                 pin_out.copy_(out, non_blocking=True)
-            return f, 8 * n2, 8 * n2 * n
-        return dict(plan=plan, step=step, N=N, props_per_step=n, bytes_per_step=32 * n2 + n * 32 * n2,
-                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: 16 * 16 * n2, 1: 16 * 16 * n2}, kind_flops={},
-                    scheme_bytes_per_step=32 * n2 + n * 32 * n2, e2e=e2e,
-                    desc="c4: depth stack, one 2048x2048 random-phase field to 64 planes z = 1..64 mm by ASM, lambda 633 nm, "
-                         "pitch 6.4 um, out 64x2048x2048 complex64",
+            return f, 8 * n2, (4 if inten else 8) * n2 * n
+        per_plane = 28 if inten else 32      # C': 8 rd + 8 wr, R': 8 rd + 8 (4) wr
+        return dict(plan=plan, step=step, N=N, props_per_step=n, bytes_per_step=32 * n2 + n * per_plane * n2,
+                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: 16 * 16 * n2, 1: 16 * (per_plane - 16) * n2}, kind_flops={},
+                    scheme_bytes_per_step=32 * n2 + n * per_plane * n2, e2e=e2e,
+                    desc="%s: depth stack, one 2048x2048 random-phase field to 64 planes z = 1..64 mm by ASM, lambda 633 nm, "
+                         "pitch 6.4 um, out 64x2048x2048 %s" % (name, "float32 intensity" if inten else "complex64"),
                     l2="spectrum (34 MB) stays in L2; the 2.1 GB output stack streams to HBM; no flush",
                     metric="planes/sec (c4 depth stack); effective HBM GB/s for 32 N^2 + n 32 N^2 bytes")
     cfg = W.CONFIGS["c5"]
@@ -466,7 +471,7 @@ def main():
                     help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = {"c5": 3, "c4": 20, "fresnel8192": 50, "asm8192": 100}.get(args.workload, 300)
+        args.steps = {"c5": 3, "c4": 20, "c4_intensity": 20, "fresnel8192": 50, "asm8192": 100}.get(args.workload, 300)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -102,6 +102,12 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
 #pragma unroll 1
     for (int tile = blockIdx.x; tile < P.n_tiles; ++it) {
         const size_t base = (size_t)(tile * H + hl) * N + us;           // sample n = us + e Q of this thread's line
+        // the amplitudes of the constraint are sent for (to L2) a convolution ahead
+        if (NCONV > 1 && threadIdx.x == 0) l2_prefetch(P.mid_amp + (size_t)tile * H * N, (uint32_t)(H * N * sizeof(float)));
+        // persistent form: the next tile's index is asked for now and used after the first barrier (the round trip of
+        // the atomic is covered by the loads)
+        int nt = 0;
+        if (K::PREFETCH && threadIdx.x == 0) nt = (int)gridDim.x + atomicAdd(P.counter, 1);
         float2 x[16];
         if constexpr (IN == CONV_IN_AMP_PHASE) {
             // GS step 1, Listing 8 lines 3-5: amp exp(i phase) with the accurate sincosf, by a rolled loop staged
@@ -124,7 +130,6 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
             for (int e = 0; e < 16; ++e) x[e] = pf[hl * N + us + e * Q];
             __syncthreads();                                 // everybody has its registers: the buffer is free
             if (threadIdx.x == 0) {
-                const int nt = (int)gridDim.x + atomicAdd(P.counter, 1);
                 *next_tile = nt;
                 if (nt < P.n_tiles) { fence_proxy_async(); fetch(nt); }
             }
@@ -193,7 +198,7 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
             __syncthreads();
         }
         if constexpr (!K::PREFETCH) break;                   // one CTA per tile
-        if constexpr (!PF) { if (threadIdx.x == 0) *next_tile = (int)gridDim.x + atomicAdd(P.counter, 1); }
+        if constexpr (!PF) { if (threadIdx.x == 0) *next_tile = nt; }
         __syncthreads();
         tile = *next_tile;
     }
