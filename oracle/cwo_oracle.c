@@ -29,6 +29,15 @@
  *                              the band edge of Ref.[56]'s closed form typed in the test, outside -> exactly 0;
  *                              O = a whole number of pitches -> circular shift of asm (sign of the ramp);
  *                              z -> -z mirrors the band; the mask only removes energy
+ *   fresnel_general_*  pinned: Gaussian-beam closed form sampled at another pitch and offset, delta response closed
+ *                              form, equal pitches and no offset -> fresnel_direct (it IS Eq.(1) discretised)
+ *   fresnel_fourier    pinned: fresnel_general_direct at the destination pitch lambda|z|/(N p) (both signs of z),
+ *                              Gaussian-beam closed form, delta response closed form
+ *   fresnel_shifted    pinned: fresnel_general_direct (pitches, offsets of both planes, z < 0), p1 = p0 and no offset
+ *                              -> fresnel_conv, p1 = lambda z/(N p0) -> fresnel_fourier
+ *   scale255           pinned: min -> 0, max -> 255, affine, numpy restatement
+ *   pls_cgh            pinned: one on-axis point = Fresnel zone plate with zeros at the closed-form radii, symmetry,
+ *                              linearity in A_j, numpy restatement at 50-digit-checked samples
  *   gs                 pinned: iters=0 kinoform identity, error non-increasing with the
  *                              unitary ASM propagator (Fienup), fixed point on a
  *                              consistent pair, step-by-step restatement in numpy
@@ -368,6 +377,175 @@ int cwo_oracle_fresnel_conv(int ny, int nx, double px, double py, double lambda,
     }
     free(U); free(Hh);
     return rc;
+}
+
+/* ---- Fresnel diffraction between planes of different pitch and lateral offset ------------------
+ * Eq.(1) P:L102 discretised with the source plane sampled at x0 = m0 p0x + O0x and the destination at
+ * x1 = m1 p1x + O1x (Eq.(14)), m = array index - N/2 (Eq.(4)):
+ *   u2[n1][m1] = exp(i 2 pi z/lambda)/(i lambda z) p0x p0y sum_{m0,n0} u1[n0][m0]
+ *                exp(i pi ((x1 - x0)^2 + (y1 - y0)^2)/(lambda z)).
+ * This sum is what BOTH the Fourier form (Eq.(7)-(9) P:L137-158) and the shifted Fresnel diffraction
+ * (Eq.(10)-(14) P:L160-192) evaluate; it is their plain definition (area element as in D-R6).
+ * Offsets are in metres (D-R16: the paper's O are in samples of their own plane, O[m] = p O[samples]). */
+typedef struct { double p0x, p0y, p1x, p1y, o0x, o0y, o1x, o1y; } fres_geom;
+
+static zc fresnel_general_point(int ny, int nx, const fres_geom* g, double lambda, double z,
+                                const zc* u1, int m1i, int n1i) {
+    double x1 = (m1i - nx / 2) * g->p1x + g->o1x, y1 = (n1i - ny / 2) * g->p1y + g->o1y;
+    zc acc = 0;
+    for (int n0 = 0; n0 < ny; ++n0) {
+        double dy = y1 - ((n0 - ny / 2) * g->p0y + g->o0y);
+        zc row = 0;
+        for (int m0 = 0; m0 < nx; ++m0) {
+            zc v = u1[(size_t)n0 * nx + m0];
+            if (v == 0) continue;
+            double dx = x1 - ((m0 - nx / 2) * g->p0x + g->o0x);
+            row += v * cis_cycles((dx * dx + dy * dy) / (2.0 * lambda * z));
+        }
+        acc += row;
+    }
+    return fresnel_coeff(g->p0x, g->p0y, lambda, z) * acc;
+}
+
+/* Whole field by the direct sum, O(N^4): tiny grids.  geom = {p0x,p0y,p1x,p1y,o0x,o0y,o1x,o1y}. */
+void cwo_oracle_fresnel_general_direct(int ny, int nx, const double* geom, double lambda, double z,
+                                       const zc* u1, zc* u2) {
+    fres_geom g = {geom[0], geom[1], geom[2], geom[3], geom[4], geom[5], geom[6], geom[7]};
+    #pragma omp parallel for num_threads(g_threads) schedule(static)
+    for (int n1 = 0; n1 < ny; ++n1)
+        for (int m1 = 0; m1 < nx; ++m1)
+            u2[(size_t)n1 * nx + m1] = fresnel_general_point(ny, nx, &g, lambda, z, u1, m1, n1);
+}
+
+/* Samples (ms[i], ns[i]) (array indices) of the direct sum, for full-size spot checks. */
+void cwo_oracle_fresnel_general_points(int ny, int nx, const double* geom, double lambda, double z,
+                                       const zc* u1, int npts, const int* ms, const int* ns, zc* out) {
+    fres_geom g = {geom[0], geom[1], geom[2], geom[3], geom[4], geom[5], geom[6], geom[7]};
+    #pragma omp parallel for num_threads(g_threads) schedule(dynamic, 1)
+    for (int i = 0; i < npts; ++i)
+        out[i] = fresnel_general_point(ny, nx, &g, lambda, z, u1, ms[i], ns[i]);
+}
+
+/* Fresnel diffraction, Fourier form, the literal Eq.(8)-(9) P:L149-156:
+ *   u' = u1 exp(i pi (x1^2 + y1^2)/(lambda z));   U = FFT[u'] over the centred indices m = j - N/2;
+ *   u2 = exp(i 2 pi z/lambda)/(i lambda z) exp(i pi (x2^2 + y2^2)/(lambda z)) U  (times p1x p1y, D-R6),
+ * on the destination pitch p2 = lambda |z| / (N p1) (D-R17: P:L158's "Delta x1/(lambda z)" is garbled; this is the
+ * pitch at which the kernel exp(-i 2 pi x2 x1/(lambda z)) of Eq.(7) becomes the DFT kernel exp(-+ i 2 pi m1 m2/N);
+ * for z < 0 its sign flips and "FFT" is the unnormalised inverse transform).  The centred transform is taken by
+ * rotating the array by N/2 before and after a plain FFT (the DFT kernel is periodic in both indices). */
+int cwo_oracle_fresnel_fourier(int ny, int nx, double px, double py, double lambda, double z,
+                               const zc* u1, zc* u2) {
+    if (z == 0.0) return -2;
+    if (nx < 2 || ny < 2 || (nx & (nx - 1)) || (ny & (ny - 1))) return -1;
+    size_t n = (size_t)nx * ny;
+    double p2x = lambda * fabs(z) / (nx * px), p2y = lambda * fabs(z) / (ny * py);
+    zc* a = (zc*)malloc(sizeof(zc) * n);
+    if (!a) return -3;
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            double x = (i - nx / 2) * px, y = (j - ny / 2) * py;
+            zc v = u1[(size_t)j * nx + i] * cis_cycles((x * x + y * y) / (2.0 * lambda * z));      /* Eq.(8) */
+            a[(size_t)((j + ny / 2) % ny) * nx + (i + nx / 2) % nx] = v;                          /* m = 0 -> index 0 */
+        }
+    int rc = cwo_oracle_fft2d(ny, nx, a, z > 0 ? -1 : +1);
+    if (!rc) {
+        double undo = z > 0 ? 1.0 : (double)nx * (double)ny;       /* fft2d's inverse carries 1/(nx ny); Eq.(9) does not */
+        zc c = fresnel_coeff(px, py, lambda, z);
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double x = (i - nx / 2) * p2x, y = (j - ny / 2) * p2y;
+                zc U = a[(size_t)((j + ny / 2) % ny) * nx + (i + nx / 2) % nx] * undo;
+                u2[(size_t)j * nx + i] = c * cis_cycles((x * x + y * y) / (2.0 * lambda * z)) * U;  /* Eq.(9) */
+            }
+    }
+    free(a);
+    return rc;
+}
+
+/* Shifted Fresnel diffraction, the algorithm of Eq.(10)-(14) P:L160-192 step by step (paper's notation, plane 0 =
+ * source, plane 1 = destination; S = p0 p1/(lambda z)):
+ *   u1'[m0,n0] = u1 exp(i pi (x0^2 + y0^2)/(lambda z)) exp(-i 2 pi (m0 Sx O1x/p1x + n0 Sy O1y/p1y))
+ *                exp(-i pi (Sx m0^2 + Sy n0^2))                                                   Eq.(12)
+ *   h[m,n]     = exp(i pi (Sx m^2 + Sy n^2))                                                      Eq.(13)
+ *   C_S[m1,n1] = coefficient exp(i pi (x1^2 + y1^2)/(lambda z)) exp(-i 2 pi (O0x x1 + O0y y1)/(lambda z))
+ *                exp(-i pi (Sx m1^2 + Sy n1^2))                                                   Eq.(11)
+ *   u2 = C_S IFFT[FFT[u1'] FFT[h]]                                                                Eq.(10)
+ * with the convolution made linear by the 2N expansion of P:L235 exactly as in fresnel_conv (taps d = -N..N-1
+ * wrapped at d mod 2N).  m, n are the centred indices; the coefficient carries p0x p0y (D-R6). */
+int cwo_oracle_fresnel_shifted(int ny, int nx, const double* geom, double lambda, double z,
+                               const zc* u1, zc* u2) {
+    if (z == 0.0) return -2;
+    fres_geom g = {geom[0], geom[1], geom[2], geom[3], geom[4], geom[5], geom[6], geom[7]};
+    const double sx = g.p0x * g.p1x / (lambda * z), sy = g.p0y * g.p1y / (lambda * z);
+    int mx = 2 * nx, my = 2 * ny;
+    size_t mm = (size_t)mx * my;
+    zc* U = (zc*)calloc(mm, sizeof(zc));
+    zc* Hh = (zc*)malloc(sizeof(zc) * mm);
+    if (!U || !Hh) { free(U); free(Hh); return -3; }
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            double m0 = i - nx / 2, n0 = j - ny / 2;
+            double x0 = m0 * g.p0x + g.o0x, y0 = n0 * g.p0y + g.o0y;
+            zc f = cis_cycles((x0 * x0 + y0 * y0) / (2.0 * lambda * z))
+                 * cis_cycles(-(m0 * sx * g.o1x / g.p1x + n0 * sy * g.o1y / g.p1y))
+                 * cis_cycles(-0.5 * (sx * m0 * m0 + sy * n0 * n0));
+            U[(size_t)j * mx + i] = u1[(size_t)j * nx + i] * f;                                   /* Eq.(12) */
+        }
+    #pragma omp parallel for num_threads(g_threads) schedule(static)
+    for (int iy = 0; iy < my; ++iy) {
+        double dn = (iy < ny) ? iy : iy - my;
+        for (int ix = 0; ix < mx; ++ix) {
+            double dm = (ix < nx) ? ix : ix - mx;
+            Hh[(size_t)iy * mx + ix] = cis_cycles(0.5 * (sx * dm * dm + sy * dn * dn));           /* Eq.(13) */
+        }
+    }
+    int rc = cwo_oracle_fft2d(my, mx, U, -1);
+    if (!rc) rc = cwo_oracle_fft2d(my, mx, Hh, -1);
+    if (!rc) {
+        for (size_t i = 0; i < mm; ++i) U[i] *= Hh[i];
+        rc = cwo_oracle_fft2d(my, mx, U, +1);                                                      /* Eq.(10) */
+    }
+    if (!rc) {
+        zc c = fresnel_coeff(g.p0x, g.p0y, lambda, z);
+        for (int j = 0; j < ny; ++j)
+            for (int i = 0; i < nx; ++i) {
+                double m1 = i - nx / 2, n1 = j - ny / 2;
+                double x1 = m1 * g.p1x + g.o1x, y1 = n1 * g.p1y + g.o1y;
+                zc cs = c * cis_cycles((x1 * x1 + y1 * y1) / (2.0 * lambda * z))
+                          * cis_cycles(-(g.o0x * x1 + g.o0y * y1) / (lambda * z))
+                          * cis_cycles(-0.5 * (sx * m1 * m1 + sy * n1 * n1));                      /* Eq.(11) */
+                u2[(size_t)j * nx + i] = cs * U[(size_t)j * mx + i];
+            }
+    }
+    free(U); free(Hh);
+    return rc;
+}
+
+/* ---- output conversions of Listings 1-3 ------------------------------------------------------- */
+
+/* "Scale", Eq.(21): I256 = (I - min I)/(max I - min I) * 255 (a constant field maps to 0, D-R18). */
+void cwo_oracle_scale255(size_t n, const double* in, double* out) {
+    double lo = in[0], hi = in[0];
+    for (size_t i = 1; i < n; ++i) { if (in[i] < lo) lo = in[i]; if (in[i] > hi) hi = in[i]; }
+    for (size_t i = 0; i < n; ++i) out[i] = (hi > lo) ? (in[i] - lo) / (hi - lo) * 255.0 : 0.0;
+}
+
+/* CGH from point light sources, Eq.(23) P:L327-332:
+ *   I(x, y) = sum_j A_j cos( (2 pi/lambda) ((x - x_j)^2 + (y - y_j)^2)/(2 z_j) ),
+ * (x, y) = ((i - nx/2) px, (j - ny/2) py) on the hologram (Eq.(4)). */
+void cwo_oracle_pls_cgh(int ny, int nx, double px, double py, double lambda, int npts,
+                        const double* xs, const double* ys, const double* zs, const double* amps, double* out) {
+    #pragma omp parallel for num_threads(g_threads) schedule(static)
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            double x = (i - nx / 2) * px, y = (j - ny / 2) * py, acc = 0.0;
+            for (int k = 0; k < npts; ++k) {
+                double dx = x - xs[k], dy = y - ys[k];
+                double c = (dx * dx + dy * dy) / (2.0 * lambda * zs[k]);     /* cycles */
+                acc += amps[k] * cos(TWO_PI * (c - floor(c)));
+            }
+            out[(size_t)j * nx + i] = acc;
+        }
 }
 
 /* ---- Rayleigh-Sommerfeld I quadrature (Goodman, ref [1] P:L765) -- sanity only -- */

@@ -66,6 +66,12 @@ def lib():
     L.cwo_oracle_fresnel_points.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _I, _i32, _i32, _c128]
     L.cwo_oracle_fresnel_direct.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_fresnel_conv.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_fresnel_general_direct.argtypes = [_I, _I, _f64, _D, _D, _c128, _c128]
+    L.cwo_oracle_fresnel_general_points.argtypes = [_I, _I, _f64, _D, _D, _c128, _I, _i32, _i32, _c128]
+    L.cwo_oracle_fresnel_fourier.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
+    L.cwo_oracle_fresnel_shifted.argtypes = [_I, _I, _f64, _D, _D, _c128, _c128]
+    L.cwo_oracle_scale255.argtypes = [ctypes.c_size_t, _f64, _f64]
+    L.cwo_oracle_pls_cgh.argtypes = [_I, _I, _D, _D, _D, _I, _f64, _f64, _f64, _f64, _f64]
     L.cwo_oracle_rs_direct.argtypes = [_I, _I, _D, _D, _D, _D, _c128, _c128]
     L.cwo_oracle_gs_init.argtypes = [_I, _I, _I, _D, _D, _D, _D, _f64, _f64, _c128]
     L.cwo_oracle_gs_iter.argtypes = [_I, _I, _I, _D, _D, _D, _D, _f64, _f64, _c128, ctypes.c_void_p]
@@ -198,6 +204,60 @@ def fresnel_points(u1, px, py, lam, z, ms, ns):
     ms = np.ascontiguousarray(ms, np.int32); ns = np.ascontiguousarray(ns, np.int32)
     out = np.empty(ms.size, np.complex128)
     lib().cwo_oracle_fresnel_points(ny, nx, px, py, lam, z, u1, ms.size, ms, ns, out)
+    return out
+
+
+def _geom(p0, p1, o0, o1):
+    """(p0x, p0y, p1x, p1y, o0x, o0y, o1x, o1y): pitches [m] and lateral offsets [m] of the source / destination plane."""
+    return np.array([p0[0], p0[1], p1[0], p1[1], o0[0], o0[1], o1[0], o1[1]], np.float64)
+
+
+def fresnel_general_direct(u1, p0, p1, lam, z, o0=(0.0, 0.0), o1=(0.0, 0.0)):
+    """Eq.(1) discretised between planes of pitch p0 / p1 = (px, py) and offsets o0 / o1 (direct O(N^4) sum)."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    lib().cwo_oracle_fresnel_general_direct(ny, nx, _geom(p0, p1, o0, o1), lam, z, u1, u2)
+    return u2
+
+
+def fresnel_general_points(u1, p0, p1, lam, z, ms, ns, o0=(0.0, 0.0), o1=(0.0, 0.0)):
+    """Direct-sum value of u2[ns[i], ms[i]] (array indices) of the same sum, for full-size spot checks."""
+    u1 = _z(u1)
+    ny, nx = u1.shape
+    ms = np.ascontiguousarray(ms, np.int32); ns = np.ascontiguousarray(ns, np.int32)
+    out = np.empty(ms.size, np.complex128)
+    lib().cwo_oracle_fresnel_general_points(ny, nx, _geom(p0, p1, o0, o1), lam, z, u1, ms.size, ms, ns, out)
+    return out
+
+
+def fresnel_fourier(u1, px, py, lam, z):
+    """Fresnel diffraction, Fourier form, Eq.(7)-(9) P:L137-158; destination pitch lam |z| / (N p)."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    _check(lib().cwo_oracle_fresnel_fourier(ny, nx, px, py, lam, z, u1, u2), "fresnel_fourier")
+    return u2
+
+
+def fresnel_shifted(u1, p0, p1, lam, z, o0=(0.0, 0.0), o1=(0.0, 0.0)):
+    """Shifted Fresnel diffraction, Eq.(10)-(14) P:L160-192."""
+    u1 = _z(u1); u2 = np.empty_like(u1)
+    ny, nx = u1.shape
+    _check(lib().cwo_oracle_fresnel_shifted(ny, nx, _geom(p0, p1, o0, o1), lam, z, u1, u2), "fresnel_shifted")
+    return u2
+
+
+def scale255(a):
+    """'Scale', Eq.(21) P:L258-262."""
+    a = _d(a); out = np.empty_like(a)
+    lib().cwo_oracle_scale255(a.size, a, out)
+    return out
+
+
+def pls_cgh(ny, nx, px, py, lam, xs, ys, zs, amps):
+    """CGH of point light sources, Eq.(23) P:L327-332."""
+    xs, ys, zs, amps = _d(xs), _d(ys), _d(zs), _d(amps)
+    out = np.empty((ny, nx), np.float64)
+    lib().cwo_oracle_pls_cgh(ny, nx, px, py, lam, xs.size, xs, ys, zs, amps, out)
     return out
 
 

@@ -13,7 +13,7 @@ mp.dps = 50
 
 
 def _m(v):
-    return mpf(v) if isinstance(v, str) else mpf(repr(v))
+    return mpf(v) if isinstance(v, str) else mpf(repr(float(v)))
 
 
 def asm_cycles(nx, ny, px, py, lam, z, k, l):
@@ -42,3 +42,20 @@ def gaussian_beam(lam, z, w0, x, y):
     zR = pi * w0 ** 2 / lam
     q = 1 + 1j * z / zR
     return complex(exp(2j * pi * (z / lam - floor(z / lam))) / q * exp(-(x * x + y * y) / (w0 ** 2 * q)))
+
+
+def fresnel_delta_xy(p0x, p0y, lam, z, dx, dy):
+    """Eq.(1) P:L102 on one source sample seen from a point (dx, dy) metres away laterally:
+    exp(i 2 pi z/lambda)/(i lambda z) p0x p0y exp(i pi (dx^2 + dy^2)/(lambda z))."""
+    p0x, p0y, lam, z, dx, dy = _m(p0x), _m(p0y), _m(lam), _m(z), _m(dx), _m(dy)
+    c = exp(2j * pi * (z / lam - floor(z / lam))) / (1j * lam * z) * p0x * p0y
+    ph = (dx * dx + dy * dy) / (2 * lam * z)
+    return complex(c * exp(2j * pi * (ph - floor(ph))))
+
+
+def pls_term(lam, zj, dx, dy):
+    """One term of Eq.(23) P:L327-332 with A_j = 1: cos((2 pi/lambda) (dx^2 + dy^2)/(2 zj))."""
+    from mpmath import cos
+    lam, zj, dx, dy = _m(lam), _m(zj), _m(dx), _m(dy)
+    ph = (dx * dx + dy * dy) / (2 * lam * zj)
+    return float(cos(2 * pi * (ph - floor(ph))))
