@@ -12,7 +12,7 @@
  *   Ownership  The caller owns every buffer, including the workspace.  A plan owns only small
  *              lookup tables (a few MiB at most); ALL of them are allocated, built and synchronised
  *              inside cwo_plan().  No other call allocates, frees or synchronises anything.
- *   Asynchrony cwo_asm / cwo_fresnel_conv / cwo_propagate_stack / cwo_gs only ENQUEUE kernels on the
+ *   Asynchrony cwo_asm / cwo_fresnel_* / cwo_propagate_stack / cwo_gs only ENQUEUE kernels on the
  *              plan's stream and return (they may be captured into a CUDA graph); results are valid
  *              once the caller has synchronised that stream.  No host<->device copies.  Host arrays
  *              (zs) are read before return.
@@ -23,7 +23,7 @@
  *              global state; use one plan per host thread at a time, on the device it was made on.
  *   Sizes      Nx, Ny powers of two.  cwo_asm / cwo_propagate_stack: 32..16384 per axis.
  *              cwo_fresnel_conv (transforms of 2Nx x 2Ny): 16..8192 per axis.  cwo_gs: the
- *              range of its propagator.
+ *              range of its propagator.  cwo_fresnel_fourier / cwo_fresnel_shifted: 256..8192 per axis.
  *   Sign       z < 0 is back-propagation for both methods.
  *   FFT        forward kernel exp(-i 2 pi jk/n), inverse exp(+i 2 pi jk/n) scaled 1/(Mx*My)
  *              (the paper is silent; with this choice cwo_asm at z = 0 is the identity).
@@ -50,7 +50,8 @@ enum {
     CWO_ENOMEM = -5         /* host or device allocation failed in cwo_plan() */
 };
 
-enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4 };
+enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4, CWO_OP_FRESNEL_FOURIER = 5,
+       CWO_OP_FRESNEL_SHIFTED = 6 };
 
 enum {
     CWO_OPT_GS_METHOD = 1,  /* value: CWO_GS_FRESNEL (default; BASELINE config 5) or CWO_GS_ASM
@@ -92,6 +93,10 @@ int cwo_plan_set_option(cwo_plan_t plan, int key, int value);
  * Default (0, 0): on-axis, band-limited only. */
 int cwo_plan_set_offset(cwo_plan_t plan, double ox, double oy);
 
+/* Sampling pitch of the DESTINATION plane for cwo_fresnel_shifted (Eq.(14): p_x1, p_y1) [m].
+ * (0, 0) (the default) = the source pitch.  Both zero or both positive. */
+int cwo_plan_set_dst_pitch_xy(cwo_plan_t plan, double p1x, double p1y);
+
 /* Workspace a call needs, in bytes (n = number of planes for CWO_OP_STACK, ignored otherwise):
  *   ASM      8*Nx*Ny            the row-transformed field in column-tile order; needed for u2 != u1 too, because
  *                               the inverse row pass cannot write row-major rows over the column-tiled data it reads
@@ -101,6 +106,7 @@ int cwo_plan_set_offset(cwo_plan_t plan, double ox, double oy);
  *                               spectrum + the planes in flight between their column and row pass + the planes'
  *                               phase tables; cwo_propagate_stack accepts anything >= 16*Nx*Ny + the tables and
  *                               batches as many planes as fit
+ *   FRESNEL_FOURIER, FRESNEL_SHIFTED   16*Nx*Ny
  *   GS       24*Nx*Ny (Fresnel) / 16*Nx*Ny (ASM)
  * Returns 0 for an unknown op. */
 size_t cwo_plan_workspace_bytes(cwo_plan_t plan, int op, int n);
@@ -119,6 +125,22 @@ int cwo_asm(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
  * h_F(m,n) = exp(i pi ((m px)^2 + (n py)^2)/(lambda z)) sampled at taps -N..N-1 per axis; i.e. the
  * exact linear convolution of u1 with the sampled impulse response.  z == 0 -> CWO_EINVAL. */
 int cwo_fresnel_conv(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
+
+/* Fresnel diffraction, Fourier form, Eq.(7)-(9): one transform instead of three,
+ *   u2[m2,n2] = exp(i 2 pi z/lambda)/(i lambda z) px py exp(i pi (x2^2 + y2^2)/(lambda z))
+ *               sum_{m1,n1} u1[m1,n1] exp(i pi (x1^2 + y1^2)/(lambda z)) exp(-i 2 pi (x1 x2 + y1 y2)/(lambda z)),
+ * sample j of an axis at m = j - N/2 (Eq.(4)), x1 = m1 px, x2 = m2 p2x on the DESTINATION PITCH
+ * p2x = lambda |z| / (Nx px), p2y = lambda |z| / (Ny py) (P:L158 is garbled; this is the pitch at which the kernel is the
+ * DFT kernel).  z < 0: the kernel's sign flips (unnormalised inverse DFT).  z == 0 -> CWO_EINVAL. */
+int cwo_fresnel_fourier(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
+
+/* Shifted Fresnel diffraction, Eq.(10)-(14): Eq.(1) between a source plane of pitch (px, py) and a
+ * destination plane of pitch (p1x, p1y) (cwo_plan_set_dst_pitch_xy) whose window is displaced by (ox, oy) metres
+ * (cwo_plan_set_offset):
+ *   u2[m1,n1] = exp(i 2 pi z/lambda)/(i lambda z) px py sum_{m0,n0} u1[m0,n0] exp(i pi ((x1-x0)^2 + (y1-y0)^2)/(lambda z)),
+ *   x0 = m0 px, x1 = m1 p1x + ox (m = j - N/2), evaluated as the scaled convolution of Eq.(10) with the chirps of
+ * Eq.(11)-(13).  With the default destination pitch and offset it equals cwo_fresnel_conv.  z == 0 -> CWO_EINVAL. */
+int cwo_fresnel_shifted(cwo_plan_t plan, const cwo_c64* u1, cwo_c64* u2, double z);
 
 /* 3-D diffraction as a stack of 2-D diffractions (Diffract3D): out[k] = cwo_asm(u1, zs[k]),
  * k = 0..n-1, the forward FFT of u1 computed once.  zs: HOST array of n doubles.  out: device,

@@ -6,6 +6,8 @@ streams.  There is no CPU fallback: if libcwo.so cannot be loaded this module ra
     plan = cwo_plan(Nx, Ny, pitch, lam)
     cwo_asm(plan, u1, u2, z)                     # u1, u2: torch.complex64 CUDA tensors [Ny, Nx]
     cwo_fresnel_conv(plan, u1, u2, z)
+    cwo_fresnel_fourier(plan, u1, u2, z)         # destination pitch lam |z| / (N pitch)
+    cwo_fresnel_shifted(plan, u1, u2, z)         # destination pitch / offset: plan.set_dst_pitch_xy, plan.set_offset
     cwo_propagate_stack(plan, u1, zs, out)       # out: [n, Ny, Nx]
     cwo_gs(plan, amp_src, amp_dst, z, iters, phase)   # phase: float32 in/out
 """
@@ -21,7 +23,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("CWO_LIBRARY_PATH") or os.path.join(_HERE, "libcwo.so")
 
 CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA, CWO_ENOMEM = 0, -1, -2, -3, -4, -5
-CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS = 1, 2, 3, 4
+CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS, CWO_OP_FRESNEL_FOURIER, CWO_OP_FRESNEL_SHIFTED = 1, 2, 3, 4, 5, 6
 CWO_OPT_GS_METHOD = 1
 CWO_OPT_PIPELINE = 3
 CWO_OPT_ASM_PAD2X = 5
@@ -31,8 +33,9 @@ CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 
 # include/cwo.h (the product boundary) and include/cwo_debug.h (measurement hooks of the harness)
 EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",
-           "cwo_plan_set_offset", "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_asm", "cwo_fresnel_conv",
-           "cwo_propagate_stack", "cwo_gs", "cwo_strerror", "cwo_last_cuda_error"]
+           "cwo_plan_set_offset", "cwo_plan_set_dst_pitch_xy", "cwo_plan_workspace_bytes", "cwo_plan_set_workspace",
+           "cwo_asm", "cwo_fresnel_conv", "cwo_fresnel_fourier", "cwo_fresnel_shifted", "cwo_propagate_stack", "cwo_gs",
+           "cwo_strerror", "cwo_last_cuda_error"]
 DEBUG_EXPORTS = ["cwo_debug_set_timing", "cwo_debug_timings", "cwo_debug_launch_count", "cwo_debug_set_fresnel_2d"]
 
 _lib = None
@@ -63,11 +66,14 @@ def lib() -> ctypes.CDLL:
     L.cwo_plan_set_pitch_xy.argtypes = [vp, D, D]
     L.cwo_plan_set_option.argtypes = [vp, I, I]
     L.cwo_plan_set_offset.argtypes = [vp, D, D]
+    L.cwo_plan_set_dst_pitch_xy.argtypes = [vp, D, D]
     L.cwo_plan_workspace_bytes.argtypes = [vp, I, I]
     L.cwo_plan_workspace_bytes.restype = sz
     L.cwo_plan_set_workspace.argtypes = [vp, vp, sz]
     L.cwo_asm.argtypes = [vp, vp, vp, D]
     L.cwo_fresnel_conv.argtypes = [vp, vp, vp, D]
+    L.cwo_fresnel_fourier.argtypes = [vp, vp, vp, D]
+    L.cwo_fresnel_shifted.argtypes = [vp, vp, vp, D]
     L.cwo_propagate_stack.argtypes = [vp, vp, ctypes.POINTER(D), I, vp]
     L.cwo_gs.argtypes = [vp, vp, vp, D, I, vp]
     L.cwo_strerror.argtypes = [I]
@@ -108,6 +114,9 @@ class Plan:
 
     def set_offset(self, ox: float, oy: float) -> None:
         self._check(lib().cwo_plan_set_offset(self._h, float(ox), float(oy)), "cwo_plan_set_offset")
+
+    def set_dst_pitch_xy(self, p1x: float, p1y: float) -> None:
+        self._check(lib().cwo_plan_set_dst_pitch_xy(self._h, float(p1x), float(p1y)), "cwo_plan_set_dst_pitch_xy")
 
     # include/cwo_debug.h: measurement hooks (harness only)
     def set_timing(self, on: bool) -> None:
@@ -188,6 +197,20 @@ def cwo_fresnel_conv(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -
     a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.complex64, s, "u2")
     plan.ensure_workspace(CWO_OP_FRESNEL); plan.bind_stream()
     plan._check(lib().cwo_fresnel_conv(plan._h, a, b, float(z)), "cwo_fresnel_conv")
+
+
+def cwo_fresnel_fourier(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
+    s = (plan.Ny, plan.Nx)
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.complex64, s, "u2")
+    plan.ensure_workspace(CWO_OP_FRESNEL_FOURIER); plan.bind_stream()
+    plan._check(lib().cwo_fresnel_fourier(plan._h, a, b, float(z)), "cwo_fresnel_fourier")
+
+
+def cwo_fresnel_shifted(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
+    s = (plan.Ny, plan.Nx)
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.complex64, s, "u2")
+    plan.ensure_workspace(CWO_OP_FRESNEL_SHIFTED); plan.bind_stream()
+    plan._check(lib().cwo_fresnel_shifted(plan._h, a, b, float(z)), "cwo_fresnel_shifted")
 
 
 def cwo_propagate_stack(plan: Plan, u1: torch.Tensor, zs: Sequence[float], out: torch.Tensor) -> None:

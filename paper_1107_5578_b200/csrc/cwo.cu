@@ -20,7 +20,9 @@ struct cwo_plan_s {
     int Nx, Ny, lognx, logny;
     int device;                     // the device the plan's tables live on
     double px, py, lambda;
-    double off_x, off_y;            // shifted angular spectrum method: destination offset [m] (Eq.(19))
+    double off_x, off_y;            // shifted ASM / shifted Fresnel: destination offset [m] (Eq.(19), Eq.(14))
+    double p1x, p1y;                // shifted Fresnel: destination pitch [m] (0: same as the source pitch)
+    float2* quad[2][2];             // [axis][pre, post] chirp / ramp tables of the Fourier-form and shifted Fresnel
     cudaStream_t stream;
     void* ws;
     size_t ws_bytes;
@@ -63,10 +65,13 @@ static const pass_launcher_t kLaunchers[MAX_LOGN + 1] = {
     nullptr, nullptr, nullptr, nullptr, nullptr,
     launch_pass_5, launch_pass_6, launch_pass_7, launch_pass_8, launch_pass_9,
     launch_pass_10, launch_pass_11, launch_pass_12, launch_pass_13, launch_pass_14};
+static const linefft_launcher_t kLineFft[MAX_LOGN + 1] = {
+    nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
+    launch_linefft_8, launch_linefft_9, launch_linefft_10, launch_linefft_11, launch_linefft_12, launch_linefft_13, nullptr};
 static const conv_launcher_t kConv[MAX_LOGN + 1] = {
     nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr,
     launch_conv_8, launch_conv_9, launch_conv_10, launch_conv_11, launch_conv_12, launch_conv_13, nullptr};
-enum { KIND_CONV = 5, KIND_TRANSPOSE = 6 };
+enum { KIND_CONV = 5, KIND_TRANSPOSE = 6, KIND_LINEFFT = 7 };
 
 // One kernel launch `f` (returns cudaError_t), counted, and bracketed by an event pair in timing mode.
 template <class F>
@@ -128,6 +133,8 @@ static int plan_alloc_and_build(cwo_plan_t p) {
         }
         CWO_CUDA(p, cudaMalloc(&p->chirp_scratch, sizeof(double2) * 2 * ((size_t)mx + my)));
     }
+    for (int a = 0; a < 2; ++a)
+        for (int k = 0; k < 2; ++k) CWO_CUDA(p, cudaMalloc(&p->quad[a][k], sizeof(float2) * (a == 0 ? p->Nx : p->Ny)));
     CWO_CUDA(p, cudaMalloc(&p->tile_counter, 2 * sizeof(int)));
     CWO_CUDA(p, cudaMemsetAsync(p->tile_counter, 0, 2 * sizeof(int), 0));
     CWO_CUDA(p, cudaMalloc(&p->asm_tab, sizeof(float) * (size_t)(pad_ok ? 2 : 1) * (p->Nx + p->Ny)));
@@ -168,6 +175,7 @@ extern "C" int cwo_plan_destroy(cwo_plan_t p) {
     if (!p) return CWO_EINVAL;
     for (int i = 0; i < MAX_LOGN + 2; ++i) { cudaFree(p->tw[i]); cudaFree(p->tw64[i]); }
     for (int s = 0; s < 2; ++s) for (int a = 0; a < 2; ++a) { cudaFree(p->chirp[s][a]); cudaFree(p->chirp_pairs[s][a]); }
+    for (int a = 0; a < 2; ++a) for (int k = 0; k < 2; ++k) cudaFree(p->quad[a][k]);
     cudaFree(p->chirp_scratch);
     cudaFree(p->asm_tab);
     cudaFree(p->tile_counter);
@@ -192,6 +200,13 @@ extern "C" int cwo_plan_set_pitch_xy(cwo_plan_t p, double px, double py) {
 extern "C" int cwo_plan_set_offset(cwo_plan_t p, double ox, double oy) {
     if (!p || !isfinite(ox) || !isfinite(oy)) return CWO_EINVAL;
     p->off_x = ox; p->off_y = oy;
+    return CWO_OK;
+}
+
+extern "C" int cwo_plan_set_dst_pitch_xy(cwo_plan_t p, double p1x, double p1y) {
+    if (!p || !(p1x >= 0.0) || !(p1y >= 0.0) || !isfinite(p1x) || !isfinite(p1y) || ((p1x == 0.0) != (p1y == 0.0)))
+        return CWO_EINVAL;
+    p->p1x = p1x; p->p1y = p1y;
     return CWO_OK;
 }
 
@@ -235,7 +250,7 @@ extern "C" size_t cwo_plan_workspace_bytes(cwo_plan_t p, int op, int n) {
     const size_t f = sizeof(float2) * (size_t)p->Nx * p->Ny;
     switch (op) {
         case CWO_OP_ASM: return p->asm_pad2x ? 2 * f : f;
-        case CWO_OP_FRESNEL: return 2 * f;
+        case CWO_OP_FRESNEL: case CWO_OP_FRESNEL_FOURIER: case CWO_OP_FRESNEL_SHIFTED: return 2 * f;
         case CWO_OP_STACK: {   // spectrum + the planes in flight (up to 16 per batch of launches, minimum 1) + tables
             const int nn = n < 1 ? 1 : n;
             const int nb = nn > STACK_BATCH ? STACK_BATCH : nn;
@@ -420,7 +435,9 @@ static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, 
 }
 
 // Fresnel: Cx, Cy for distance z into table set `set` (coefficient of Eq.(1) and 1/(MxMy) folded in).
-static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int set) {
+static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int set, double p1x = 0.0, double p1y = 0.0) {
+    // shifted Fresnel (Eq.(13)): h = exp(i pi S m^2), S = p0 p1/(lambda z); p1 = p0 is the convolution form
+    if (p1x == 0.0) { p1x = p->px; p1y = p->py; }
     // c = exp(i 2 pi z/lambda)/(i lambda z) * px py / (Mx My), split as cx = c/sqrt|c|, cy = sqrt|c|
     const double kz = z / p->lambda, fr = kz - floor(kz);
     const double cr = cos(2.0 * M_PI * fr), ci = sin(2.0 * M_PI * fr);
@@ -432,11 +449,11 @@ static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int s
     ChirpAxis ax, ay;
     ax.out = p->chirp[set][0]; ax.out_pairs = p->chirp_pairs[set][0];
     ax.scratch = p->chirp_scratch; ax.tw64 = p->tw64[g.logmx]; ax.logm = g.logmx;
-    ax.a_cycles = p->px * p->px / (2.0 * p->lambda * z);
+    ax.a_cycles = p->px * p1x / (2.0 * p->lambda * z);
     ax.coef = make_double2(c_re / rt, c_im / rt);
     ay.out = p->chirp[set][1]; ay.out_pairs = p->chirp_pairs[set][1];
     ay.scratch = p->chirp_scratch + 2 * (size_t)g.mx; ay.tw64 = p->tw64[g.logmy]; ay.logm = g.logmy;
-    ay.a_cycles = p->py * p->py / (2.0 * p->lambda * z);
+    ay.a_cycles = p->py * p1y / (2.0 * p->lambda * z);
     ay.coef = make_double2(rt, 0.0);
     CWO_CUDA(p, build_chirp_spectrum(ax, ay, p->stream));
     p->launches++;
@@ -601,6 +618,85 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
     }
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
     return run_passes(p, CWO_GS_FRESNEL, z, 0, false, false, io, (float2*)p->ws);
+}
+
+// ---- Fresnel diffraction on another destination grid: Fourier form (f2) and shifted Fresnel (f3) -------------------
+
+static int build_quad(cwo_plan_t p, const QuadTabBatch& b) {
+    CWO_CUDA(p, build_quad_phase_tables(b, 4, p->stream));
+    p->launches++;
+    return CWO_OK;
+}
+// coefficient of Eq.(1)/(9)/(11), exp(i 2 pi z/lambda)/(i lambda z) px py, as (phase in cycles, magnitude)
+static void fresnel_coef(cwo_plan_t p, double z, double* cycles, double* mag) {
+    const double kz = z / p->lambda;
+    *cycles = (kz - floor(kz)) - (z > 0 ? 0.25 : -0.25);        // 1/(i z) = -i/z
+    *mag = p->px * p->py / (p->lambda * fabs(z));
+}
+
+extern "C" int cwo_fresnel_fourier(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
+    if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_separable(p)) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
+    if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL_FOURIER, 0)) return CWO_EWORKSPACE;
+    // Eq.(8): pre = (-1)^j exp(i pi x1^2/(lambda z)); Eq.(9): post = (-1)^j exp(i pi x2^2/(lambda z)) [x c on the x axis],
+    // x2 = m lambda|z|/(N p) (reading R17)
+    double cc, cm; fresnel_coef(p, z, &cc, &cm);
+    const double lz = p->lambda * z;
+    const double p2x = p->lambda * fabs(z) / (p->Nx * p->px), p2y = p->lambda * fabs(z) / (p->Ny * p->py);
+    QuadTabBatch b;
+    b.t[0] = QuadTab{p->quad[0][0], p->Nx, 1, 0.0, 0.0, p->px * p->px / (2.0 * lz), 1.0};
+    b.t[1] = QuadTab{p->quad[0][1], p->Nx, 1, cc, 0.0, p2x * p2x / (2.0 * lz), cm};
+    b.t[2] = QuadTab{p->quad[1][0], p->Ny, 1, 0.0, 0.0, p->py * p->py / (2.0 * lz), 1.0};
+    b.t[3] = QuadTab{p->quad[1][1], p->Ny, 1, 0.0, 0.0, p2y * p2y / (2.0 * lz), 1.0};
+    int rc = build_quad(p, b);
+    if (rc != CWO_OK) return rc;
+    const size_t f = (size_t)p->Nx * p->Ny;
+    float2* w0 = (float2*)p->ws;
+    float2* w1 = w0 + f;
+    LineFftParams lp; memset(&lp, 0, sizeof(lp));
+    lp.in = (const float2*)u1; lp.out = w0; lp.pre = p->quad[0][0]; lp.post = p->quad[0][1];
+    lp.tw = p->tw[p->lognx]; lp.n_lines = p->Ny; lp.inverse = z < 0;
+    rc = launch_tagged(p, p->lognx * 16 + KIND_LINEFFT, [&] { return kLineFft[p->lognx](p->stream, lp); });   // rows: u1 -> w0
+    if (rc != CWO_OK) return rc;
+    if ((rc = transpose_c64(p, w0, w1, p->Ny, p->Nx)) != CWO_OK) return rc;
+    lp.in = w1; lp.out = w1; lp.pre = p->quad[1][0]; lp.post = p->quad[1][1];
+    lp.tw = p->tw[p->logny]; lp.n_lines = p->Nx;
+    rc = launch_tagged(p, p->logny * 16 + KIND_LINEFFT, [&] { return kLineFft[p->logny](p->stream, lp); });   // columns, in place
+    if (rc != CWO_OK) return rc;
+    return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);
+}
+
+extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
+    if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_separable(p)) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
+    if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL_SHIFTED, 0)) return CWO_EWORKSPACE;
+    const double p1x = p->p1x > 0.0 ? p->p1x : p->px, p1y = p->p1y > 0.0 ? p->p1y : p->py;
+    // spectra of h = exp(i pi S m^2) with the coefficient folded in (Eq.(13), Eq.(11))
+    int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0, p1x, p1y);
+    if (rc != CWO_OK) return rc;
+    // Eq.(12) and Eq.(11) with O0 = 0, O1 = (off_x, off_y) in metres (reading R16), in cycles:
+    //   pre(m0)  = m0^2 p0 (p0 - p1)/(2 lambda z) - m0 p0 O1/(lambda z)
+    //   post(m1) = m1^2 p1 (p1 - p0)/(2 lambda z) + m1 p1 O1/(lambda z) + O1^2/(2 lambda z)
+    const double lz = p->lambda * z;
+    QuadTabBatch b;
+    b.t[0] = QuadTab{p->quad[0][0], p->Nx, 0, 0.0, -p->px * p->off_x / lz, p->px * (p->px - p1x) / (2.0 * lz), 1.0};
+    b.t[1] = QuadTab{p->quad[0][1], p->Nx, 0, p->off_x * p->off_x / (2.0 * lz), p1x * p->off_x / lz, p1x * (p1x - p->px) / (2.0 * lz), 1.0};
+    b.t[2] = QuadTab{p->quad[1][0], p->Ny, 0, 0.0, -p->py * p->off_y / lz, p->py * (p->py - p1y) / (2.0 * lz), 1.0};
+    b.t[3] = QuadTab{p->quad[1][1], p->Ny, 0, p->off_y * p->off_y / (2.0 * lz), p1y * p->off_y / lz, p1y * (p1y - p->py) / (2.0 * lz), 1.0};
+    if ((rc = build_quad(p, b)) != CWO_OK) return rc;
+    const size_t f = (size_t)p->Nx * p->Ny;
+    float2* w0 = (float2*)p->ws;
+    float2* w1 = w0 + f;
+    ConvParams cp; memset(&cp, 0, sizeof(cp));
+    cp.in = (const float2*)u1; cp.out = w0; cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][0];
+    cp.pre = p->quad[0][0]; cp.post = p->quad[0][1];
+    if ((rc = conv_pass(p, 0, 4, cp)) != CWO_OK) return rc;
+    if ((rc = transpose_c64(p, w0, w1, p->Ny, p->Nx)) != CWO_OK) return rc;
+    memset(&cp, 0, sizeof(cp));
+    cp.in = w1; cp.out = w1; cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][1];
+    cp.pre = p->quad[1][0]; cp.post = p->quad[1][1];
+    if ((rc = conv_pass(p, 1, 4, cp)) != CWO_OK) return rc;
+    return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);
 }
 
 extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double* zs, int n, void* out) {

@@ -87,6 +87,8 @@ struct ConvParams {
     void* out;                 // [n_lines][N] complex, or float phase (variant 3); may alias `in`
     const float* mid_amp;      // variant 2: amplitude imposed between the two convolutions, [n_lines][N]
     const ulonglong2* tab[2];  // spectrum of the sampled chirp for convolution 0 / 1, planar pairs, N entries
+    const float2* pre;         // variant 4: factor on every input sample, N entries (Eq.(12))
+    const float2* post;        // variant 4: factor on every output sample, N entries (Eq.(11))
     const float2* tw;          // N-point forward twiddles
     const float2* tw2;         // 2N-point forward twiddles
     int n_lines;
@@ -95,7 +97,7 @@ struct ConvParams {
     int* counter;              // persistent form: {next tile, CTAs done}, zero between launches (self-resetting)
 };
 // variant: 0 complex -> conv -> complex; 1 amp, phase -> conv -> complex; 2 complex -> conv, GS constraint, conv -> complex;
-//          3 complex -> conv -> phase
+//          3 complex -> conv -> phase; 4 complex -> x pre -> conv -> x post -> complex (shifted Fresnel)
 typedef cudaError_t (*conv_launcher_t)(int variant, cudaStream_t s, const ConvParams& p);
 
 // one launcher per transform length, defined in pass_inst.cu compiled with -DCWO_LOGN=<k>
@@ -110,6 +112,19 @@ CWO_DECL_LAUNCH(10) CWO_DECL_LAUNCH(11) CWO_DECL_LAUNCH(12) CWO_DECL_LAUNCH(13) 
 CWO_DECL_LAUNCH(8) CWO_DECL_LAUNCH(9) CWO_DECL_LAUNCH(10) CWO_DECL_LAUNCH(11) CWO_DECL_LAUNCH(12) CWO_DECL_LAUNCH(13)
 #undef CWO_DECL_LAUNCH
 constexpr int MIN_PAIR_LOGN = 8, MAX_PAIR_LOGN = 13;
+
+// ---- line transforms of the Fourier-form Fresnel diffraction (linefft_kernel.cuh) ---------------------------
+// out[line][k] = post[k] * DFT_N(pre[j] * in[line][j])[k]  (inverse != 0: the unnormalised inverse kernel); may run in place
+struct LineFftParams {
+    const float2* in; float2* out;
+    const float2* pre; const float2* post;     // N entries each
+    const float2* tw;                          // N-point forward twiddles
+    int n_lines, inverse;
+};
+#define CWO_DECL_LAUNCH(k) cudaError_t launch_linefft_##k(cudaStream_t s, const LineFftParams& p);
+CWO_DECL_LAUNCH(8) CWO_DECL_LAUNCH(9) CWO_DECL_LAUNCH(10) CWO_DECL_LAUNCH(11) CWO_DECL_LAUNCH(12) CWO_DECL_LAUNCH(13)
+#undef CWO_DECL_LAUNCH
+typedef cudaError_t (*linefft_launcher_t)(cudaStream_t s, const LineFftParams& p);
 
 // tables.cu
 cudaError_t build_twiddles(float2* tw, int n, cudaStream_t s);                 // exp(-i 2 pi m/n), fp64 -> fp32
@@ -126,6 +141,10 @@ constexpr int ASM_PLANE_BATCH = 128;                      // planes per launch (
 struct AsmPlaneBatch { AsmPlane p[ASM_PLANE_BATCH]; };
 cudaError_t build_asm_phase_tables(float* tab, float* resc, const AsmPlaneBatch& planes, int n_planes, int mx, int my,
                                    cudaStream_t s);    // resc (may be null): z/lambda of every plane
+// t[i] = scale (-1)^(alt i) exp(i 2 pi (c0 + c1 m + c2 m^2)), m = i - n/2, i < n; up to 4 tables per launch
+struct QuadTab { float2* out; int n; int alt; double c0, c1, c2, scale; };
+struct QuadTabBatch { QuadTab t[4]; };
+cudaError_t build_quad_phase_tables(const QuadTabBatch& b, int n_tabs, cudaStream_t s);
 // out[c][r] = in[r][c] (transpose.cu); rows, cols multiples of 32
 cudaError_t launch_transpose_c64(const float2* in, float2* out, int rows, int cols, cudaStream_t s);
 cudaError_t launch_transpose_f32(const float* in, float* out, int rows, int cols, cudaStream_t s);

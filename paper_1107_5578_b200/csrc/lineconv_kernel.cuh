@@ -29,7 +29,7 @@
 
 namespace cwo {
 
-enum ConvIn { CONV_IN_COMPLEX = 0, CONV_IN_AMP_PHASE = 1 };
+enum ConvIn { CONV_IN_COMPLEX = 0, CONV_IN_AMP_PHASE = 1, CONV_IN_COMPLEX_PRE = 2 };   // _PRE: x pre[n] on load, x post[n] on store
 enum ConvOut { CONV_OUT_COMPLEX = 0, CONV_OUT_PHASE = 1 };
 
 // x C, then swap re <-> im (opens the inverse transform)
@@ -67,7 +67,8 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
     using K = ConvCfg<LOGN>;
     static_assert(C::PAIR && LOGN >= 8, "lane-pair tiles");
     constexpr int W = C::W, Q = C::Q, N = C::N, H = W / 2;        // H lines per tile
-    constexpr bool PF = K::PREFETCH && IN == CONV_IN_COMPLEX;
+    constexpr bool PF = K::PREFETCH && IN != CONV_IN_AMP_PHASE;
+    constexpr bool PREPOST = IN == CONV_IN_COMPLEX_PRE;
     extern __shared__ float2 sm[];
     unsigned char* raw = reinterpret_cast<unsigned char*>(sm);
     uint64_t* bars = reinterpret_cast<uint64_t*>(raw + K::BAR_OFF);      // [0], [1]: SyncSplit; [2]: tile landed
@@ -137,6 +138,10 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
 #pragma unroll
             for (int e = 0; e < 16; ++e) x[e] = __ldcs(&P.in[base + e * Q]);   // streamed: keep L1 for the tables
         }
+        if constexpr (PREPOST) {                             // Eq.(12): the chirp and ramp factors of the source plane
+#pragma unroll
+            for (int e = 0; e < 16; ++e) x[e] = cmul(x[e], __ldg(&P.pre[us + e * Q]));
+        }
 
 #pragma unroll 1
         for (int c = 0; c < NCONV; ++c) {
@@ -179,6 +184,10 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
             }
         }
 
+        if constexpr (PREPOST) {                             // Eq.(11): C_S of the destination plane
+#pragma unroll
+            for (int e = 0; e < 16; ++e) x[e] = cmul(x[e], __ldg(&P.post[us + e * Q]));
+        }
         if constexpr (OUT == CONV_OUT_COMPLEX) {
             float2* out = reinterpret_cast<float2*>(P.out);
 #pragma unroll
@@ -237,7 +246,8 @@ static cudaError_t launch_lineconv_inst(cudaStream_t s, const ConvParams& p) {
 }
 
 // variant: 0 plain (complex -> conv -> complex), 1 GS first (amp, phase -> conv -> complex),
-//          2 GS middle (complex -> conv, constraint, conv -> complex), 3 GS last (complex -> conv -> phase)
+//          2 GS middle (complex -> conv, constraint, conv -> complex), 3 GS last (complex -> conv -> phase),
+//          4 shifted Fresnel (complex -> x pre -> conv -> x post -> complex)
 template <int LOGN>
 static cudaError_t launch_lineconv_impl(int variant, cudaStream_t s, const ConvParams& p) {
     switch (variant) {
@@ -245,6 +255,7 @@ static cudaError_t launch_lineconv_impl(int variant, cudaStream_t s, const ConvP
         case 1: return launch_lineconv_inst<LOGN, CONV_IN_AMP_PHASE, 1, CONV_OUT_COMPLEX>(s, p);
         case 2: return launch_lineconv_inst<LOGN, CONV_IN_COMPLEX, 2, CONV_OUT_COMPLEX>(s, p);
         case 3: return launch_lineconv_inst<LOGN, CONV_IN_COMPLEX, 1, CONV_OUT_PHASE>(s, p);
+        case 4: return launch_lineconv_inst<LOGN, CONV_IN_COMPLEX_PRE, 1, CONV_OUT_COMPLEX>(s, p);
     }
     return cudaErrorInvalidValue;
 }

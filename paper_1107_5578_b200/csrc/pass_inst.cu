@@ -4,6 +4,7 @@
 #include "cluster_kernel.cuh"
 #include "prefetch_kernel.cuh"
 #include "lineconv_kernel.cuh"
+#include "linefft_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"
@@ -19,6 +20,9 @@ cudaError_t CWO_CAT(launch_pass_, CWO_LOGN)(int kind, int pad, int mid, int n_ti
 #if CWO_LOGN >= 8 && CWO_LOGN <= 13
 cudaError_t CWO_CAT(launch_conv_, CWO_LOGN)(int variant, cudaStream_t s, const ConvParams& p) {
     return launch_lineconv_impl<CWO_LOGN>(variant, s, p);
+}
+cudaError_t CWO_CAT(launch_linefft_, CWO_LOGN)(cudaStream_t s, const LineFftParams& p) {
+    return launch_linefft_impl<CWO_LOGN>(s, p);
 }
 #endif
 }  // namespace cwo

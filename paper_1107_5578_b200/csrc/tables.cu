@@ -113,4 +113,27 @@ cudaError_t build_asm_phase_tables(float* tab, float* resc, const AsmPlaneBatch&
     return cudaLaunchKernelEx(&cfg, asm_phase_kernel, tab, resc, planes, mx, my);
 }
 
+// Quadratic-phase tables of the Fourier-form and shifted Fresnel diffraction (Eq.(8)-(9), Eq.(11)-(12)):
+// t[i] = scale (-1)^(alt i) exp(i 2 pi (c0 + c1 m + c2 m^2)), m = i - n/2 (Eq.(4)); the phase is formed and reduced mod 1
+// in fp64 (c2 m^2 reaches 1e4 cycles), then rounded once to fp32.
+__global__ void quad_phase_kernel(const __grid_constant__ QuadTabBatch b) {
+    const QuadTab& t = b.t[blockIdx.y];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < t.n; i += gridDim.x * blockDim.x) {
+        const double m = (double)(i - t.n / 2);
+        double c = t.c0 + (t.c1 + t.c2 * m) * m;
+        c -= rint(c);
+        double sn, cs;
+        sincospi(2.0 * c, &sn, &cs);
+        const double sc = (t.alt && (i & 1)) ? -t.scale : t.scale;
+        t.out[i] = make_float2((float)(sc * cs), (float)(sc * sn));
+    }
+}
+
+cudaError_t build_quad_phase_tables(const QuadTabBatch& b, int n_tabs, cudaStream_t s) {
+    int nmax = 1;
+    for (int i = 0; i < n_tabs; ++i) nmax = b.t[i].n > nmax ? b.t[i].n : nmax;
+    quad_phase_kernel<<<dim3((nmax + 255) / 256, n_tabs), 256, 0, s>>>(b);
+    return cudaGetLastError();
+}
+
 }  // namespace cwo
