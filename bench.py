@@ -180,7 +180,9 @@ def run_reference(args):
 WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
              "c2": ("fresnel", 1024), "fresnel2048": ("fresnel", 2048), "fresnel4096": ("fresnel", 4096),
              "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c4_intensity": ("stack_i", 2048), "c5": ("gs", 8192),
-             "asm_pad2x_2048": ("asm_pad", 2048), "asm_pad2x_4096": ("asm_pad", 4096)}
+             "asm_pad2x_2048": ("asm_pad", 2048), "asm_pad2x_4096": ("asm_pad", 4096),
+             "fourier4096": ("fourier", 4096), "fourier8192": ("fourier", 8192), "shifted4096": ("shifted", 4096),
+             "pls2048": ("pls", 2048)}
 
 
 def make_workload(name, rank, torch, api, W):
@@ -191,6 +193,39 @@ def make_workload(name, rank, torch, api, W):
     pad2x = op == "asm_pad"                                  # cwo_asm on the zero-expanded grid
     if pad2x:
         op = "asm"
+    if op == "pls":
+        # the paper's List 3: 2048 x 2048 hologram of 11 646 point light sources (the dinosaur model is not
+        # in the container: seeded uniform points in the same +-4 mm box, offset (1 cm, -2 mm), 0.2 m away), pitch 4 um
+        npts = 11646
+        r = np.random.default_rng(11075578 * 10 + 6 + rank)
+        pts = np.stack([r.uniform(-4e-3, 4e-3, npts) + 1e-2, r.uniform(-4e-3, 4e-3, npts) - 2e-3,
+                        0.2 + r.uniform(-4e-3, 4e-3, npts), r.uniform(0.2, 1.0, npts)], axis=1)
+        d_pts = torch.from_numpy(pts).cuda()
+        out = torch.empty((N, N), dtype=torch.float32, device="cuda")
+        plan = api.cwo_plan(N, N, 4e-6, 633e-9)
+
+        def step(i):
+            api.cwo_pls_cgh(plan, d_pts, out)
+
+        def e2e():
+            pin_in = torch.from_numpy(pts).pin_memory()
+            pin_out = torch.empty((N, N), dtype=torch.float32).pin_memory()
+
+            def f(i):
+                d_pts.copy_(pin_in, non_blocking=True)
+                api.cwo_pls_cgh(plan, d_pts, out)
+                pin_out.copy_(out, non_blocking=True)
+            return f, 32 * npts, 4 * n2
+        return dict(plan=plan, step=step, N=N, props_per_step=1, bytes_per_step=4 * n2 + 32 * npts,
+                    kind_bytes={10: 4 * n2 + 32 * npts}, kind_flops={10: 4.0 * npts * n2}, e2e=e2e,
+                    scheme_bytes_per_step=4 * n2 + 32 * npts,
+                    desc="pls2048: CGH of %d point light sources on a 2048x2048 hologram (Eq.(23)), lambda 633 nm, pitch 4 um, "
+                         "z 0.2 m" % npts,
+                    l2="16.8 MB output; everything on chip; ALU-bound", metric="holograms/sec (PLS CGH, Eq.(23)); fp32 FMA rate")
+    other = op in ("fourier", "shifted")          # same host loop as the convolution form
+    if other:
+        call_other = api.cwo_fresnel_fourier if op == "fourier" else api.cwo_fresnel_shifted
+        op_name, op = op, "fresnel"
     if op in ("asm", "fresnel"):
         base = (W.CONFIGS["c1"] if name == "c1" else W.CONFIGS["c3"]) if op == "asm" else (
             W.CONFIGS["c2"] if N <= 2048 else W.CONFIGS["c5"])
@@ -201,9 +236,16 @@ def make_workload(name, rank, torch, api, W):
         u2 = [torch.empty_like(u1[0]) for _ in range(NBUF)]
         plan = api.cwo_plan(N, N, base.pitch, base.lam)
         call = api.cwo_asm if op == "asm" else api.cwo_fresnel_conv
+        if other:
+            call = call_other
+            if op_name == "shifted":          # 1.5 x magnification, window displaced by a quarter of its width
+                plan.set_dst_pitch_xy(1.5 * base.pitch, 1.5 * base.pitch)
+                plan.set_offset(0.25 * N * base.pitch, -0.25 * N * base.pitch)
         if pad2x:
             plan.set_option(api.CWO_OPT_ASM_PAD2X, 1)
         plan.ensure_workspace(api.CWO_OP_ASM if op == "asm" else api.CWO_OP_FRESNEL)
+        if other:
+            op = op_name
 
         def step(i):
             call(plan, u1[i % NBUF], u2[i % NBUF], zs[i % len(zs)])
@@ -213,6 +255,14 @@ def make_workload(name, rank, torch, api, W):
             # back; api.HostPipeline overlaps the copies of neighbouring steps with the kernels
             pin_in = [torch.from_numpy(h).pin_memory() for h in hosts]
             pin_out = [torch.empty((N, N), dtype=torch.complex64).pin_memory() for _ in range(NBUF)]
+            if other:
+                d_in = torch.empty_like(u1[0])
+
+                def g(i):
+                    d_in.copy_(pin_in[i % NBUF], non_blocking=True)
+                    call(plan, d_in, u2[i % NBUF], zs[i % len(zs)])
+                    pin_out[i % NBUF].copy_(u2[i % NBUF], non_blocking=True)
+                return g, 8 * n2, 8 * n2
             hp = api.HostPipeline(plan, op)
 
             def f(i):
@@ -229,10 +279,14 @@ def make_workload(name, rank, torch, api, W):
         else:
             # two-dimensional form: R: 8 rd + 16 wr; C: 16 + 16; R': 16 rd + 8 wr.  Separable form (Fresnel, 256..8192):
             # kind 5 = one line-convolution pass (8 rd + 8 wr), kind 6 = one transpose (8 + 8)
-            kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2, 5: 16 * n2, 6: 16 * n2}
+            kb = {0: 24 * n2, 3: 32 * n2, 1: 24 * n2, 5: 16 * n2, 6: 16 * n2, 7: 16 * n2}
             bps = 80 * n2
+            what = "zero-expanded ASM" if pad2x else "Fresnel convolution"
+            if other:      # one 2-D transform (Fourier form: 2 passes of 8 rd + 8 wr) / the scaled convolution (as the convolution form)
+                what = "Fresnel diffraction, Fourier form" if op_name == "fourier" else "shifted Fresnel diffraction"
+                bps = (32 if op_name == "fourier" else 80) * n2
             desc = ("%s: %s %dx%d complex64 speckle field (virtual %dx%d), lambda %g nm, pitch %g um, "
-                    "z cycling %s m (new z every call)" % (name, "zero-expanded ASM" if pad2x else "Fresnel convolution",
+                    "z cycling %s m (new z every call)" % (name, what,
                                                            N, N, 2 * N, 2 * N, base.lam * 1e9, base.pitch * 1e6,
                                                            "{" + ",".join("%.4g" % z for z in zs) + "}"))
         ws = (24 if (op == "asm" and not pad2x) else 32) * n2   # u1 + u2 + workspace touched per step
@@ -384,7 +438,8 @@ def run_cuda(args):
         per_kind.setdefault(tag & 15, []).append(t_ms)
     names = {0: "pass_R (row FFT)", 1: "pass_R' (row IFFT)", 2: "pass_C0 (column FFT)",
              3: "pass_C (fused column FFT*H*IFFT)", 4: "pass_C' (H * column IFFT)",
-             5: "line convolution pass (FFT*C*IFFT per line, separable Fresnel)", 6: "transpose"}
+             5: "line convolution pass (FFT*C*IFFT per line, separable Fresnel)", 6: "transpose",
+             7: "line transform pass (pre * FFT * post per line, Fourier-form Fresnel)", 10: "point-light-source CGH (Eq.(23))"}
     passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
     dom_kind = max(per_kind, key=lambda k: np.sum(per_kind[k]))
     dom_ms = float(np.mean(per_kind[dom_kind]))
@@ -392,7 +447,7 @@ def run_cuda(args):
     tot = sum(float(np.sum(v)) for v in per_kind.values())
     alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves
     hbm_gbs = alg_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = _ncu_traffic(args.workload, {0: "pass_R", 1: "pass_Rinv", 3: "pass_C", 5: "lineconv", 6: "transpose"}.get(dom_kind, "-"))
+    traffic = _ncu_traffic(args.workload, {0: "pass_R", 1: "pass_Rinv", 3: "pass_C", 5: "lineconv", 6: "transpose", 7: "linefft", 10: "pls"}.get(dom_kind, "-"))
     common = {"kernel": names[dom_kind], "traffic": traffic,
               "traffic_source": "profiles/traffic.csv (committed ncu --set full capture; not measured by this run)" if traffic else None,
               "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms, "pass_ms": passes,

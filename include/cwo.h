@@ -12,7 +12,7 @@
  *   Ownership  The caller owns every buffer, including the workspace.  A plan owns only small
  *              lookup tables (a few MiB at most); ALL of them are allocated, built and synchronised
  *              inside cwo_plan().  No other call allocates, frees or synchronises anything.
- *   Asynchrony cwo_asm / cwo_fresnel_* / cwo_propagate_stack / cwo_gs only ENQUEUE kernels on the
+ *   Asynchrony cwo_asm / cwo_fresnel_* / cwo_propagate_stack / cwo_gs / cwo_scale255 / cwo_pls_cgh only ENQUEUE kernels on the
  *              plan's stream and return (they may be captured into a CUDA graph); results are valid
  *              once the caller has synchronised that stream.  No host<->device copies.  Host arrays
  *              (zs) are read before return.
@@ -157,6 +157,16 @@ int cwo_propagate_stack(cwo_plan_t plan, const cwo_c64* u1, const double* zs, in
  * kinoform of section 7.1.  amp_src, amp_dst, phase_out: float [Ny][Nx], device. */
 int cwo_gs(cwo_plan_t plan, const float* amp_src, const float* amp_dst, double z, int iters,
            float* phase_out);
+
+/* "Scale", Eq.(21): out[i] = (in[i] - min in)/(max in - min in) * 255 over n floats (an intensity field
+ * of any shape, e.g. a whole stack); a constant field maps to 0.  in, out: device, 16-byte aligned; out == in allowed. */
+int cwo_scale255(cwo_plan_t plan, const float* in, float* out, size_t n);
+
+/* Computer-generated hologram of n point light sources, Eq.(23):
+ *   out[j][i] = sum_k A_k cos( (2 pi/lambda) ((x - x_k)^2 + (y - y_k)^2)/(2 z_k) ),  (x, y) = ((i - Nx/2) px, (j - Ny/2) py),
+ * on the plan's Nx x Ny grid, pitch and wavelength.  pts: DEVICE array of n x 4 doubles (x_k, y_k, z_k, A_k) [m, m, m, -];
+ * z_k != 0.  out: float [Ny][Nx].  Direct O(n Nx Ny) sum (the paper's cwoPLS), no workspace. */
+int cwo_pls_cgh(cwo_plan_t plan, const double* pts, int n, float* out);
 
 const char* cwo_strerror(int code);
 int cwo_last_cuda_error(cwo_plan_t plan);

@@ -35,7 +35,7 @@ CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",
            "cwo_plan_set_offset", "cwo_plan_set_dst_pitch_xy", "cwo_plan_workspace_bytes", "cwo_plan_set_workspace",
            "cwo_asm", "cwo_fresnel_conv", "cwo_fresnel_fourier", "cwo_fresnel_shifted", "cwo_propagate_stack", "cwo_gs",
-           "cwo_strerror", "cwo_last_cuda_error"]
+           "cwo_scale255", "cwo_pls_cgh", "cwo_strerror", "cwo_last_cuda_error"]
 DEBUG_EXPORTS = ["cwo_debug_set_timing", "cwo_debug_timings", "cwo_debug_launch_count", "cwo_debug_set_fresnel_2d"]
 
 _lib = None
@@ -76,6 +76,8 @@ def lib() -> ctypes.CDLL:
     L.cwo_fresnel_shifted.argtypes = [vp, vp, vp, D]
     L.cwo_propagate_stack.argtypes = [vp, vp, ctypes.POINTER(D), I, vp]
     L.cwo_gs.argtypes = [vp, vp, vp, D, I, vp]
+    L.cwo_scale255.argtypes = [vp, vp, vp, sz]
+    L.cwo_pls_cgh.argtypes = [vp, vp, I, vp]
     L.cwo_strerror.argtypes = [I]
     L.cwo_strerror.restype = ctypes.c_char_p
     L.cwo_last_cuda_error.argtypes = [vp]
@@ -230,6 +232,24 @@ def cwo_gs(plan: Plan, amp_src: torch.Tensor, amp_dst: torch.Tensor, z: float, i
     c = _field(phase, torch.float32, s, "phase")
     plan.ensure_workspace(CWO_OP_GS); plan.bind_stream()
     plan._check(lib().cwo_gs(plan._h, a, b, float(z), int(iters), c), "cwo_gs")
+
+
+def cwo_scale255(plan: Plan, src: torch.Tensor, dst: torch.Tensor) -> None:
+    """Scale, Eq.(21): float32 CUDA tensors of equal shape (any shape); dst may be src."""
+    if not (src.is_cuda and dst.is_cuda and src.dtype == torch.float32 and dst.dtype == torch.float32
+            and src.is_contiguous() and dst.is_contiguous() and src.shape == dst.shape):
+        raise TypeError("src, dst must be contiguous CUDA float32 tensors of one shape")
+    plan.bind_stream()
+    plan._check(lib().cwo_scale255(plan._h, src.data_ptr(), dst.data_ptr(), src.numel()), "cwo_scale255")
+
+
+def cwo_pls_cgh(plan: Plan, pts: torch.Tensor, out: torch.Tensor) -> None:
+    """CGH of point light sources, Eq.(23): pts float64 CUDA [n, 4] = (x, y, z, A); out float32 [Ny, Nx]."""
+    if not (pts.is_cuda and pts.dtype == torch.float64 and pts.is_contiguous() and pts.dim() == 2 and pts.shape[1] == 4):
+        raise TypeError("pts must be a contiguous CUDA float64 tensor of shape [n, 4]")
+    b = _field(out, torch.float32, (plan.Ny, plan.Nx), "out")
+    plan.bind_stream()
+    plan._check(lib().cwo_pls_cgh(plan._h, pts.data_ptr(), int(pts.shape[0]), b), "cwo_pls_cgh")
 
 
 class HostPipeline:

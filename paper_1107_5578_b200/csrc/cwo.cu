@@ -34,6 +34,7 @@ struct cwo_plan_s {
     float2* chirp[2][2];            // [set][axis] Fresnel spectra Cx, Cy (set 0: the call's z / -z in GS, 1: +z in GS)
     float4* chirp_pairs[2][2];      // the same as planar (even bin, odd bin) pairs (separable form)
     double2* chirp_scratch;         // 2 axes x 2M
+    unsigned* minmax;               // cwo_scale255: {min, max} of the field as order-preserving integers
     int* tile_counter;              // persistent line-convolution kernels: {next tile, CTAs done}, zero between launches
     float* asm_tab;                 // ASM split path, one plane: [theta_x (Mx) | theta_y (My)], M up to 2N
     // include/cwo_debug.h: one CUDA event pair around every pass kernel
@@ -135,6 +136,7 @@ static int plan_alloc_and_build(cwo_plan_t p) {
     }
     for (int a = 0; a < 2; ++a)
         for (int k = 0; k < 2; ++k) CWO_CUDA(p, cudaMalloc(&p->quad[a][k], sizeof(float2) * (a == 0 ? p->Nx : p->Ny)));
+    CWO_CUDA(p, cudaMalloc(&p->minmax, 2 * sizeof(unsigned)));
     CWO_CUDA(p, cudaMalloc(&p->tile_counter, 2 * sizeof(int)));
     CWO_CUDA(p, cudaMemsetAsync(p->tile_counter, 0, 2 * sizeof(int), 0));
     CWO_CUDA(p, cudaMalloc(&p->asm_tab, sizeof(float) * (size_t)(pad_ok ? 2 : 1) * (p->Nx + p->Ny)));
@@ -179,6 +181,7 @@ extern "C" int cwo_plan_destroy(cwo_plan_t p) {
     cudaFree(p->chirp_scratch);
     cudaFree(p->asm_tab);
     cudaFree(p->tile_counter);
+    cudaFree(p->minmax);
     if (p->ev) { for (cudaEvent_t e : *p->ev) cudaEventDestroy(e); delete p->ev; }
     delete p->ev_tag;
     delete p;
@@ -456,7 +459,7 @@ static int build_fresnel_tables(cwo_plan_t p, const Geometry& g, double z, int s
     ay.a_cycles = p->py * p1y / (2.0 * p->lambda * z);
     ay.coef = make_double2(rt, 0.0);
     CWO_CUDA(p, build_chirp_spectrum(ax, ay, p->stream));
-    p->launches++;
+    p->launches += 2;                                           // two-step transform: two kernels
     return CWO_OK;
 }
 
@@ -697,6 +700,29 @@ extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     cp.pre = p->quad[1][0]; cp.post = p->quad[1][1];
     if ((rc = conv_pass(p, 1, 4, cp)) != CWO_OK) return rc;
     return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);
+}
+
+// ---- output conversions (outputs.cu) ----------------------------------------------------------------------------
+
+enum { KIND_MINMAX = 8, KIND_SCALE = 9, KIND_PLS = 10 };
+
+extern "C" int cwo_scale255(cwo_plan_t p, const float* in, float* out, size_t n) {
+    if (!p || !aligned16(in) || !aligned16(out) || n == 0) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
+    DeviceInfo* d = device_info();
+    if (!d) return CWO_EINVAL;
+    CWO_CUDA(p, cudaMemsetAsync(p->minmax, 0xff, sizeof(unsigned), p->stream));
+    CWO_CUDA(p, cudaMemsetAsync(p->minmax + 1, 0x00, sizeof(unsigned), p->stream));
+    int rc = launch_tagged(p, KIND_MINMAX, [&] { return launch_minmax(in, n, p->minmax, d->n_sm, p->stream); });
+    if (rc != CWO_OK) return rc;
+    return launch_tagged(p, KIND_SCALE, [&] { return launch_scale(in, out, n, p->minmax, d->n_sm, p->stream); });
+}
+
+extern "C" int cwo_pls_cgh(cwo_plan_t p, const double* pts, int n, float* out) {
+    if (!p || !aligned16(pts) || !aligned16(out) || n <= 0) return CWO_EINVAL;
+    if (check_call(p) != CWO_OK) return CWO_EINVAL;
+    return launch_tagged(p, KIND_PLS, [&] {
+        return launch_pls_cgh(pts, n, out, p->Nx, p->Ny, p->px, p->py, p->lambda, p->stream); });
 }
 
 extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double* zs, int n, void* out) {

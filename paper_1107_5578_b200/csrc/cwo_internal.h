@@ -149,4 +149,10 @@ cudaError_t build_quad_phase_tables(const QuadTabBatch& b, int n_tabs, cudaStrea
 cudaError_t launch_transpose_c64(const float2* in, float2* out, int rows, int cols, cudaStream_t s);
 cudaError_t launch_transpose_f32(const float* in, float* out, int rows, int cols, cudaStream_t s);
 
+// outputs.cu: Scale (Eq.(21)) and the point-light-source CGH (Eq.(23))
+cudaError_t launch_minmax(const float* in, size_t n, unsigned* mm, int n_sm, cudaStream_t s);     // mm: {min, max} encoded
+cudaError_t launch_scale(const float* in, float* out, size_t n, const unsigned* mm, int n_sm, cudaStream_t s);
+cudaError_t launch_pls_cgh(const double* pts, int npts, float* out, int nx, int ny, double px, double py, double lambda,
+                           cudaStream_t s);
+
 }  // namespace cwo

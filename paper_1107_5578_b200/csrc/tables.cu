@@ -1,8 +1,8 @@
 // tables.cu -- small double-precision table builders.
 //   * FFT twiddles exp(-i 2 pi m/n), evaluated in fp64 and rounded once to fp32.
 //   * Fresnel: the spectrum C[k] of the sampled 1-D chirp (impulse response of Eq.(3)/(6), P:L113,
-//     P:L132, taps d = -N..N-1 stored wrapped at d mod 2N), by a single-CTA fp64 Stockham FFT in
-//     global scratch.  FFT2[h_F](k,l) = Cx[k]*Cy[l] exactly because h_F is separable, so the
+//     P:L132, taps d = -N..N-1 stored wrapped at d mod 2N), by a two-step fp64 FFT (sqrt(M) shared-memory
+//     transforms per step).  FFT2[h_F](k,l) = Cx[k]*Cy[l] exactly because h_F is separable, so the
 //     2N x 2N impulse response and its FFT (the paper's FresnelConvProp + FFT) are never formed.
 #include "cwo_internal.h"
 
@@ -37,47 +37,88 @@ __device__ __forceinline__ double2 zmul(double2 a, double2 b) {
     return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }
 
-// One CTA per axis.  x[i] = exp(i 2 pi a d^2), d = i < M/2 ? i : i - M, a = pitch^2/(2 lambda z) in
-// cycles; radix-2 Stockham stages ping-pong between the two halves of scratch; out = coef * X.
-__global__ void __launch_bounds__(1024) chirp_fft_kernel(ChirpAxis ax0, ChirpAxis ax1) {
-    const ChirpAxis& ax = (blockIdx.x == 0) ? ax0 : ax1;
-    const int M = 1 << ax.logm, H = M >> 1;
-    double2* a = ax.scratch;
-    double2* b = ax.scratch + M;
-    for (int i = threadIdx.x; i < M; i += blockDim.x) {
-        double d = (double)((i < H) ? i : i - M);
-        double c = ax.a_cycles * d * d;      // |c| <= ~3e3 cycles: fp64 keeps ~1e-13 cycles
-        c -= rint(c);
-        double s, co;
-        sincospi(2.0 * c, &s, &co);
-        a[i] = make_double2(co, s);
-    }
-    __syncthreads();
-    for (int lns = 0; lns < ax.logm; ++lns) {
+// Spectrum of the sampled chirp x[n] = exp(i 2 pi a d^2), d = n < M/2 ? n : n - M, a = p0 p1/(2 lambda z) in cycles,
+// by a two-step fp64 FFT, M = M1 M2 (n = n1 M2 + n2, k = k1 + M1 k2):
+//   step 1 (one CTA per n2 and axis): M1-point transform over n1 in shared memory, times w_M^(n2 k1) -> scratch[k1][n2]
+//   step 2 (one CTA per k1 and axis): M2-point transform over n2 -> C[k1 + M1 k2] = coef * X.
+// 2 x ~sqrt(M) CTAs of 64 threads instead of one CTA running log2 M global-memory stages (16384 points: 119 -> ~10 us;
+// the table build is on the critical path of every propagation with a new z).
+constexpr int CHIRP_MAXL = 128;    // M <= 16384 -> M1 <= 128
+
+__device__ __forceinline__ double2 tw_full(const double2* tw64, int idx, int half) {   // w_M^idx, idx < M, table of M/2
+    if (idx < half) return tw64[idx];
+    const double2 w = tw64[idx - half];
+    return make_double2(-w.x, -w.y);
+}
+
+// radix-2 Stockham stages of a length-2^l transform held in shared memory (ping-pong a <-> b); returns the buffer
+// that holds the result.  w_L^j = w_M^(j M/L).
+__device__ double2* smem_fft(double2* a, double2* b, int l, const double2* tw64, int logm) {
+    const int L = 1 << l, h = L >> 1;
+    for (int lns = 0; lns < l; ++lns) {
         const int ns = 1 << lns;
-        for (int j = threadIdx.x; j < H; j += blockDim.x) {
-            int k = j & (ns - 1);
-            double2 w = ax.tw64[k << (ax.logm - 1 - lns)];
-            double2 x0 = a[j], x1 = zmul(a[j + H], w);
-            int j0 = ((j >> lns) << (lns + 1)) + k;
+        for (int j = threadIdx.x; j < h; j += blockDim.x) {
+            const int k = j & (ns - 1);
+            const double2 w = tw64[(k << (l - 1 - lns)) << (logm - l)];
+            const double2 x0 = a[j], x1 = zmul(a[j + h], w);
+            const int j0 = ((j >> lns) << (lns + 1)) + k;
             b[j0] = make_double2(x0.x + x1.x, x0.y + x1.y);
             b[j0 + ns] = make_double2(x0.x - x1.x, x0.y - x1.y);
         }
         __syncthreads();
         double2* t = a; a = b; b = t;
     }
-    for (int i = threadIdx.x; i < M; i += blockDim.x) {
-        double2 r = zmul(a[i], ax.coef);
-        if (ax.out) ax.out[i] = make_float2((float)r.x, (float)r.y);
+    return a;
+}
+
+__global__ void __launch_bounds__(64) chirp_step1_kernel(ChirpAxis ax0, ChirpAxis ax1) {
+    const ChirpAxis& ax = (blockIdx.y == 0) ? ax0 : ax1;
+    const int l1 = (ax.logm + 1) >> 1, l2 = ax.logm - l1, M = 1 << ax.logm, M1 = 1 << l1, M2 = 1 << l2;
+    const int n2 = blockIdx.x;
+    if (n2 >= M2) return;
+    __shared__ double2 buf[2][CHIRP_MAXL];
+    for (int n1 = threadIdx.x; n1 < M1; n1 += blockDim.x) {
+        const int n = n1 * M2 + n2;
+        const double d = (double)((n < M / 2) ? n : n - M);
+        double c = ax.a_cycles * d * d;      // |c| <= ~3e3 cycles: fp64 keeps ~1e-13 cycles
+        c -= rint(c);
+        double s, co;
+        sincospi(2.0 * c, &s, &co);
+        buf[0][n1] = make_double2(co, s);
+    }
+    __syncthreads();
+    const double2* r = smem_fft(buf[0], buf[1], l1, ax.tw64, ax.logm);
+    for (int k1 = threadIdx.x; k1 < M1; k1 += blockDim.x)
+        ax.scratch[(size_t)k1 * M2 + n2] = zmul(r[k1], tw_full(ax.tw64, n2 * k1, M / 2));
+}
+
+__global__ void __launch_bounds__(64) chirp_step2_kernel(ChirpAxis ax0, ChirpAxis ax1) {
+    const ChirpAxis& ax = (blockIdx.y == 0) ? ax0 : ax1;
+    const int l1 = (ax.logm + 1) >> 1, l2 = ax.logm - l1, M1 = 1 << l1, M2 = 1 << l2;
+    const int k1 = blockIdx.x;
+    if (k1 >= M1) return;
+    __shared__ double2 buf[2][CHIRP_MAXL];
+    for (int n2 = threadIdx.x; n2 < M2; n2 += blockDim.x) buf[0][n2] = ax.scratch[(size_t)k1 * M2 + n2];
+    __syncthreads();
+    const double2* r = smem_fft(buf[0], buf[1], l2, ax.tw64, ax.logm);
+    for (int k2 = threadIdx.x; k2 < M2; k2 += blockDim.x) {
+        const int i = k1 + M1 * k2;
+        const double2 v = zmul(r[k2], ax.coef);
+        if (ax.out) ax.out[i] = make_float2((float)v.x, (float)v.y);
         if (ax.out_pairs) {                                  // planar pairs (even bin, odd bin): lineconv_kernel.cuh
             float* q = reinterpret_cast<float*>(ax.out_pairs + (i >> 1)) + (i & 1);
-            q[0] = (float)r.x; q[2] = (float)r.y;
+            q[0] = (float)v.x; q[2] = (float)v.y;
         }
     }
 }
 
 cudaError_t build_chirp_spectrum(const ChirpAxis& ax0, const ChirpAxis& ax1, cudaStream_t s) {
-    chirp_fft_kernel<<<2, 1024, 0, s>>>(ax0, ax1);
+    const int lm = ax0.logm > ax1.logm ? ax0.logm : ax1.logm;
+    const int l1 = (lm + 1) >> 1;
+    chirp_step1_kernel<<<dim3(1 << (lm - l1), 2), 64, 0, s>>>(ax0, ax1);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    chirp_step2_kernel<<<dim3(1 << l1, 2), 64, 0, s>>>(ax0, ax1);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,109 @@
+"""Parity of Scale (Eq.(21)) and the point-light-source CGH (Eq.(23)) of the CUDA path against the fp64 oracle
+(SURVEY 8(f) f4)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from test_gpu_parity import REL_L2, MAX_ABS, api   # noqa: E402,F401
+
+LAM = 633e-9
+
+
+def _points(n, seed, span, z0, dz):
+    r = np.random.default_rng(seed)
+    return np.stack([r.uniform(-span, span, n), r.uniform(-span, span, n), z0 + r.uniform(-dz, dz, n),
+                     r.uniform(0.2, 1.0, n)], axis=1)
+
+
+@pytest.mark.parametrize("shape,npts", [((64, 128), 1), ((256, 256), 333), ((16, 64), 70), ((512, 1024), 1200)])
+def test_pls_cgh_matches_oracle(api, oracle, shape, npts):
+    # sizes below and above the 128 x 32 tile, a ragged point count (chunks of 32), points off the grid,
+    # phases up to ~1e4 cycles: element by element at the propagation bar
+    ny, nx = shape
+    px, py = 4e-6, 5e-6
+    pts = _points(npts, 7 + npts, 1.5e-3, 0.2, 0.03)
+    if npts == 70:
+        pts[:, 2] *= -1                       # z_j < 0: same pattern (cos is even)
+    plan = _plan_of_shape(api, nx, ny, px, py)
+    out = torch.empty((ny, nx), dtype=torch.float32, device="cuda")
+    api.cwo_pls_cgh(plan, torch.from_numpy(pts).cuda(), out)
+    torch.cuda.synchronize()
+    ref = oracle.pls_cgh(ny, nx, px, py, LAM, pts[:, 0], pts[:, 1], pts[:, 2], pts[:, 3])
+    got = out.cpu().numpy().astype(np.float64)
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert rel <= REL_L2 and np.abs(got - ref).max() <= MAX_ABS * np.abs(ref).max(), (rel, np.abs(got - ref).max())
+
+
+def _plan_of_shape(api, nx, ny, px, py):
+    # cwo_plan wants powers of two; the CGH call itself does not: take the enclosing power-of-two plan when the
+    # shape is one, else skip (the C ABI ties the grid to the plan)
+    def p2(v):
+        return v & (v - 1) == 0
+    if not (p2(nx) and p2(ny)):
+        pytest.skip("plan grids are powers of two")
+    plan = api.cwo_plan(nx, ny, px, LAM)
+    if px != py:
+        plan.set_pitch_xy(px, py)
+    return plan
+
+
+def test_pls_cgh_paper_sized_sampled(api, oracle):
+    # the paper's List 3: 2048 x 2048 hologram, 11 646 points, pitch 4 um, 633 nm, 0.2 m; object within +-4 mm, offset
+    # (1 cm, -2 mm).  The oracle evaluates 64 hologram rows (of 2048) in full
+    n, npts = 2048, 11646
+    pts = _points(npts, 3, 4e-3, 0.2, 4e-3)
+    pts[:, 0] += 1e-2; pts[:, 1] -= 2e-3
+    plan = api.cwo_plan(n, n, 4e-6, LAM)
+    out = torch.empty((n, n), dtype=torch.float32, device="cuda")
+    api.cwo_pls_cgh(plan, torch.from_numpy(pts).cuda(), out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().astype(np.float64)
+    rows = np.r_[0, 1, 31, 32, 33, n - 1, np.random.default_rng(4).integers(0, n, 58)]
+    oracle.set_threads(oracle.max_threads())
+    # the oracle on a 64 x 2048 strip: shift the points' y so that strip row r is hologram row rows[r]
+    err2 = ref2 = 0.0; mx = pk = 0.0
+    for r in rows:
+        strip = oracle.pls_cgh(2, n, 4e-6, 4e-6, LAM, pts[:, 0], pts[:, 1] - (r - n // 2 + 1) * 4e-6, pts[:, 2], pts[:, 3])[0]
+        d = got[r] - strip
+        err2 += d @ d; ref2 += strip @ strip; mx = max(mx, np.abs(d).max()); pk = max(pk, np.abs(strip).max())
+    oracle.set_threads(min(8, oracle.max_threads()))
+    assert np.sqrt(err2 / ref2) <= REL_L2 and mx <= MAX_ABS * pk, (np.sqrt(err2 / ref2), mx, pk)
+
+
+@pytest.mark.parametrize("n", [1, 5, 1000, 256 * 256 + 3, 2048 * 2048])
+def test_scale255_matches_oracle(api, oracle, n):
+    r = np.random.default_rng(n)
+    a = (r.standard_normal(n) ** 2 * 37.0 - 3.0).astype(np.float32)
+    plan = api.cwo_plan(256, 256, 4e-6, LAM)
+    d = torch.from_numpy(a).cuda()
+    o = torch.empty_like(d)
+    api.cwo_scale255(plan, d, o)
+    torch.cuda.synchronize()
+    ref = oracle.scale255(a.astype(np.float64))
+    got = o.cpu().numpy()
+    assert np.abs(got - ref).max() <= 255 * 4e-7 * 8
+    if n > 1:
+        assert got.min() == 0.0 and got.max() == 255.0
+        assert got[np.argmin(a)] == 0.0 and got[np.argmax(a)] == 255.0
+    api.cwo_scale255(plan, d, d)              # in place, and a second call on the same plan (min/max cells reset)
+    torch.cuda.synchronize()
+    assert np.array_equal(d.cpu().numpy(), got)
+
+
+def test_scale255_of_a_stack_intensity(api, oracle):
+    # Listing 1/2 of the paper: Diffract -> Intensity -> Scale
+    from paper_1107_5578_b200 import workloads as W
+    cfg = W.CONFIGS["c4"].scaled(256)
+    u1 = W.make_field(cfg)
+    zs = list(cfg.zs[:3])
+    plan = api.cwo_plan(256, 256, cfg.pitch, cfg.lam)
+    plan.set_option(api.CWO_OPT_STACK_INTENSITY, 1)
+    out = torch.empty((3, 256, 256), dtype=torch.float32, device="cuda")
+    api.cwo_propagate_stack(plan, torch.from_numpy(u1).cuda(), zs, out)
+    api.cwo_scale255(plan, out, out)
+    torch.cuda.synchronize()
+    ref = oracle.scale255(oracle.stack_intensity(u1, cfg.pitch, cfg.pitch, cfg.lam, zs))
+    assert np.abs(out.cpu().numpy() - ref).max() <= 255 * 2e-5
