@@ -30,6 +30,12 @@ long long cwo_debug_launch_count(cwo_plan_t plan);
  * (256..8192 per axis); 0 (default): separable form where it exists.  Same result either way (comparison runs). */
 int cwo_debug_set_fresnel_2d(cwo_plan_t plan, int on);
 
+/* The separable Fresnel form (cwo_fresnel_conv, cwo_fresnel_shifted, cwo_gs) has two ways of switching axes: transpose
+ * passes between contiguous line passes, or line passes that gather their lines from the columns of their input.
+ * mode -1 (default): chosen by field size (gathering up to 2048 x 2048 samples, where the field stays in L2);
+ * 0: always transposing; 1: always gathering.  Same result either way (parity tests run both). */
+int cwo_debug_set_fresnel_gather(cwo_plan_t plan, int mode);
+
 #ifdef __cplusplus
 }
 #endif

@@ -36,7 +36,8 @@ EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_
            "cwo_plan_set_offset", "cwo_plan_set_dst_pitch_xy", "cwo_plan_workspace_bytes", "cwo_plan_set_workspace",
            "cwo_asm", "cwo_fresnel_conv", "cwo_fresnel_fourier", "cwo_fresnel_shifted", "cwo_propagate_stack", "cwo_gs",
            "cwo_scale255", "cwo_pls_cgh", "cwo_strerror", "cwo_last_cuda_error"]
-DEBUG_EXPORTS = ["cwo_debug_set_timing", "cwo_debug_timings", "cwo_debug_launch_count", "cwo_debug_set_fresnel_2d"]
+DEBUG_EXPORTS = ["cwo_debug_set_timing", "cwo_debug_timings", "cwo_debug_launch_count", "cwo_debug_set_fresnel_2d",
+                 "cwo_debug_set_fresnel_gather"]
 
 _lib = None
 
@@ -86,6 +87,7 @@ def lib() -> ctypes.CDLL:
     L.cwo_debug_timings.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(I), I]
     L.cwo_debug_set_timing.argtypes = [vp, I]
     L.cwo_debug_set_fresnel_2d.argtypes = [vp, I]
+    L.cwo_debug_set_fresnel_gather.argtypes = [vp, I]
     _lib = L
     return L
 
@@ -126,6 +128,9 @@ class Plan:
 
     def set_fresnel_2d(self, on: bool) -> None:
         self._check(lib().cwo_debug_set_fresnel_2d(self._h, int(bool(on))), "cwo_debug_set_fresnel_2d")
+
+    def set_fresnel_gather(self, mode: int) -> None:
+        self._check(lib().cwo_debug_set_fresnel_gather(self._h, int(mode)), "cwo_debug_set_fresnel_gather")
 
     def workspace_bytes(self, op: int, n: int = 0) -> int:
         return int(lib().cwo_plan_workspace_bytes(self._h, int(op), int(n)))

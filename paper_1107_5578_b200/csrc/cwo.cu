@@ -27,6 +27,7 @@ struct cwo_plan_s {
     void* ws;
     size_t ws_bytes;
     int gs_method, pipeline, asm_pad2x, stack_intensity, band_limit, fresnel_2d;
+    int fresnel_gather;             // include/cwo_debug.h: -1 auto (by field size), 0 transposing form, 1 gathering form
     int last_cuda_error;
     long long launches;
     float2* tw[MAX_LOGN + 2];       // fp32 twiddles per log2 length
@@ -161,6 +162,7 @@ extern "C" int cwo_plan(int Nx, int Ny, double pitch, double lambda, cwo_plan_t*
     p->px = p->py = pitch; p->lambda = lambda;
     p->gs_method = CWO_GS_FRESNEL;
     p->pipeline = 1;
+    p->fresnel_gather = -1;
     p->ev = new (std::nothrow) std::vector<cudaEvent_t>();
     p->ev_tag = new (std::nothrow) std::vector<int>();
     int rc = (p->ev && p->ev_tag) ? plan_alloc_and_build(p) : CWO_ENOMEM;
@@ -308,6 +310,12 @@ extern "C" long long cwo_debug_launch_count(cwo_plan_t p) { return p ? p->launch
 extern "C" int cwo_debug_set_fresnel_2d(cwo_plan_t p, int on) {
     if (!p || (on != 0 && on != 1)) return CWO_EINVAL;
     p->fresnel_2d = on;
+    return CWO_OK;
+}
+
+extern "C" int cwo_debug_set_fresnel_gather(cwo_plan_t p, int mode) {
+    if (!p || mode < -1 || mode > 1) return CWO_EINVAL;
+    p->fresnel_gather = mode;
     return CWO_OK;
 }
 
@@ -583,6 +591,13 @@ static bool fresnel_separable(cwo_plan_t p) {
     return !p->fresnel_2d && p->lognx >= MIN_PAIR_LOGN && p->lognx <= MAX_PAIR_LOGN && p->logny >= MIN_PAIR_LOGN &&
            p->logny <= MAX_PAIR_LOGN;
 }
+// Fields that stay in L2 (<= 32 MB) skip the transposes: every pass gathers its lines from the COLUMNS of its input
+// (lineconv_kernel.cuh GATHER) and writes them contiguously, i.e. in the transposed layout.  Measured: c2 42.3 -> 37.7 us,
+// 2048^2 110 -> 104 us; from HBM the 8-byte gathers cost more than the transposes they replace (4096^2: 384 -> 436 us,
+// 8192^2: 2043 -> 2946 us, c5 75.6 -> 94.2 ms), so larger fields keep the transposing form.
+static bool separable_gather(cwo_plan_t p) {
+    return p->fresnel_gather < 0 ? (size_t)p->Nx * p->Ny <= ((size_t)1 << 22) : p->fresnel_gather != 0;
+}
 // axis 0: convolve along x (lines = rows of a [Ny][Nx] field); axis 1: along y (lines = rows of the transposed field)
 static int conv_pass(cwo_plan_t p, int axis, int variant, ConvParams& cp) {
     const int logn = axis == 0 ? p->lognx : p->logny;
@@ -606,6 +621,19 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL, 0)) return CWO_EWORKSPACE;
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0);
     if (rc != CWO_OK) return rc;
+    if (fresnel_separable(p) && separable_gather(p)) {
+        // y first (lines = columns of u1, gathered; result in the transposed layout [Nx][Ny]), then x (lines = columns
+        // of that, gathered; result row-major [Ny][Nx])
+        float2* w0 = (float2*)p->ws;
+        ConvParams cp; memset(&cp, 0, sizeof(cp));
+        cp.in = (const float2*)u1; cp.gather = 1; cp.in_stride = p->Nx; cp.out = w0;
+        cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][1];
+        if ((rc = conv_pass(p, 1, 0, cp)) != CWO_OK) return rc;                     // columns: u1 -> w0 [Nx][Ny]
+        memset(&cp, 0, sizeof(cp));
+        cp.in = w0; cp.gather = 1; cp.in_stride = p->Ny; cp.out = u2;
+        cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][0];
+        return conv_pass(p, 0, 0, cp);                                               // rows: w0 -> u2 [Ny][Nx]
+    }
     if (fresnel_separable(p)) {
         const size_t f = (size_t)p->Nx * p->Ny;
         float2* w0 = (float2*)p->ws;
@@ -687,6 +715,17 @@ extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     b.t[2] = QuadTab{p->quad[1][0], p->Ny, 0, 0.0, -p->py * p->off_y / lz, p->py * (p->py - p1y) / (2.0 * lz), 1.0};
     b.t[3] = QuadTab{p->quad[1][1], p->Ny, 0, p->off_y * p->off_y / (2.0 * lz), p1y * p->off_y / lz, p1y * (p1y - p->py) / (2.0 * lz), 1.0};
     if ((rc = build_quad(p, b)) != CWO_OK) return rc;
+    if (separable_gather(p)) {
+        float2* w0 = (float2*)p->ws;
+        ConvParams cp; memset(&cp, 0, sizeof(cp));
+        cp.in = (const float2*)u1; cp.gather = 1; cp.in_stride = p->Nx; cp.out = w0;
+        cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][1]; cp.pre = p->quad[1][0]; cp.post = p->quad[1][1];
+        if ((rc = conv_pass(p, 1, 4, cp)) != CWO_OK) return rc;                     // y: u1 -> w0 [Nx][Ny]
+        memset(&cp, 0, sizeof(cp));
+        cp.in = w0; cp.gather = 1; cp.in_stride = p->Ny; cp.out = u2;
+        cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][0]; cp.pre = p->quad[0][0]; cp.post = p->quad[0][1];
+        return conv_pass(p, 0, 4, cp);                                               // x: w0 -> u2 [Ny][Nx]
+    }
     const size_t f = (size_t)p->Nx * p->Ny;
     float2* w0 = (float2*)p->ws;
     float2* w1 = w0 + f;
@@ -810,6 +849,22 @@ static int gs_fresnel_separable(cwo_plan_t p, const float* amp_src, const float*
     memset(&cp, 0, sizeof(cp));
     cp.in_amp = amp_dst; cp.in_phase = phase_out; cp.out = cur; cp.tab[0] = X[0];
     if ((rc = conv_pass(p, 0, 1, cp)) != CWO_OK) return rc;
+    if (separable_gather(p)) {
+        // every later pass gathers its lines from the columns of the previous pass' output: cur is [Ny][Nx] before an
+        // odd (y) pass and [Nx][Ny] before an even (x) pass
+        for (int m = 1; m <= 2 * iters; ++m) {
+            memset(&cp, 0, sizeof(cp));
+            cp.in = cur; cp.out = oth; cp.gather = 1;
+            if (m & 1) { cp.tab[0] = Y[0]; cp.tab[1] = Y[1]; cp.mid_amp = amp_src_t; cp.in_stride = p->Nx; }
+            else { cp.tab[0] = X[1]; cp.tab[1] = X[0]; cp.mid_amp = amp_dst; cp.in_stride = p->Ny; }
+            if ((rc = conv_pass(p, (m & 1) ? 1 : 0, 2, cp)) != CWO_OK) return rc;
+            float2* t = cur; cur = oth; oth = t;
+        }
+        memset(&cp, 0, sizeof(cp));
+        cp.in = cur; cp.out = oth; cp.tab[0] = Y[0]; cp.gather = 1; cp.in_stride = p->Nx;
+        if ((rc = conv_pass(p, 1, 3, cp)) != CWO_OK) return rc;
+        return transpose_f32(p, (const float*)oth, phase_out, p->Nx, p->Ny);
+    }
     if ((rc = transpose_c64(p, cur, oth, p->Ny, p->Nx)) != CWO_OK) return rc;
     { float2* t = cur; cur = oth; oth = t; }
     for (int m = 1; m <= 2 * iters; ++m) {

@@ -81,7 +81,9 @@ struct FuncOnce {
 
 // ---- separable Fresnel convolution (lineconv_kernel.cuh) ---------------------------------------------------
 struct ConvParams {
-    const float2* in;          // [n_lines][N] complex
+    const float2* in;          // [n_lines][N] complex; gather: sample n of line l at in[n * in_stride + l] (the lines are the
+                               // COLUMNS of a row-major [N][in_stride] field: no transpose between the two axes' passes)
+    int gather, in_stride;
     const float* in_amp;       // variant 1: amplitude and phase, [n_lines][N]
     const float* in_phase;
     void* out;                 // [n_lines][N] complex, or float phase (variant 3); may alias `in`

@@ -61,7 +61,17 @@ template <int LOGN> struct ConvCfg {
     static constexpr size_t SMEM = PREFETCH ? PF_OFF + PF_BYTES : PF_OFF;
 };
 
-template <int LOGN, int IN, int NCONV, int OUT>
+// 8-byte asynchronous copy global -> shared (LSU path; completion by cp.async.wait_group of the issuing thread)
+__device__ __forceinline__ void cp_async8(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+
+// GATHER: the lines are the columns of a row-major field (sample n of line l at in[n * in_stride + l]); the output is
+// always written as contiguous lines, i.e. in the transposed layout, which is what the other axis' pass gathers from:
+// the two axes alternate without any transpose pass.  The 32-byte sector a sample sits in also holds the samples of
+// the three neighbouring lines, which other CTAs request within a microsecond (tiles are handed out in order): HBM
+// still moves every sector once, L2 serves it four times.
+template <int LOGN, int IN, int NCONV, int OUT, bool GATHER>
 __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kernel(const __grid_constant__ ConvParams P) {
     using C = Tile<LOGN>;
     using K = ConvCfg<LOGN>;
@@ -92,10 +102,25 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
         for (uint32_t o = 0; o < K::PF_BYTES; o += 16384u)
             bulk_g2s(reinterpret_cast<unsigned char*>(pf) + o, src + o, 16384u, &bars[2]);
     };
-    if (PF && threadIdx.x == 0) fetch(blockIdx.x);
-    if (!K::PREFETCH && threadIdx.x == 0 && (int)blockIdx.x + P.pf_dist < P.n_tiles)
+    // gathered prefetch: every thread copies exactly the 16 samples it will read back (its own slots of pf: no barrier)
+    auto fetch_gather = [&](int tile) {
+        const float2* src = P.in + (size_t)us * P.in_stride + (tile * H + hl);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) cp_async8(&pf[hl * N + us + e * Q], src + (size_t)e * Q * P.in_stride);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    if (PF && !GATHER && threadIdx.x == 0) fetch(blockIdx.x);
+    if (PF && GATHER) fetch_gather(blockIdx.x);
+    if (!K::PREFETCH && !GATHER && threadIdx.x == 0 && (int)blockIdx.x + P.pf_dist < P.n_tiles)
         l2_prefetch(P.in + (size_t)(blockIdx.x + P.pf_dist) * H * N, (uint32_t)K::PF_BYTES);
+    // persistent gathered form: tile indices are known one tile ahead (the copies of tile i + 1 start as soon as the
+    // registers of tile i are loaded); cur/nxt are uniform over the CTA
+    int nxt = 0;
+    if (PF && GATHER) {
+        if (threadIdx.x == 0) *next_tile = (int)gridDim.x + atomicAdd(P.counter, 1);
+    }
     __syncthreads();
+    if (PF && GATHER) nxt = *next_tile;
 
     const SyncSplit sy{&bars[0], &bars[1], 0u, 0u};
     sy.consumed();                                          // the exchange region starts free
@@ -125,6 +150,11 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
 #pragma unroll
             for (int e = 0; e < 16; ++e) x[e] = mine[e * C::T];
             __syncthreads();
+        } else if constexpr (PF && GATHER) {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+            for (int e = 0; e < 16; ++e) x[e] = pf[hl * N + us + e * Q];
+            if (nxt < P.n_tiles) fetch_gather(nxt);          // own slots only: no barrier needed
         } else if constexpr (PF) {
             mbar_wait(&bars[2], it & 1);
 #pragma unroll
@@ -134,6 +164,10 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
                 *next_tile = nt;
                 if (nt < P.n_tiles) { fence_proxy_async(); fetch(nt); }
             }
+        } else if constexpr (GATHER) {
+            const float2* src = P.in + (size_t)us * P.in_stride + (tile * H + hl);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) x[e] = __ldg(src + (size_t)e * Q * P.in_stride);
         } else {
 #pragma unroll
             for (int e = 0; e < 16; ++e) x[e] = __ldcs(&P.in[base + e * Q]);   // streamed: keep L1 for the tables
@@ -207,6 +241,14 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
             __syncthreads();
         }
         if constexpr (!K::PREFETCH) break;                   // one CTA per tile
+        if constexpr (PF && GATHER) {
+            // nt (asked for at the top of this tile) becomes the tile after next
+            if (threadIdx.x == 0) *next_tile = nt;
+            __syncthreads();
+            tile = nxt; nxt = *next_tile;
+            __syncthreads();                                 // everybody has read it before thread 0 overwrites it
+            continue;
+        }
         if constexpr (!PF) { if (threadIdx.x == 0) *next_tile = nt; }
         __syncthreads();
         tile = *next_tile;
@@ -218,14 +260,14 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
     }
 }
 
-template <int LOGN, int IN, int NCONV, int OUT>
-static cudaError_t launch_lineconv_inst(cudaStream_t s, const ConvParams& p) {
+template <int LOGN, int IN, int NCONV, int OUT, bool GATHER>
+static cudaError_t launch_lineconv_gi(cudaStream_t s, const ConvParams& p) {
     using K = ConvCfg<LOGN>;
     DeviceInfo* d = device_info();
     if (!d) return cudaErrorInvalidDevice;
     static FuncOnce once;
     if (!once.done(d->index)) {
-        cudaError_t e = cudaFuncSetAttribute(lineconv_kernel<LOGN, IN, NCONV, OUT>,
+        cudaError_t e = cudaFuncSetAttribute(lineconv_kernel<LOGN, IN, NCONV, OUT, GATHER>,
                                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM);
         if (e != cudaSuccess) return e;
         once.set(d->index);
@@ -242,7 +284,14 @@ static cudaError_t launch_lineconv_inst(cudaStream_t s, const ConvParams& p) {
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, lineconv_kernel<LOGN, IN, NCONV, OUT>, q);
+    return cudaLaunchKernelEx(&cfg, lineconv_kernel<LOGN, IN, NCONV, OUT, GATHER>, q);
+}
+template <int LOGN, int IN, int NCONV, int OUT>
+static cudaError_t launch_lineconv_inst(cudaStream_t s, const ConvParams& p) {
+    if constexpr (IN != CONV_IN_AMP_PHASE) {
+        if (p.gather) return launch_lineconv_gi<LOGN, IN, NCONV, OUT, true>(s, p);
+    }
+    return launch_lineconv_gi<LOGN, IN, NCONV, OUT, false>(s, p);
 }
 
 // variant: 0 plain (complex -> conv -> complex), 1 GS first (amp, phase -> conv -> complex),

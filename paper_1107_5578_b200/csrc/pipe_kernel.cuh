@@ -214,7 +214,7 @@ template <int LOGN, int KIND> struct PipeCfg {
     static constexpr size_t SMEM_NOTAB = TAB_OFF, SMEM_TAB = TAB_OFF + TAB_BYTES;
     // row-major staging (ROW_FWD in, ROW_INV out): row r of the tile at element r * (points + ROWPAD)
     // (bank stagger between lane pairs)
-    static constexpr int ROWPAD = C::W > 2 ? 16 / C::W : 0;
+    static constexpr int ROWPAD = 16 / C::W;              // (W = 2: the packed row passes read rows r, r+1 from neighbouring threads)
 };
 
 // Pipelined passes exist for the tile shapes that matter for HBM-sized fields: 256 threads per tile,

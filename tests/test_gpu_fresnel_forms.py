@@ -121,3 +121,59 @@ def test_shifted_and_fourier_error_codes(api):
         assert e.value.code == api.CWO_EINVAL
     with pytest.raises(api.CwoError):
         plan.set_dst_pitch_xy(5e-6, 0.0)
+
+
+# ---- both ways of switching axes in the separable form (include/cwo_debug.h cwo_debug_set_fresnel_gather) ----------
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("shape", [(256, 256), (512, 2048), (2048, 1024), (8192, 256), (256, 8192), (4096, 1024)])
+def test_fresnel_conv_transposing_and_gathering_forms(api, oracle, mode, shape):
+    # the default picks one of the two by field size; here each is forced on every tile shape, incl. the persistent
+    # 8192-point kernel with its gathered prefetch, Nx != Ny, px != py, both signs of z, in place
+    from paper_1107_5578_b200 import workloads as W
+    cfg = W.CONFIGS["c5"]
+    ny, nx = shape
+    u1 = _rand(shape, 140 + ny % 17)
+    px, py = cfg.pitch, 1.3 * cfg.pitch
+    plan = api.cwo_plan(nx, ny, px, cfg.lam)
+    plan.set_pitch_xy(px, py)
+    plan.set_fresnel_gather(mode)
+    for z in (cfg.zs[0] * max(shape) / 8192, -0.11):
+        d1 = _dev(u1); d2 = torch.empty_like(d1)
+        api.cwo_fresnel_conv(plan, d1, d2, z)
+        api.cwo_fresnel_conv(plan, d1, d1, z)
+        torch.cuda.synchronize()
+        ref = oracle.fresnel_conv(u1, px, py, cfg.lam, z)
+        _assert_parity(d2.cpu().numpy(), ref, "fresnel mode %d %s z=%g" % (mode, shape, z))
+        _assert_parity(d1.cpu().numpy(), ref, "fresnel in place mode %d %s z=%g" % (mode, shape, z))
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_shifted_and_gs_in_both_forms(api, oracle, mode):
+    from paper_1107_5578_b200 import workloads as W
+    from test_gpu_parity import _phasor_rel_l2
+    # shifted Fresnel
+    u1 = _rand((1024, 512), 151)
+    p0, p1, off = (8e-6, 6e-6), (5e-6, 9e-6), (-310e-6, 170e-6)
+    plan = api.cwo_plan(512, 1024, p0[0], LAM)
+    plan.set_pitch_xy(*p0); plan.set_dst_pitch_xy(*p1); plan.set_offset(*off); plan.set_fresnel_gather(mode)
+    d1 = _dev(u1); d2 = torch.empty_like(d1)
+    api.cwo_fresnel_shifted(plan, d1, d2, 0.2)
+    torch.cuda.synchronize()
+    _assert_parity(d2.cpu().numpy(), oracle.fresnel_shifted(u1, p0, p1, LAM, 0.2, o1=off), "shifted mode %d" % mode)
+    # Gerchberg-Saxton, Fresnel propagator: kinoform and two loop passes from the oracle's state (non-square: the
+    # layouts [Ny][Nx] and [Nx][Ny] alternate)
+    cfg = W.CONFIGS["c5"]
+    shape = (512, 1024)
+    z = cfg.zs[0] * 1024 / 8192
+    amp_src, amp_dst, phi0 = W.gs_inputs(shape, 9)
+    plan = api.cwo_plan(shape[1], shape[0], cfg.pitch, cfg.lam)
+    plan.set_fresnel_gather(mode)
+    for iters in (0, 2):
+        ph = _dev(phi0.astype(np.float32))
+        api.cwo_gs(plan, _dev(amp_src), _dev(amp_dst), z, iters, ph)
+        torch.cuda.synchronize()
+        p = oracle.gs_init(0, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z)
+        for _ in range(iters):
+            p = oracle.gs_iter(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z)
+        assert _phasor_rel_l2(ph.cpu().numpy(), p) <= REL_L2 * (1 + 2 * iters), "gs mode %d iters %d" % (mode, iters)
