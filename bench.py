@@ -447,7 +447,7 @@ def run_cuda(args):
     tot = sum(float(np.sum(v)) for v in per_kind.values())
     alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves
     hbm_gbs = alg_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = _ncu_traffic(args.workload, {0: "pass_R", 1: "pass_Rinv", 3: "pass_C", 5: "lineconv", 6: "transpose", 7: "linefft", 10: "pls"}.get(dom_kind, "-"))
+    traffic = _ncu_traffic(args.workload, {0: "pass_R", 1: "pass_Rinv", 2: "pass_C0", 3: "pass_C", 4: "pass_Cmidinv", 5: "lineconv", 6: "transpose", 7: "linefft", 10: "pls"}.get(dom_kind, "-"))
     common = {"kernel": names[dom_kind], "traffic": traffic,
               "traffic_source": "profiles/traffic.csv (committed ncu --set full capture; not measured by this run)" if traffic else None,
               "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms, "pass_ms": passes,

@@ -82,10 +82,19 @@ constexpr int PLS_C = 4;       // columns per thread (PLS_T apart: coalesced sto
 constexpr int PLS_R = 16;      // rows per CTA
 constexpr int PLS_CHUNK = 32;  // points staged per step
 
-__device__ __forceinline__ float2 cis_frac(double c) {      // exp(i 2 pi c), c in cycles
-    c -= rint(c);                                            // [-0.5, 0.5]
+// exp(i 2 pi c), c in cycles.  The fraction is taken without conversion instructions (FRND / F2F / MUFU share the 16-lane
+// XU pipe, which would bound the kernel): adding 1.5 * 2^20 leaves frac(c) * 2^32 in the low word of the sum (|c| < 2^19),
+// an int32 in units of 2^-32 cycles; larger phases (never in the paper's geometry) take the rounding instruction.
+__device__ __forceinline__ float2 cis_frac(double c) {
+    int q;
+    if (fabs(c) < 524288.0) {
+        q = __double2loint(c + 1572864.0);
+    } else {
+        c -= rint(c);
+        q = (int)(long long)(c * 4294967296.0);
+    }
     float sn, cs;
-    __sincosf(6.283185307179586f * (float)c, &sn, &cs);
+    __sincosf((float)q * 1.4629180792671596e-9f, &sn, &cs);      // 2 pi / 2^32
     return make_float2(cs, sn);
 }
 
