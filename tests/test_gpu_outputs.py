@@ -107,3 +107,44 @@ def test_scale255_of_a_stack_intensity(api, oracle):
     torch.cuda.synchronize()
     ref = oracle.scale255(oracle.stack_intensity(u1, cfg.pitch, cfg.pitch, cfg.lam, zs))
     assert np.abs(out.cpu().numpy() - ref).max() <= 255 * 2e-5
+
+
+def test_new_calls_capture_into_a_cuda_graph_and_replay(api, oracle):
+    """cwo_fresnel_fourier, cwo_fresnel_shifted, cwo_pls_cgh and cwo_scale255 only enqueue (kernels and two memsets): a
+    sequence of them is captured into a CUDA graph and replayed on new data."""
+    from test_gpu_parity import _assert_parity, _dev, _rand
+    n, p, lam = 512, 8e-6, 532e-9
+    plan = api.cwo_plan(n, n, p, lam)
+    plan.set_dst_pitch_xy(5e-6, 11e-6); plan.set_offset(2e-4, -1e-4)
+    plan.ensure_workspace(api.CWO_OP_FRESNEL_SHIFTED)
+    a = torch.empty((n, n), dtype=torch.complex64, device="cuda")
+    b = torch.empty_like(a); c = torch.empty_like(a)
+    holo = torch.empty((n, n), dtype=torch.float32, device="cuda"); holo8 = torch.empty_like(holo)
+    pts = _points(50, 5, 1e-3, 0.2, 0.02)
+    d_pts = torch.from_numpy(pts).cuda()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        api.cwo_fresnel_fourier(plan, a, b, 0.1); api.cwo_fresnel_shifted(plan, a, c, 0.1)
+        api.cwo_pls_cgh(plan, d_pts, holo); api.cwo_scale255(plan, holo, holo8)
+        s.synchronize()
+        with torch.cuda.graph(g, stream=s):
+            api.cwo_fresnel_fourier(plan, a, b, 0.1)
+            api.cwo_fresnel_shifted(plan, a, c, -0.07)
+            api.cwo_pls_cgh(plan, d_pts, holo)
+            api.cwo_scale255(plan, holo, holo8)
+    for seed in (71, 72):
+        u1 = _rand((n, n), seed)
+        a.copy_(_dev(u1))
+        pts2 = _points(50, seed, 1e-3, 0.2, 0.02)
+        d_pts.copy_(torch.from_numpy(pts2).cuda())
+        g.replay()
+        torch.cuda.synchronize()
+        _assert_parity(b.cpu().numpy(), oracle.fresnel_fourier(u1, p, p, lam, 0.1), "graph: fourier")
+        _assert_parity(c.cpu().numpy(), oracle.fresnel_shifted(u1, (p, p), (5e-6, 11e-6), lam, -0.07, o1=(2e-4, -1e-4)),
+                       "graph: shifted")
+        ref = oracle.pls_cgh(n, n, p, p, lam, pts2[:, 0], pts2[:, 1], pts2[:, 2], pts2[:, 3])
+        got = holo.cpu().numpy().astype(np.float64)
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= REL_L2
+        assert np.abs(holo8.cpu().numpy() - oracle.scale255(got)).max() <= 255 * 4e-6
