@@ -327,7 +327,7 @@ def make_workload(name, rank, torch, api, W):
             return f, 8 * n2, (4 if inten else 8) * n2 * n
         per_plane = 28 if inten else 32      # C': 8 rd + 8 wr, R': 8 rd + 8 (4) wr
         return dict(plan=plan, step=step, N=N, props_per_step=n, bytes_per_step=32 * n2 + n * per_plane * n2,
-                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: 16 * 16 * n2, 1: 16 * (per_plane - 16) * n2}, kind_flops={},
+                    kind_bytes={0: 16 * n2, 2: 16 * n2, 4: min(n, 64) * 16 * n2, 1: min(n, 64) * (per_plane - 16) * n2}, kind_flops={},   # C' / R' launches cover up to 64 planes
                     scheme_bytes_per_step=32 * n2 + n * per_plane * n2, e2e=e2e,
                     desc="%s: depth stack, one 2048x2048 random-phase field to 64 planes z = 1..64 mm by ASM, lambda 633 nm, "
                          "pitch 6.4 um, out 64x2048x2048 %s" % (name, "float32 intensity" if inten else "complex64"),

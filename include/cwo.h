@@ -102,7 +102,7 @@ int cwo_plan_set_dst_pitch_xy(cwo_plan_t plan, double p1x, double p1y);
  *                               the inverse row pass cannot write row-major rows over the column-tiled data it reads
  *            (16*Nx*Ny with CWO_OPT_ASM_PAD2X)
  *   FRESNEL  16*Nx*Ny           two copies of the field (the 2Nx x 2Ny padded array is never stored)
- *   STACK    8*Nx*Ny*(1 + min(n, 16)) + 4*n*(Nx+Ny+1) rounded up to 256
+ *   STACK    8*Nx*Ny*(1 + min(n, 64)) + 4*n*(Nx+Ny+1) rounded up to 256
  *                               spectrum + the planes in flight between their column and row pass + the planes'
  *                               phase tables; cwo_propagate_stack accepts anything >= 16*Nx*Ny + the tables and
  *                               batches as many planes as fit

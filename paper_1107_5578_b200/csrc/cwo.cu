@@ -243,7 +243,7 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
     return CWO_EINVAL;
 }
 
-enum { STACK_BATCH = 16 };
+enum { STACK_BATCH = 64 };   // measured at c4: 16 planes per launch pair 1632 us, 32: 1579 us, 64: 1553 us
 
 static size_t align256(size_t v) { return (v + 255) & ~(size_t)255; }
 static size_t stack_table_bytes(cwo_plan_t p, int n) {      // per plane: theta_x, theta_y, z/lambda
@@ -256,7 +256,7 @@ extern "C" size_t cwo_plan_workspace_bytes(cwo_plan_t p, int op, int n) {
     switch (op) {
         case CWO_OP_ASM: return p->asm_pad2x ? 2 * f : f;
         case CWO_OP_FRESNEL: case CWO_OP_FRESNEL_FOURIER: case CWO_OP_FRESNEL_SHIFTED: return 2 * f;
-        case CWO_OP_STACK: {   // spectrum + the planes in flight (up to 16 per batch of launches, minimum 1) + tables
+        case CWO_OP_STACK: {   // spectrum + the planes in flight (up to 64 per batch of launches, minimum 1) + tables
             const int nn = n < 1 ? 1 : n;
             const int nb = nn > STACK_BATCH ? STACK_BATCH : nn;
             return (size_t)(1 + nb) * f + stack_table_bytes(p, nn);
