@@ -14,7 +14,8 @@
 // measured too and is NOT used: its workspace side writes 16-byte pieces, half a DRAM sector each, and scattered
 // partial-sector writes run at about half the rate of the 32-byte pieces the two-row tiles of pass R write
 // (641 us with TMA stores, 745 us with st.global, against 350 us).
-// Same producer / consumer-group / mbarrier structure as pipe_kernel.cuh; transform = pp_core.cuh.
+// Same producer / consumer-group / mbarrier structure as pipe_kernel.cuh; transform = the packed lane pair of
+// fft_packed.cuh (round 2; the scalar ping-pong form of pp_core.cuh took 277 us at 8192^2).
 #pragma once
 #include "pipe_kernel.cuh"
 
@@ -94,29 +95,26 @@ __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(con
     for (int j = g; j < nt; j += K::GROUPS) {
         const int b = j % K::NBUF;
         float2* sm = reinterpret_cast<float2*>(smraw + b * K::BUF);
-        float2 v[2][16];
+        PV pv;
         mbar_wait(&full[b], (j / K::NBUF) & 1);
-        // one planar element per column pair: (re X[2k], re X[2k+1], im X[2k], im X[2k+1]), k = us + e*Q;
-        // the column pass left conj(field) here (pass_kernel.cuh)
+        // one planar element per column pair: (re X[2k], re X[2k+1], im X[2k], im X[2k+1]), k = us + e*Q = the packed
+        // register pair (slot 0 = even columns, slot 1 = odd columns); the column pass left conj(field) here
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-            const float4 t4 = *reinterpret_cast<const float4*>(&sm[2 * (us + e * Q)]);
-            v[0][e] = make_float2(t4.x, t4.z); v[1][e] = make_float2(t4.y, t4.w);
+            const ulonglong2 t2 = *reinterpret_cast<const ulonglong2*>(&sm[2 * (us + e * Q)]);
+            pv.r[e] = t2.x; pv.i[e] = t2.y;
         }
         sync();                                             // staged image retired
-        pp_run<LOGC, false, 0, M, false>(v, us, 0, sm, sm + PP<LOGC>::REGION, tws, sync);
-        unpermute<16>(v[0]); unpermute<16>(v[1]);
-        sync();                                             // nobody still reads the exchange regions
+        transform_p<LOGC, false, true, false>(pv, us, 0, sm, tws, MidNone(), sync);
+        sync();                                             // nobody still reads the exchange image
         const float sc = P.out_scale;                       // conj completes the inverse transform
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
-            const float2 t = cmul(v[1][e], cmul(wb, w32_pow(e)));   // w^x B[x], x = us + e*Q
-            const float2 lo = cadd(v[0][e], t);
-            sm[us + e * Q] = make_float2(lo.x * sc, -lo.y * sc);
-            if constexpr (!PAD) {
-                const float2 hi = csub(v[0][e], t);
-                sm[N + us + e * Q] = make_float2(hi.x * sc, -hi.y * sc);
-            }
+            float ar, br, ai, bi;
+            pk_split(pv.r[e], ar, br); pk_split(pv.i[e], ai, bi);
+            const float2 t = cmul(make_float2(br, bi), cmul(wb, w32_pow(e)));   // w^x B[x], x = us + e*Q
+            sm[us + e * Q] = make_float2((ar + t.x) * sc, -(ai + t.y) * sc);
+            if constexpr (!PAD) sm[N + us + e * Q] = make_float2((ar - t.x) * sc, -(ai - t.y) * sc);
         }
         fence_proxy_async();
         mbar_arrive(&staged[b]);
