@@ -202,10 +202,12 @@ __device__ __forceinline__ void butterflies_p(PV& v, int us, int lns, const floa
 // The padded index of point j0 + q*2^lns is affine in q when lns == 0 (j0 is a multiple of 2^LR = 16) or
 // lns >= 4, and that of point us + e*Q is affine in e (Q is a multiple of 16): one address computation per
 // unit, immediate offsets per access.
-template <int LOGN, int LR, class SY>
+// LOGW: log2 of the lanes of the tile (default: the tile shape of the length; the 8192-point forward row pass runs
+// 4096-point lanes on a four-lane tile)
+template <int LOGN, int LR, class SY, int LOGW = tile_logw(LOGN)>
 __device__ __forceinline__ void exchange_store_p(const PV& v, int us, int w0, int lns, float2* sm, const SY& sync) {
     using C = Tile<LOGN>;
-    constexpr int R = 1 << LR, S = 16 / R, H = C::W / 2;
+    constexpr int R = 1 << LR, S = 16 / R, H = (1 << LOGW) / 2;
     ulonglong2* rg = reinterpret_cast<ulonglong2*>(sm);
     const int wh = w0 >> 1;
     if (!SY::EARLY_WAR) sync.war();                       // else taken by butterflies_p (war = true)
@@ -230,10 +232,10 @@ __device__ __forceinline__ void exchange_store_p(const PV& v, int us, int w0, in
         }
     }
 }
-template <int LOGN, class SY>
+template <int LOGN, class SY, int LOGW = tile_logw(LOGN)>
 __device__ __forceinline__ void exchange_load_p(PV& v, int us, int w0, const float2* sm, const SY& sync) {
     using C = Tile<LOGN>;
-    constexpr int H = C::W / 2;
+    constexpr int H = (1 << LOGW) / 2;
     const ulonglong2* rg = reinterpret_cast<const ulonglong2*>(sm);
     const int wh = w0 >> 1;
     static_assert(C::Q % 16 == 0, "Q multiple of 16");
@@ -245,11 +247,11 @@ __device__ __forceinline__ void exchange_load_p(PV& v, int us, int w0, const flo
     }
     sync.consumed();
 }
-template <int LOGN, int LR, class SY>
+template <int LOGN, int LR, class SY, int LOGW = tile_logw(LOGN)>
 __device__ __forceinline__ void exchange_p(PV& v, int us, int w0, int lns, float2* sm, const SY& sync) {
-    exchange_store_p<LOGN, LR>(v, us, w0, lns, sm, sync);
+    exchange_store_p<LOGN, LR, SY, LOGW>(v, us, w0, lns, sm, sync);
     sync.raw();
-    exchange_load_p<LOGN>(v, us, w0, sm, sync);
+    exchange_load_p<LOGN, SY, LOGW>(v, us, w0, sm, sync);
 }
 
 // radix-16 stage with the twiddle powers w[1..15] supplied (computed during the previous exchange)
@@ -272,7 +274,7 @@ __device__ __forceinline__ void stage_powers(int us, int lns, const float2* tw, 
 // Forward and/or inverse transform of the tile held in registers (fft_core.cuh transform()).  `mid`
 // (mid.packed(v), which must also conjugate) runs between the two, or first when MID_FIRST.  The last
 // forward stage, mid and the first inverse stage (no twiddles) form one compute phase without an exchange.
-template <int LOGN, bool HAS_FWD, bool HAS_INV, bool MID_FIRST, class Mid, class SY>
+template <int LOGN, bool HAS_FWD, bool HAS_INV, bool MID_FIRST, class Mid, class SY, int LOGW = tile_logw(LOGN)>
 __device__ __forceinline__ void transform_ahead_p(PV& v, int us, int w0, float2* sm, const float2* tw, const Mid& mid,
                                             const SY& sync) {
     using C = Tile<LOGN>;
@@ -280,7 +282,7 @@ __device__ __forceinline__ void transform_ahead_p(PV& v, int us, int w0, float2*
     static_assert(!(HAS_FWD && HAS_INV) || M >= 2, "merged middle phase needs an exchange after it");
     if constexpr (HAS_FWD && L0 > 0) {
         butterflies_p<LOGN, L0>(v, us, 0, tw, sync, true);
-        exchange_p<LOGN, L0>(v, us, w0, 0, sm, sync);
+        exchange_p<LOGN, L0, SY, LOGW>(v, us, w0, 0, sm, sync);
     }
     constexpr int NST = (HAS_FWD ? M : 0) + (HAS_INV ? M : 0);
     // Ns = 2^lns of radix-16 stage s of the list [forward 0..M-1 | inverse M..2M-1]
@@ -308,11 +310,11 @@ __device__ __forceinline__ void transform_ahead_p(PV& v, int us, int w0, float2*
         }
         // exchange; the next stage's twiddle powers are formed between publishing the stores and waiting for
         // everybody else's (they need neither, and v is dead in between)
-        exchange_store_p<LOGN, 4>(v, us, w0, lns, sm, sync);
+        exchange_store_p<LOGN, 4, SY, LOGW>(v, us, w0, lns, sm, sync);
         sync.raw_arrive();
         if (s + 1 < NST) stage_powers<LOGN>(us, lns_of(s + 1), tw, w);
         sync.raw_wait();
-        exchange_load_p<LOGN>(v, us, w0, sm, sync);
+        exchange_load_p<LOGN, SY, LOGW>(v, us, w0, sm, sync);
     }
     if constexpr (HAS_INV && L0 > 0) {
         butterflies_p<LOGN, L0>(v, us, 4 * M, tw, sync, false);
@@ -323,19 +325,19 @@ __device__ __forceinline__ void transform_ahead_p(PV& v, int us, int w0, float2*
 // Forward and/or inverse transform of the tile held in registers (fft_core.cuh transform()).  `mid`
 // (mid.packed(v), which must also conjugate) runs between the two, or first when MID_FIRST.  The last
 // forward stage, mid and the first inverse stage (no twiddles) form one compute phase without an exchange.
-template <int LOGN, bool HAS_FWD, bool HAS_INV, bool MID_FIRST, class Mid, class SY>
+template <int LOGN, bool HAS_FWD, bool HAS_INV, bool MID_FIRST, class Mid, class SY, int LOGW = tile_logw(LOGN)>
 __device__ __forceinline__ void transform_p(PV& v, int us, int w0, float2* sm, const float2* tw, const Mid& mid,
                                             const SY& sync) {
     using C = Tile<LOGN>;
     constexpr int L0 = C::L0, M = C::M;
     static_assert(!(HAS_FWD && HAS_INV) || M >= 2, "merged middle phase needs an exchange after it");
     if constexpr (SY::EARLY_WAR) {
-        transform_ahead_p<LOGN, HAS_FWD, HAS_INV, MID_FIRST>(v, us, w0, sm, tw, mid, sync);
+        transform_ahead_p<LOGN, HAS_FWD, HAS_INV, MID_FIRST, Mid, SY, LOGW>(v, us, w0, sm, tw, mid, sync);
         return;
     }
     if constexpr (HAS_FWD && L0 > 0) {
         butterflies_p<LOGN, L0>(v, us, 0, tw, sync, true);
-        exchange_p<LOGN, L0>(v, us, w0, 0, sm, sync);
+        exchange_p<LOGN, L0, SY, LOGW>(v, us, w0, 0, sm, sync);
     }
     constexpr int NST = (HAS_FWD ? M : 0) + (HAS_INV ? M : 0);
 #pragma unroll 1
@@ -357,7 +359,7 @@ __device__ __forceinline__ void transform_p(PV& v, int us, int w0, float2* sm, c
             unpermute_p<16>(v);
             break;
         }
-        exchange_p<LOGN, 4>(v, us, w0, lns, sm, sync);
+        exchange_p<LOGN, 4, SY, LOGW>(v, us, w0, lns, sm, sync);
     }
     if constexpr (HAS_INV && L0 > 0) {
         butterflies_p<LOGN, L0>(v, us, 4 * M, tw, sync, false);

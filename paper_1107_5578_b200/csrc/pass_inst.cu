@@ -5,6 +5,7 @@
 #include "prefetch_kernel.cuh"
 #include "lineconv_kernel.cuh"
 #include "linefft_kernel.cuh"
+#include "rowpair_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"

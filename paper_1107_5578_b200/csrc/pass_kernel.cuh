@@ -501,8 +501,16 @@ constexpr size_t PREFETCH_BYTES = 65536;
 template <int LOGN, int MID>
 static cudaError_t launch_colpref(int n_tiles, cudaStream_t s, const PassParams& p);
 
+// rowpair_kernel.cuh: forward row pass over 8192-point rows in packed arithmetic (one CTA per two-row tile)
+constexpr int ROWPAIR_LOGN = 13;
+template <int LOGN>
+static cudaError_t launch_rowpair_fwd(int n_tiles, cudaStream_t s, const PassParams& p);
+
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
+    if constexpr (LOGN == ROWPAIR_LOGN && KIND == ROW_FWD && !PAD && IOM == IN_COMPLEX) {
+        if (p.use_pipe && p.logwc == 1 && p.rows % 2 == 0 && !p.use_cluster) return launch_rowpair_fwd<LOGN>(n_tiles, s, p);
+    }
     if constexpr (KIND == COL_FUSED && PAD && MID != MID_ASM_F64 && LOGN >= 13) {
         if (p.use_pipe && (size_t)p.ly * Tile<LOGN>::W * 8 <= PREFETCH_BYTES) return launch_colpref<LOGN, MID>(n_tiles, s, p);
     }
