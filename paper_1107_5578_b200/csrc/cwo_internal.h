@@ -122,6 +122,7 @@ struct LineFftParams {
     const float2* pre; const float2* post;     // N entries each
     const float2* tw;                          // N-point forward twiddles
     int n_lines, inverse;
+    int pf_dist;                               // tiles between a CTA and the one that replaces it on its SM
 };
 #define CWO_DECL_LAUNCH(k) cudaError_t launch_linefft_##k(cudaStream_t s, const LineFftParams& p);
 CWO_DECL_LAUNCH(8) CWO_DECL_LAUNCH(9) CWO_DECL_LAUNCH(10) CWO_DECL_LAUNCH(11) CWO_DECL_LAUNCH(12) CWO_DECL_LAUNCH(13)

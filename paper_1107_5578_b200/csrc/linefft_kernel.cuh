@@ -34,6 +34,9 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) linefft_kerne
     const SyncSplit sy{&bars[0], &bars[1], 0u, 0u};
     sy.consumed();
 
+    // the tile of the CTA that will take this one's place on the SM: have L2 fetch it now (lineconv_kernel.cuh)
+    if (threadIdx.x == 0 && P.pf_dist > 0 && (int)blockIdx.x + P.pf_dist < P.n_lines / W)
+        l2_prefetch(P.in + (size_t)(blockIdx.x + P.pf_dist) * W * N, (uint32_t)(sizeof(float2) * W * N));
     const size_t base = ((size_t)blockIdx.x * W + w0) * N + us;       // point us + e Q of line (tile W + w0), then + N
     PV v;
 #pragma unroll
@@ -73,7 +76,9 @@ static cudaError_t launch_linefft_inst(cudaStream_t s, const LineFftParams& p) {
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, linefft_kernel<LOGN, INV>, p);
+    LineFftParams q = p;
+    q.pf_dist = d->n_sm * Tile<LOGN>::MINB;
+    return cudaLaunchKernelEx(&cfg, linefft_kernel<LOGN, INV>, q);
 }
 
 template <int LOGN>
