@@ -23,7 +23,10 @@ def _declared(header="cwo.h"):
 def test_header_declares_the_calls_of_the_scope_table():
     names = _declared()
     for must in ("cwo_plan", "cwo_asm", "cwo_fresnel_conv", "cwo_propagate_stack", "cwo_gs",
-                 "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_plan_set_stream", "cwo_strerror"):
+                 "cwo_plan_workspace_bytes", "cwo_plan_set_workspace", "cwo_plan_set_stream", "cwo_strerror",
+                 # SURVEY 8(f) rows f1-f4
+                 "cwo_plan_set_offset", "cwo_fresnel_fourier", "cwo_fresnel_shifted", "cwo_plan_set_dst_pitch_xy",
+                 "cwo_scale255", "cwo_pls_cgh"):
         assert must in names
 
 
