@@ -177,3 +177,20 @@ def test_shifted_and_gs_in_both_forms(api, oracle, mode):
         for _ in range(iters):
             p = oracle.gs_iter(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z)
         assert _phasor_rel_l2(ph.cpu().numpy(), p) <= REL_L2 * (1 + 2 * iters), "gs mode %d iters %d" % (mode, iters)
+
+
+@pytest.mark.parametrize("seed", range(10))
+def test_random_shapes_and_parameters_fourier_and_shifted(api, oracle, seed):
+    # seeded sweep over shapes (both tile orders), pitches, wavelengths, distances, destination pitches and offsets
+    r = np.random.default_rng(500 + seed)
+    ny, nx = (int(2 ** r.integers(8, 12)), int(2 ** r.integers(8, 12)))
+    lam = float(r.choice([405e-9, 532e-9, 633e-9]))
+    px, py = float(r.uniform(3e-6, 12e-6)), float(r.uniform(3e-6, 12e-6))
+    z = float(r.uniform(0.02, 0.6) * r.choice([-1.0, 1.0]))
+    u1 = _rand((ny, nx), 600 + seed)
+    _assert_parity(_gpu_fourier(api, u1, px, py, lam, z), oracle.fresnel_fourier(u1, px, py, lam, z),
+                   "fourier %dx%d z=%g" % (ny, nx, z))
+    p1 = (float(px * r.uniform(0.5, 2.0)), float(py * r.uniform(0.5, 2.0)))
+    off = (float(r.uniform(-1, 1) * nx * px), float(r.uniform(-1, 1) * ny * py))
+    _assert_parity(_gpu_shifted(api, u1, (px, py), p1, lam, z, off), oracle.fresnel_shifted(u1, (px, py), p1, lam, z, o1=off),
+                   "shifted %dx%d z=%g" % (ny, nx, z))
