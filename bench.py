@@ -425,6 +425,30 @@ def run_cuda(args):
     ms = S.max_over_ranks(ms, device="cuda")
     value = S.whole_job_rate([args.steps * wl["props_per_step"]] * world, ms)
 
+    # ---- launch-bound workloads: the same steps replayed from a CUDA graph (no Python / launch overhead) ----
+    graph_ms = None
+    if N <= 1024 and not use_dist:
+        try:
+            gs = torch.cuda.Stream()
+            gs.wait_stream(stream)
+            with torch.cuda.stream(gs):
+                step(0); gs.synchronize()
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=gs):
+                    for i in range(20):
+                        step(i)
+                g.replay()
+                g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                g0.record(gs)
+                for _ in range(10):
+                    g.replay()
+                g1.record(gs); gs.synchronize()
+                graph_ms = g0.elapsed_time(g1) / 200.0
+            stream.wait_stream(gs)
+        except Exception:
+            graph_ms = None
+        torch.cuda.synchronize()
+
     # ---- per-kernel durations (library-recorded CUDA events on the same stream) -------------------
     plan.set_timing(True)
     reps = min(max(args.steps, 6), 60) if wl["props_per_step"] == 1 else 2
@@ -502,6 +526,8 @@ def run_cuda(args):
                 "effective_gbs": eff, "pct_of_8TBs": 100.0 * eff / NOMINAL_HBM_GBS, "pct_of_measured_copy": 100.0 * eff / peak,
                 "scheme_bytes_per_step": int(wl["scheme_bytes_per_step"]),
                 "roofline": roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+        if graph_ms is not None:
+            line["ms_per_step_cuda_graph"] = graph_ms       # the step is launch-bound through the Python binding
         if args.fresnel_2d or args.no_pipeline:
             line["not_a_benchmark"] = "fresnel_2d=%d no_pipeline=%d" % (int(args.fresnel_2d), int(args.no_pipeline))
         if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
