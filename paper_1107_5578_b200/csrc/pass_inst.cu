@@ -6,6 +6,7 @@
 #include "lineconv_kernel.cuh"
 #include "linefft_kernel.cuh"
 #include "rowpair_kernel.cuh"
+#include "colpad_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"

@@ -503,13 +503,22 @@ static cudaError_t launch_colpref(int n_tiles, cudaStream_t s, const PassParams&
 
 // rowpair_kernel.cuh: forward row pass over 8192-point rows in packed arithmetic (one CTA per two-row tile)
 constexpr int ROWPAIR_LOGN = 13;
-template <int LOGN>
+template <int LOGN, bool PAD>
 static cudaError_t launch_rowpair_fwd(int n_tiles, cudaStream_t s, const PassParams& p);
+
+// colpad_kernel.cuh: fused column pass of the zero-expanded ASM on (even, odd)-bin lane pairs (zero half pruned)
+constexpr bool colpad_supported(int logn) { return logn == 13; }   // (4096-point padded columns: 84.4 vs 78.8 us, not used)
+template <int LOGN>
+static cudaError_t launch_colpad_fused_asm(int n_tiles, cudaStream_t s, const PassParams& p);
 
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
-    if constexpr (LOGN == ROWPAIR_LOGN && KIND == ROW_FWD && !PAD && IOM == IN_COMPLEX) {
-        if (p.use_pipe && p.logwc == 1 && p.rows % 2 == 0 && !p.use_cluster) return launch_rowpair_fwd<LOGN>(n_tiles, s, p);
+    if constexpr (colpad_supported(LOGN) && KIND == COL_FUSED && PAD && MID == MID_ASM_SPLIT) {
+        if (p.use_pipe && p.res_poly && !p.band && p.n_planes <= 1 && p.ly * 2 == Tile<LOGN>::N)
+            return launch_colpad_fused_asm<LOGN>(n_tiles, s, p);
+    }
+    if constexpr (LOGN == ROWPAIR_LOGN && KIND == ROW_FWD && IOM == IN_COMPLEX) {
+        if (p.use_pipe && p.logwc == 1 && p.rows % 2 == 0 && !p.use_cluster) return launch_rowpair_fwd<LOGN, PAD>(n_tiles, s, p);
     }
     if constexpr (KIND == COL_FUSED && PAD && MID != MID_ASM_F64 && LOGN >= 13) {
         if (p.use_pipe && (size_t)p.ly * Tile<LOGN>::W * 8 <= PREFETCH_BYTES) return launch_colpref<LOGN, MID>(n_tiles, s, p);

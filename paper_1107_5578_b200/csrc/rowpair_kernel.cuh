@@ -23,7 +23,8 @@ template <int LOGN> struct RowPairCfg {
     static constexpr size_t SMEM = EX_BYTES + 64 + sizeof(float2) * NTW;
 };
 
-template <int LOGN>
+// PAD (zero-expanded rows, Fresnel / CWO_OPT_ASM_PAD2X): only the first h points are stored, x[m+h] = 0: a = x, b = x w^m
+template <int LOGN, bool PAD>
 __global__ void __launch_bounds__(RowPairCfg<LOGN>::T, 1) rowpair_fwd_kernel(const __grid_constant__ PassParams P) {
     using K = RowPairCfg<LOGN>;
     using CH = typename K::CH;
@@ -45,7 +46,7 @@ __global__ void __launch_bounds__(RowPairCfg<LOGN>::T, 1) rowpair_fwd_kernel(con
     // the rows of the CTA that will take this one's place on the SM: have L2 fetch them now (nothing overlaps that
     // CTA's loads: the whole tile goes to registers before the first butterfly)
     if (threadIdx.x < 2 && P.pf_dist > 0 && (int)blockIdx.x + P.pf_dist < P.n_tiles)
-        l2_prefetch(P.in + (size_t)((blockIdx.x + P.pf_dist) * 2 + threadIdx.x) * P.pitch, (uint32_t)(2 * H * sizeof(float2)));
+        l2_prefetch(P.in + (size_t)((blockIdx.x + P.pf_dist) * 2 + threadIdx.x) * P.pitch, (uint32_t)((PAD ? 1 : 2) * H * sizeof(float2)));
     float2 tq[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) tq[e] = e == 0 ? wb : cmul(wb, w32_pow(e));
@@ -54,7 +55,7 @@ __global__ void __launch_bounds__(RowPairCfg<LOGN>::T, 1) rowpair_fwd_kernel(con
         const float2* x = P.in + (size_t)row * P.pitch + hus;
         float2 lo[16], hi[16];
 #pragma unroll
-        for (int e = 0; e < 16; ++e) { lo[e] = __ldcs(&x[e * QH]); hi[e] = __ldcs(&x[H + e * QH]); }
+        for (int e = 0; e < 16; ++e) { lo[e] = __ldcs(&x[e * QH]); hi[e] = PAD ? make_float2(0.f, 0.f) : __ldcs(&x[H + e * QH]); }
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             const float2 a = cadd(lo[e], hi[e]), d = csub(lo[e], hi[e]);
@@ -73,14 +74,14 @@ __global__ void __launch_bounds__(RowPairCfg<LOGN>::T, 1) rowpair_fwd_kernel(con
         __stcs(&out[(size_t)(hus + e * QH) * P.ly + row], make_ulonglong2(pv.r[e], pv.i[e]));
 }
 
-template <int LOGN>
+template <int LOGN, bool PAD>
 static cudaError_t launch_rowpair_fwd(int n_tiles, cudaStream_t s, const PassParams& p) {
     using K = RowPairCfg<LOGN>;
     DeviceInfo* d = device_info();
     if (!d) return cudaErrorInvalidDevice;
     static FuncOnce once;
     if (!once.done(d->index)) {
-        cudaError_t e = cudaFuncSetAttribute(rowpair_fwd_kernel<LOGN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM);
+        cudaError_t e = cudaFuncSetAttribute(rowpair_fwd_kernel<LOGN, PAD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)K::SMEM);
         if (e != cudaSuccess) return e;
         once.set(d->index);
     }
@@ -94,7 +95,7 @@ static cudaError_t launch_rowpair_fwd(int n_tiles, cudaStream_t s, const PassPar
     PassParams q = p;
     q.n_tiles = n_tiles;
     q.pf_dist = d->n_sm;
-    return cudaLaunchKernelEx(&cfg, rowpair_fwd_kernel<LOGN>, q);
+    return cudaLaunchKernelEx(&cfg, rowpair_fwd_kernel<LOGN, PAD>, q);
 }
 
 }  // namespace cwo
