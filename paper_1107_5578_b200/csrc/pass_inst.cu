@@ -7,6 +7,7 @@
 #include "linefft_kernel.cuh"
 #include "rowpair_kernel.cuh"
 #include "colpad_kernel.cuh"
+#include "colfold_kernel.cuh"
 
 #ifndef CWO_LOGN
 #error "compile with -DCWO_LOGN=<5..14>"

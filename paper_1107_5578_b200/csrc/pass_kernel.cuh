@@ -511,8 +511,17 @@ constexpr bool colpad_supported(int logn) { return logn == 13; }   // (4096-poin
 template <int LOGN>
 static cudaError_t launch_colpad_fused_asm(int n_tiles, cudaStream_t s, const PassParams& p);
 
+// colfold_kernel.cuh: fused ASM column pass over 8192-point columns as (even, odd)-bin lane pairs (4 exchanges)
+constexpr int COLFOLD_LOGN = 13;
+template <int LOGN>
+static cudaError_t launch_colfold_fused_asm(int n_tiles, cudaStream_t s, const PassParams& p);
+
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) {
+    if constexpr (LOGN == COLFOLD_LOGN && KIND == COL_FUSED && !PAD && MID == MID_ASM_SPLIT) {
+        if (p.use_pipe && p.res_poly && !p.band && p.n_planes <= 1 && p.ly == Tile<LOGN>::N)
+            return launch_colfold_fused_asm<LOGN>(n_tiles, s, p);
+    }
     if constexpr (colpad_supported(LOGN) && KIND == COL_FUSED && PAD && MID == MID_ASM_SPLIT) {
         if (p.use_pipe && p.res_poly && !p.band && p.n_planes <= 1 && p.ly * 2 == Tile<LOGN>::N)
             return launch_colpad_fused_asm<LOGN>(n_tiles, s, p);
