@@ -177,7 +177,7 @@ def run_reference(args):
 # workloads: c3 is the headline (BASELINE.json); the others time the same C-ABI calls on other configs
 # ------------------------------------------------------------------------------------------------------
 
-WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048),
+WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), "asm2048": ("asm", 2048), "asm16384": ("asm", 16384),
              "c2": ("fresnel", 1024), "fresnel2048": ("fresnel", 2048), "fresnel4096": ("fresnel", 4096),
              "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c4_intensity": ("stack_i", 2048), "c5": ("gs", 8192),
              "asm_pad2x_2048": ("asm_pad", 2048), "asm_pad2x_4096": ("asm_pad", 4096),
@@ -552,7 +552,7 @@ def main():
                     help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = {"c5": 3, "c4": 20, "c4_intensity": 20, "fresnel8192": 50, "asm8192": 100}.get(args.workload, 300)
+        args.steps = {"c5": 3, "c4": 20, "c4_intensity": 20, "fresnel8192": 50, "asm8192": 100, "asm16384": 10, "pls2048": 20}.get(args.workload, 300)
     if args.impl == "reference":
         run_reference(args)
     else:
