@@ -1,5 +1,5 @@
-// fold_kernel.cuh -- pipelined INVERSE row pass (R') for transform length 2n = 8192, built on the n = 4096
-// tile of pipe_kernel.cuh: one row is FOLDED into the two slots of a thread.
+// fold_kernel.cuh -- pipelined INVERSE row pass (R') for transform length 2n = 8192 (and zero-expanded 4096), built on
+// the n-point tile of pipe_kernel.cuh: one row is FOLDED into the two slots of a thread.
 //
 // A tile of two 8192-point lanes no longer fits three times in shared memory, so the 8192-point passes of
 // pass_kernel.cuh run one 139 KB tile per SM with nothing overlapped.  One radix-2 step (decimation in time,
@@ -23,14 +23,31 @@ namespace cwo {
 
 template <int LOGC> struct FoldCfg {
     using C = Tile<LOGC>;
-    static constexpr int GROUPS = 2, NBUF = 3, GT = 256;
+    // one row = the lane pair (even columns, odd columns) of the n-point transform: n/16 threads; 512 consumer threads
+    // per CTA in groups of one row each, and as many row buffers as fit (n = 4096: 2 groups, 3 buffers of 70 KB;
+    // n = 2048: 4 groups, 6 buffers of 35 KB)
+    static constexpr int GT = C::Q, GROUPS = 512 / GT, NBUF = GROUPS + GROUPS / 2;
     static constexpr int THREADS = GROUPS * GT + 128;
-    static constexpr size_t BUF = (C::SMEM_BYTES + 127) / 128 * 128;          // >= one row of 2n points (16 n bytes)
-    static constexpr size_t TW_OFF = NBUF * BUF + 64;                          // n-point twiddles, first Q entries
-    static constexpr size_t TW2_OFF = TW_OFF + sizeof(float2) * C::Q;          // 2n-point twiddles w^us, us < Q
+    static constexpr size_t BUF = (sizeof(float2) * (size_t)(C::N + C::N / 16) * 2 + 127) / 128 * 128;   // >= one row (16 n bytes)
+    static constexpr int NTW = PP<LOGC>::NTW_P;
+    static constexpr size_t TW_OFF = NBUF * BUF + 128;                         // n-point stage twiddles
+    static constexpr size_t TW2_OFF = TW_OFF + sizeof(float2) * NTW;           // 2n-point twiddles w^us, us < Q
     static constexpr size_t SMEM = TW2_OFF + sizeof(float2) * C::Q;
-    static_assert(C::L0 == 0 && C::W == 2 && C::T == GT, "fold core: n = 16^m, two slots, 256 threads per tile");
+    static_assert(GT == 128 || GT == 256, "rows of 4096 or 8192 points");
     static_assert(BUF >= sizeof(float2) * 2 * C::N, "row staging fits the tile buffer");
+    static_assert(2 * NBUF * sizeof(uint64_t) <= 128, "mbarriers fit their slot");
+};
+
+// barrier over the GT threads of one row group
+template <int GT> struct SyncRow {
+    static constexpr bool EARLY_WAR = false;
+    int id;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(GT) : "memory"); }
+    __device__ __forceinline__ void consumed() const {}
+    __device__ __forceinline__ void war() const { (*this)(); }
+    __device__ __forceinline__ void raw() const { (*this)(); }
+    __device__ __forceinline__ void raw_arrive() const {}
+    __device__ __forceinline__ void raw_wait() const { (*this)(); }
 };
 
 // Pass R': workspace -> IFFT_2n -> u2.
@@ -39,9 +56,10 @@ template <int LOGC, bool PAD>
 __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(const __grid_constant__ PassParams P) {
     using C = Tile<LOGC>;
     using K = FoldCfg<LOGC>;
-    constexpr int Q = C::Q, N = C::N, M = C::M;
+    constexpr int Q = C::Q, N = C::N;
     constexpr int NPR = PAD ? N : 2 * N;                    // points of a row that exist in the row-major field
     constexpr int GR = N / 256;                             // TMA boxes (256 column pairs each) per row
+    constexpr int GT = K::GT;
     extern __shared__ __align__(128) unsigned char smraw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smraw + K::NBUF * K::BUF);
     uint64_t* staged = full + K::NBUF;
@@ -54,7 +72,8 @@ __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(con
     }
     float2* tws = reinterpret_cast<float2*>(smraw + K::TW_OFF);
     float2* tw2 = reinterpret_cast<float2*>(smraw + K::TW2_OFF);
-    for (int i = threadIdx.x; i < Q; i += K::THREADS) { tws[i] = __ldg(&P.tw[2 * i]); tw2[i] = __ldg(&P.tw[i]); }
+    for (int i = threadIdx.x; i < K::NTW; i += K::THREADS) tws[i] = __ldg(&P.tw[2 * i]);
+    for (int i = threadIdx.x; i < Q; i += K::THREADS) tw2[i] = __ldg(&P.tw[i]);
     asm volatile("griddepcontrol.wait;" ::: "memory");      // see pipe_kernel.cuh
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     __syncthreads();
@@ -73,7 +92,7 @@ __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(con
             const int b = j % K::NBUF, row = blockIdx.x + j * gridDim.x;
             const unsigned char* src = smraw + b * K::BUF;
             unsigned char* dst = reinterpret_cast<unsigned char*>(P.out + (size_t)row * P.pitch);
-            for (uint32_t o = 0; o < NPR * 8u; o += 32768u) bulk_s2g(dst + o, src + o, 32768u);
+            for (uint32_t o = 0; o < NPR * 8u; o += 16384u) bulk_s2g(dst + o, src + o, 16384u);
             bulk_commit();
         };
         for (int j = 0; j < nt && j < K::NBUF; ++j) load(j);
@@ -88,8 +107,8 @@ __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(con
 
     // ===================================== consumer groups =====================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 112;");
-    const int g = threadIdx.x >> 8, us = threadIdx.x & 255;
-    const SyncGroup sync{1 + g};
+    const int g = threadIdx.x / GT, us = threadIdx.x % GT;
+    const SyncRow<GT> sync{1 + g};
     const float2 wb = tw2[us];                              // w^us
 #pragma unroll 1
     for (int j = g; j < nt; j += K::GROUPS) {
@@ -105,7 +124,7 @@ __global__ void __launch_bounds__(FoldCfg<LOGC>::THREADS, 1) fold_row_kernel(con
             pv.r[e] = t2.x; pv.i[e] = t2.y;
         }
         sync();                                             // staged image retired
-        transform_p<LOGC, false, true, false>(pv, us, 0, sm, tws, MidNone(), sync);
+        transform_p<LOGC, false, true, false, MidNone, SyncRow<GT>, 1>(pv, us, 0, sm, tws, MidNone(), sync);
         sync();                                             // nobody still reads the exchange image
         const float sc = P.out_scale;                       // conj completes the inverse transform
 #pragma unroll

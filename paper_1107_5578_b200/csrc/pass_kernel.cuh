@@ -485,8 +485,8 @@ constexpr bool pipe_supported(int logn) { return logn >= 10 && logn <= 12; }
 template <int LOGN, int KIND, bool PAD, int MID, int IOM>
 static cudaError_t launch_pipe(int n_tiles, cudaStream_t s, const PassParams& p);
 
-// fold_kernel.cuh: pipelined inverse row pass of length 2n = 8192 on the n = 4096 tile (one row per tile)
-constexpr int FOLD_LOGN = 13;
+// fold_kernel.cuh: pipelined inverse row pass of length 2n = 4096 / 8192 on one-row tiles (lane pair of the n-point transform)
+constexpr bool fold_supported(int logn) { return logn == 12 || logn == 13; }
 template <int LOGC, bool PAD>
 static cudaError_t launch_fold(int n_rows, cudaStream_t s, const PassParams& p);
 
@@ -536,7 +536,7 @@ static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) 
         if (p.use_cluster) return launch_cluster_row_fwd<LOGN, PAD>(n_tiles, s, p);           // n_tiles = rows
     }
     constexpr bool ROWPASS = (KIND == ROW_FWD || KIND == ROW_INV);
-    if constexpr (LOGN == FOLD_LOGN && KIND == ROW_INV && IOM == OUT_COMPLEX) {
+    if constexpr (fold_supported(LOGN) && KIND == ROW_INV && IOM == OUT_COMPLEX) {
         if (p.use_fold) return launch_fold<LOGN - 1, PAD>(n_tiles, s, p);                     // n_tiles = rows
     }
 #ifndef CWO_PIPE_FUSED
