@@ -182,7 +182,7 @@ WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), 
              "fresnel8192": ("fresnel", 8192), "c4": ("stack", 2048), "c4_intensity": ("stack_i", 2048), "c5": ("gs", 8192),
              "asm_pad2x_2048": ("asm_pad", 2048), "asm_pad2x_4096": ("asm_pad", 4096),
              "fourier4096": ("fourier", 4096), "fourier8192": ("fourier", 8192), "shifted4096": ("shifted", 4096),
-             "pls2048": ("pls", 2048)}
+             "pls2048": ("pls", 2048), "gs_asm2048": ("gs_asm", 2048)}
 
 
 def make_workload(name, rank, torch, api, W):
@@ -333,6 +333,39 @@ def make_workload(name, rank, torch, api, W):
                          "pitch 6.4 um, out 64x2048x2048 %s" % (name, "float32 intensity" if inten else "complex64"),
                     l2="spectrum (34 MB) stays in L2; the 2.1 GB output stack streams to HBM; no flush",
                     metric="planes/sec (c4 depth stack); effective HBM GB/s for 32 N^2 + n 32 N^2 bytes")
+    if op == "gs_asm":
+        # the paper's own GS experiment (Listing 8 / Table 7): angular spectrum propagator, 2048 x 2048, its
+        # default wavelength and pitch (633 nm, 10 um), 0.1 m, 20 iterations; inputs drawn like c5's
+        lam, pitch, z, iters = 633e-9, 10e-6, 0.1, 20
+        a_src, a_dst, phi0 = W.gs_inputs((N, N), 11 + rank)
+        d_src, d_dst = torch.from_numpy(a_src).cuda(), torch.from_numpy(a_dst).cuda()
+        d_phi0 = torch.from_numpy(phi0).cuda()
+        d_phi = torch.empty_like(d_phi0)
+        plan = api.cwo_plan(N, N, pitch, lam)
+        plan.set_option(api.CWO_OPT_GS_METHOD, api.CWO_GS_ASM)
+        plan.ensure_workspace(api.CWO_OP_GS)
+
+        def step(i):
+            d_phi.copy_(d_phi0)
+            api.cwo_gs(plan, d_src, d_dst, z, iters, d_phi)
+
+        def e2e():
+            pins = [torch.from_numpy(x).pin_memory() for x in (a_src, a_dst, phi0)]
+            pin_out = torch.empty((N, N), dtype=torch.float32).pin_memory()
+
+            def f(i):
+                d_src.copy_(pins[0], non_blocking=True); d_dst.copy_(pins[1], non_blocking=True)
+                d_phi.copy_(pins[2], non_blocking=True)
+                api.cwo_gs(plan, d_src, d_dst, z, iters, d_phi)
+                pin_out.copy_(d_phi, non_blocking=True)
+            return f, 12 * n2, 4 * n2
+        bps = iters * 2 * (48 + 4) * n2 + 52 * n2          # per propagation 48 N^2 + one amplitude read
+        return dict(plan=plan, step=step, N=N, props_per_step=2 * iters + 1, bytes_per_step=bps,
+                    kind_bytes={0: 16 * n2, 3: 16 * n2, 1: 20 * n2}, kind_flops={}, scheme_bytes_per_step=bps, e2e=e2e,
+                    desc="gs_asm2048: Gerchberg-Saxton with the angular spectrum propagator (the paper's Listing 8), 2048x2048, "
+                         "lambda 633 nm, pitch 10 um, z 0.1 m, 20 iterations (41 propagations per call)",
+                    l2="34 MB field + 34 MB workspace (L2-resident); no flush",
+                    metric="propagations/sec inside cwo_gs (ASM propagator, 41 per call)")
     cfg = W.CONFIGS["c5"]
     a_src, a_dst, phi0 = W.gs_inputs_c5(cfg)
     d_src, d_dst = torch.from_numpy(a_src).cuda(), torch.from_numpy(a_dst).cuda()
@@ -562,7 +595,7 @@ def main():
                     help="c3 (default) is the headline; the others are extra measurements of the same calls")
     args = ap.parse_args()
     if args.steps is None:
-        args.steps = {"c5": 3, "c4": 20, "c4_intensity": 20, "fresnel8192": 50, "asm8192": 100, "asm16384": 10, "pls2048": 20}.get(args.workload, 300)
+        args.steps = {"c5": 3, "gs_asm2048": 10, "c4": 20, "c4_intensity": 20, "fresnel8192": 50, "asm8192": 100, "asm16384": 10, "pls2048": 20}.get(args.workload, 300)
     if args.impl == "reference":
         run_reference(args)
     else:
