@@ -544,7 +544,7 @@ static cudaError_t launch_one(int n_tiles, cudaStream_t s, const PassParams& p) 
 #endif
     if constexpr (pipe_supported(LOGN) && MID != MID_ASM_F64 && (CWO_PIPE_FUSED || KIND != COL_FUSED) &&
                   (!ROWPASS || (KIND == ROW_FWD && IOM == IN_COMPLEX) ||
-                   (KIND == ROW_INV && (IOM == OUT_COMPLEX || IOM == OUT_INTENSITY)))) {
+                   (KIND == ROW_INV && (IOM == OUT_COMPLEX || IOM == OUT_INTENSITY || (IOM == OUT_PHASOR_AMP && !PAD))))) {
         if (p.use_pipe && (!ROWPASS || (p.use_tmap && p.rows % Tile<LOGN>::W == 0)))
             return launch_pipe<LOGN, KIND, PAD, MID, IOM>(n_tiles, s, p);
     }

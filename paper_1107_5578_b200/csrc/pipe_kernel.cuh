@@ -443,6 +443,28 @@ pipe_kernel(const __grid_constant__ PassParams P) {
                         y[e * QH] = (lo.x * lo.x + lo.y * lo.y) * (sc * sc);
                         y[H + e * QH] = (hi.x * hi.x + hi.y * hi.y) * (sc * sc);
                     }
+                } else if constexpr (IOM == OUT_PHASOR_AMP) {
+                    // GS constraints (S10; Listing 8 lines 11-13 / 15-16): keep u/|u| (1 where u == 0), impose the amplitude
+                    // of the next plane.  The amplitudes of all the thread's samples are requested before the first is used.
+                    const float* am = P.out_amp + (size_t)(tile * W + hr) * P.pitch + hus;
+                    float alo[16], ahi[16];
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) { alo[e] = __ldg(&am[e * QH]); ahi[e] = __ldg(&am[H + e * QH]); }
+                    float2* y = sm + hr * RS + hus;
+                    auto constrain = [](float2 u, float a) {           // u is conj(sample)
+                        const float m2 = u.x * u.x + u.y * u.y;
+                        float2 ph = make_float2(1.f, 0.f);
+                        if (m2 > 0.f) { const float r = rsqrtf(m2); ph = make_float2(u.x * r, -u.y * r); }
+                        return make_float2(a * ph.x, a * ph.y);
+                    };
+#pragma unroll
+                    for (int e = 0; e < 16; ++e) {
+                        float ar, br, ai, bi;
+                        pk_split(pv.r[e], ar, br); pk_split(pv.i[e], ai, bi);
+                        const float2 m = cmul(make_float2(br, bi), e < 8 ? tq[e] : cmul_mi(tq[e - 8]));
+                        y[e * QH] = constrain(make_float2(ar + m.x, ai + m.y), alo[e]);
+                        y[H + e * QH] = constrain(make_float2(ar - m.x, ai - m.y), ahi[e]);
+                    }
                 } else {
                     float2* y = sm + hr * RS + hus;
 #pragma unroll
@@ -538,7 +560,7 @@ pipe_kernel(const __grid_constant__ PassParams P) {
             for (int e = 0; e < 16; ++e)
                 *reinterpret_cast<float4*>(d + e * Q * W) = make_float4(v[0][e].x, v[1][e].x, v[0][e].y, v[1][e].y);
         } else if constexpr (KIND == ROW_INV) {
-            static_assert(IOM == OUT_COMPLEX || IOM == OUT_INTENSITY, "GS store modes run in pass_kernel");
+            static_assert(!PAD || IOM == OUT_COMPLEX || IOM == OUT_INTENSITY, "padded rows: GS store modes run in pass_kernel");
             const float sc = P.out_scale;                     // conj completes the inverse transform
             if constexpr (IOM == OUT_INTENSITY) {             // Eq.(20): |u|^2 as floats, same row stride (bytes) of the staging
                 float* smf = reinterpret_cast<float*>(sm);
