@@ -47,7 +47,8 @@ enum {
     CWO_EWORKSPACE = -2,    /* workspace missing or smaller than cwo_plan_workspace_bytes() */
     CWO_EUNSUPPORTED = -3,  /* current device is not compute capability 10.x */
     CWO_ECUDA = -4,         /* CUDA runtime failure; code via cwo_last_cuda_error() */
-    CWO_ENOMEM = -5         /* host or device allocation failed in cwo_plan() */
+    CWO_ENOMEM = -5,        /* host or device allocation failed in cwo_plan() */
+    CWO_ELIMIT = -6         /* cwo_scale255_static: n exceeds CWO_SCALE255_STATIC_MAX_N (its scratch is a fixed array) */
 };
 
 enum { CWO_OP_ASM = 1, CWO_OP_FRESNEL = 2, CWO_OP_STACK = 3, CWO_OP_GS = 4, CWO_OP_FRESNEL_FOURIER = 5,
@@ -161,6 +162,30 @@ int cwo_gs(cwo_plan_t plan, const float* amp_src, const float* amp_dst, double z
 /* "Scale", Eq.(21): out[i] = (in[i] - min in)/(max in - min in) * 255 over n floats (an intensity field
  * of any shape, e.g. a whole stack); a constant field maps to 0.  in, out: device, 16-byte aligned; out == in allowed. */
 int cwo_scale255(cwo_plan_t plan, const float* in, float* out, size_t n);
+
+/* Scale (Eq.(21)) without a plan and without any allocation: the same map as cwo_scale255, bit for bit,
+ * for callers that are not allowed to allocate device memory -- and therefore cannot call cwo_plan(), whose tables
+ * (the {min, max} cell of Scale among them) come from cudaMalloc.  Typical cases: a thread working while a CUDA graph
+ * is being captured elsewhere in the process in global mode (cudaMalloc is refused then), a component of a server or
+ * plug-in host that owns all device memory through its own pool, a real-time loop that cannot afford the device-wide
+ * synchronisation of cudaMalloc / cudaFree.
+ *   in, out      DEVICE pointers to n floats, 16-byte aligned, owned by the caller; out == in allowed.
+ *   cuda_stream  a cudaStream_t passed as void* (NULL: the null stream) on the CURRENT device; the call only enqueues
+ *                three kernels on it and returns.
+ *   cuda_error_out  may be NULL; receives the cudaError_t when the call returns CWO_ECUDA, else 0.
+ * Scratch: per-chunk minima / maxima go to a fixed array compiled into libcwo.so (256.25 KiB of device memory on every
+ * GPU that loads the library, held until the process exits), which bounds the size:
+ *   n <= CWO_SCALE255_STATIC_MAX_N (2^28 floats = 1 GiB, a 16384 x 16384 plane); larger n returns CWO_ELIMIT and
+ *   enqueues nothing.  n == 0, NULL or misaligned pointers: CWO_EINVAL.  Device not 10.x: CWO_EUNSUPPORTED.
+ * The call itself never calls cudaMalloc, cudaFree or any allocating routine.  The FIRST call on each device looks up
+ * the device address of the array (cudaGetSymbolAddress, once per device, with that device current); make that first
+ * call outside any stream capture.
+ * Every call on a GPU uses the same array, which keeps whatever the previous call left in it.  A call writes each
+ * word before it reads it, so leftovers are harmless and nothing needs clearing -- but two calls that may run on the
+ * GPU at the same time (streams with no ordering between them, or concurrent host threads) race on the array: keep
+ * calls on one device ordered (one stream, or events). */
+#define CWO_SCALE255_STATIC_MAX_N ((size_t)1 << 28)
+int cwo_scale255_static(const float* in, float* out, size_t n, void* cuda_stream, int* cuda_error_out);
 
 /* Computer-generated hologram of n point light sources, Eq.(23):
  *   out[j][i] = sum_k A_k cos( (2 pi/lambda) ((x - x_k)^2 + (y - y_k)^2)/(2 z_k) ),  (x, y) = ((i - Nx/2) px, (j - Ny/2) py),

@@ -22,7 +22,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("CWO_LIBRARY_PATH") or os.path.join(_HERE, "libcwo.so")
 
-CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA, CWO_ENOMEM = 0, -1, -2, -3, -4, -5
+CWO_OK, CWO_EINVAL, CWO_EWORKSPACE, CWO_EUNSUPPORTED, CWO_ECUDA, CWO_ENOMEM, CWO_ELIMIT = 0, -1, -2, -3, -4, -5, -6
+CWO_SCALE255_STATIC_MAX_N = 1 << 28
 CWO_OP_ASM, CWO_OP_FRESNEL, CWO_OP_STACK, CWO_OP_GS, CWO_OP_FRESNEL_FOURIER, CWO_OP_FRESNEL_SHIFTED = 1, 2, 3, 4, 5, 6
 CWO_OPT_GS_METHOD = 1
 CWO_OPT_PIPELINE = 3
@@ -35,7 +36,7 @@ CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 EXPORTS = ["cwo_plan", "cwo_plan_destroy", "cwo_plan_set_stream", "cwo_plan_set_pitch_xy", "cwo_plan_set_option",
            "cwo_plan_set_offset", "cwo_plan_set_dst_pitch_xy", "cwo_plan_workspace_bytes", "cwo_plan_set_workspace",
            "cwo_asm", "cwo_fresnel_conv", "cwo_fresnel_fourier", "cwo_fresnel_shifted", "cwo_propagate_stack", "cwo_gs",
-           "cwo_scale255", "cwo_pls_cgh", "cwo_strerror", "cwo_last_cuda_error"]
+           "cwo_scale255", "cwo_scale255_static", "cwo_pls_cgh", "cwo_strerror", "cwo_last_cuda_error"]
 DEBUG_EXPORTS = ["cwo_debug_set_timing", "cwo_debug_timings", "cwo_debug_launch_count", "cwo_debug_set_fresnel_2d",
                  "cwo_debug_set_fresnel_gather"]
 
@@ -78,6 +79,7 @@ def lib() -> ctypes.CDLL:
     L.cwo_propagate_stack.argtypes = [vp, vp, ctypes.POINTER(D), I, vp]
     L.cwo_gs.argtypes = [vp, vp, vp, D, I, vp]
     L.cwo_scale255.argtypes = [vp, vp, vp, sz]
+    L.cwo_scale255_static.argtypes = [vp, vp, sz, vp, ctypes.POINTER(I)]
     L.cwo_pls_cgh.argtypes = [vp, vp, I, vp]
     L.cwo_strerror.argtypes = [I]
     L.cwo_strerror.restype = ctypes.c_char_p
@@ -246,6 +248,25 @@ def cwo_scale255(plan: Plan, src: torch.Tensor, dst: torch.Tensor) -> None:
         raise TypeError("src, dst must be contiguous CUDA float32 tensors of one shape")
     plan.bind_stream()
     plan._check(lib().cwo_scale255(plan._h, src.data_ptr(), dst.data_ptr(), src.numel()), "cwo_scale255")
+
+
+def cwo_scale255_static(src: torch.Tensor, dst: torch.Tensor) -> None:
+    """Scale, Eq.(21), for callers that must not allocate device memory (no plan: cwo_plan() calls cudaMalloc).
+
+    Same result as cwo_scale255, bit for bit.  The library keeps the per-chunk minima and maxima in a fixed array inside
+    libcwo.so, so at most CWO_SCALE255_STATIC_MAX_N (2**28) floats per call; larger tensors raise CwoError(CWO_ELIMIT).
+    This binding allocates nothing either: it passes the two data pointers and torch's current stream.  All calls on a
+    GPU share that array: keep them ordered on one stream (calls that overlap on the GPU race).  Make the first call on a
+    device outside stream capture (it resolves the array's device address once)."""
+    if not (src.is_cuda and dst.is_cuda and src.dtype == torch.float32 and dst.dtype == torch.float32
+            and src.is_contiguous() and dst.is_contiguous() and src.shape == dst.shape and src.device == dst.device):
+        raise TypeError("src, dst must be contiguous CUDA float32 tensors of one shape on one device")
+    err = ctypes.c_int(0)
+    with torch.cuda.device(src.device):
+        rc = lib().cwo_scale255_static(src.data_ptr(), dst.data_ptr(), src.numel(),
+                                       torch.cuda.current_stream().cuda_stream, ctypes.byref(err))
+    if rc != CWO_OK:
+        raise CwoError(rc, "cwo_scale255_static", err.value)
 
 
 def cwo_pls_cgh(plan: Plan, pts: torch.Tensor, out: torch.Tensor) -> None:

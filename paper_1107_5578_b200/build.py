@@ -62,7 +62,7 @@ def build(force: bool = False, verbose: bool = False, ptxas_v: bool = False) -> 
     for k in LOGNS:
         o = os.path.join(OBJ, "pass_%d.o" % k)
         jobs.append((["nvcc"] + flags + ["-DCWO_LOGN=%d" % k, "-c", os.path.join(CSRC, "pass_inst.cu"), "-o", o], o))
-    for name in ("tables", "transpose", "outputs", "cwo"):
+    for name in ("tables", "transpose", "outputs", "scale_static", "cwo"):
         o = os.path.join(OBJ, name + ".o")
         jobs.append((["nvcc"] + flags + ["-c", os.path.join(CSRC, name + ".cu"), "-o", o], o))
     logs = []

@@ -281,6 +281,7 @@ extern "C" const char* cwo_strerror(int code) {
         case CWO_EUNSUPPORTED: return "device is not compute capability 10.x (B200)";
         case CWO_ECUDA: return "CUDA runtime error (see cwo_last_cuda_error)";
         case CWO_ENOMEM: return "out of memory while building the plan";
+        case CWO_ELIMIT: return "size exceeds the fixed scratch of the no-allocation entry point (CWO_SCALE255_STATIC_MAX_N)";
     }
     return "unknown error";
 }
