@@ -69,7 +69,8 @@ enum {
     CWO_OPT_ASM_BAND_LIMIT = 7 /* value 1: cwo_asm multiplies the transfer function by the two Rect band limits of
                                Eq.(18)-(19) for the on-axis case: bins with |fx| > 1/(lambda
                                sqrt((2 dfx z)^2 + 1)) (same in y) are zeroed, which removes the aliased part of H at
-                               long distances.  Default 0. */
+                               long distances.  Default 0.  cwo_propagate_stack and cwo_gs ignore this option and the
+                               offset of cwo_plan_set_offset: they always apply the plain H of Eq.(16). */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
 

@@ -101,6 +101,7 @@ class Plan:
         self.Nx, self.Ny = int(Nx), int(Ny)
         self._h = ctypes.c_void_p()
         self._ws = None
+        self._ws_streams = set()      # streams (handles) the current workspace tensor has been recorded on
         self.stack_intensity = False
         rc = lib().cwo_plan(self.Nx, self.Ny, float(pitch), float(lam), ctypes.byref(self._h))
         if rc != CWO_OK:
@@ -139,6 +140,7 @@ class Plan:
 
     def set_workspace(self, t: "torch.Tensor | None") -> None:
         self._ws = t
+        self._ws_streams = set()
         if t is None:
             self._check(lib().cwo_plan_set_workspace(self._h, None, 0), "cwo_plan_set_workspace")
         else:
@@ -149,15 +151,18 @@ class Plan:
         need = self.workspace_bytes(op, n)
         have = 0 if self._ws is None else self._ws.numel() * self._ws.element_size()
         if have < need:
-            old = self._ws
+            # Kernels already enqueued may still use the old block.  bind_stream() has recorded it on every stream the
+            # plan was bound to while it was the workspace, so the caching allocator keeps it back until those streams
+            # have passed this point, whichever stream is current now.
             self.set_workspace(torch.empty(need, dtype=torch.uint8, device="cuda"))
-            if old is not None:
-                # kernels enqueued on the plan's stream may still use the old block: keep the allocator from handing
-                # it out before they are done
-                old.record_stream(torch.cuda.current_stream())
 
     def bind_stream(self) -> None:
-        self._check(lib().cwo_plan_set_stream(self._h, torch.cuda.current_stream().cuda_stream), "cwo_plan_set_stream")
+        st = torch.cuda.current_stream()
+        self._check(lib().cwo_plan_set_stream(self._h, st.cuda_stream), "cwo_plan_set_stream")
+        # the call about to be enqueued on `st` uses the workspace, which torch may have allocated under another stream
+        if self._ws is not None and st.cuda_stream not in self._ws_streams:
+            self._ws.record_stream(st)
+            self._ws_streams.add(st.cuda_stream)
 
     def timings(self, cap: int = 4096):
         """[(tag, ms), ...] of the pass kernels launched since timing was switched on / last read."""

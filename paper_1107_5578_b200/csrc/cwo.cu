@@ -386,9 +386,10 @@ static bool asm_poly_ok(cwo_plan_t p, const double* zs, int n) {
 }
 
 // tab: n planes x [theta_x (mx) | theta_y (my)]; resc (may be null): z/lambda per plane.  Tiny kernels, no allocation.
-static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, int n, float* tab, float* resc) {
+// band: the call honours CWO_OPT_ASM_BAND_LIMIT and the offset (cwo_asm only: the stack and GS pass false, as cwo.h says).
+static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, int n, float* tab, float* resc, bool band) {
     const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
-    const bool shifted = p->band_limit != 0;
+    const bool shifted = band;
     for (int i0 = 0; i0 < n; i0 += ASM_PLANE_BATCH) {
         AsmPlaneBatch b;
         const int m = n - i0 < ASM_PLANE_BATCH ? n - i0 : ASM_PLANE_BATCH;
@@ -402,7 +403,7 @@ static int build_asm_tables(cwo_plan_t p, const Geometry& g, const double* zs, i
             b.p[i].oy = shifted ? p->off_y * dfy : 0.0;
         }
         CWO_CUDA(p, build_asm_phase_tables(tab + (size_t)i0 * (g.mx + g.my), resc ? resc + i0 : nullptr, b, m, g.mx, g.my,
-                                           p->stream));
+                                           p->stream, tab == p->asm_tab));
         p->launches++;
     }
     return CWO_OK;
@@ -425,7 +426,8 @@ static void band_range(double z, double lambda, double off, double df, int m, in
     *lo_out = lo; *hi_out = hi;
 }
 
-static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, bool poly, const float* tab, PassParams& pp) {
+static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, bool poly, const float* tab, PassParams& pp,
+                         bool band) {
     const double dfx = 1.0 / ((double)g.mx * p->px), dfy = 1.0 / ((double)g.my * p->py);
     pp.n_lane_bins = g.mx;
     if (split) {
@@ -437,10 +439,10 @@ static void fill_asm_mid(cwo_plan_t p, const Geometry& g, double z, bool split, 
     } else {
         pp.z = z; pp.inv_lam2 = 1.0 / (p->lambda * p->lambda);
         pp.df_lane = dfx; pp.df_point = dfy;
-        pp.off_lane = p->band_limit ? p->off_x : 0.0; pp.off_point = p->band_limit ? p->off_y : 0.0;
+        pp.off_lane = band ? p->off_x : 0.0; pp.off_point = band ? p->off_y : 0.0;
     }
-    pp.band = p->band_limit;
-    if (p->band_limit) {
+    pp.band = band ? 1 : 0;
+    if (band) {
         band_range(z, p->lambda, p->off_x, dfx, g.mx, &pp.band_lane_lo, &pp.band_lane_hi);
         band_range(z, p->lambda, p->off_y, dfy, g.my, &pp.band_point_lo, &pp.band_point_hi);
     }
@@ -549,7 +551,7 @@ static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const
 // One propagation of the two-dimensional form = pass R, pass C (fused), pass R'.  `ws` holds Ny rows x Mx columns
 // in column-tile order.  Fresnel: table set `set` must hold the spectra for this z.  ASM: tables (if split) in asm_tab.
 static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, bool poly, const PropIO& io, float2* ws,
-                      bool pad2x = false) {
+                      bool pad2x = false, bool band = false) {
     const Geometry g = geometry(p, method, pad2x);
     int rc;
     if ((rc = pass_row_fwd(p, g, io, ws)) != CWO_OK) return rc;
@@ -559,7 +561,7 @@ static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, b
     float scale = 1.0f;
     if (method == CWO_GS_ASM) {
         mid = split ? MID_ASM_SPLIT : MID_ASM_F64;
-        fill_asm_mid(p, g, z, split, poly, p->asm_tab, pp);
+        fill_asm_mid(p, g, z, split, poly, p->asm_tab, pp, band);
         scale = (float)(1.0 / ((double)g.mx * (double)g.my));       // 1/(MxMy) of the inverse FFT (reading R3)
     } else {
         mid = MID_TABLES; pp.tab_lane = p->chirp[set][0]; pp.tab_point = p->chirp[set][1]; pp.n_lane_bins = g.mx;
@@ -582,9 +584,10 @@ extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     const Geometry g = geometry(p, CWO_GS_ASM, pad2x);
     const bool split = asm_split_ok(p, &z, 1), poly = split && asm_poly_ok(p, &z, 1);
     int rc;
-    if (split && (rc = build_asm_tables(p, g, &z, 1, p->asm_tab, nullptr)) != CWO_OK) return rc;
+    const bool band = p->band_limit != 0;
+    if (split && (rc = build_asm_tables(p, g, &z, 1, p->asm_tab, nullptr, band)) != CWO_OK) return rc;
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
-    return run_passes(p, CWO_GS_ASM, z, 0, split, poly, io, (float2*)p->ws, pad2x);
+    return run_passes(p, CWO_GS_ASM, z, 0, split, poly, io, (float2*)p->ws, pad2x, band);
 }
 
 // ---- Fresnel diffraction, separable form (lineconv_kernel.cuh) --------------------------------------------------
@@ -773,7 +776,8 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     const Geometry g = geometry(p, CWO_GS_ASM);
     const size_t f = (size_t)p->Nx * p->Ny, fb = sizeof(float2) * f, tb = stack_table_bytes(p, n);
     if (!p->ws || p->ws_bytes < 2 * fb + tb) return CWO_EWORKSPACE;               // the minimum: one plane in flight
-    const int cap = (int)((p->ws_bytes - tb) / fb) - 1;                            // planes in flight
+    int cap = (int)((p->ws_bytes - tb) / fb) - 1;                                  // planes in flight
+    if (cap > STACK_BATCH) cap = STACK_BATCH;                                      // the measured and tested batch size
     float2* A = (float2*)p->ws;       // FFT2[u1] in column-tile order, computed once (S9)
     float2* B = A + f;                // planes between their column and row pass
     float* tab = (float*)((unsigned char*)p->ws + (size_t)(1 + cap) * fb);        // n x [theta_x | theta_y], then z/lambda
@@ -788,11 +792,14 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     // as the workspace holds, so the persistent CTAs fill and drain once per batch instead of once per plane.
     const bool pipe_len = g.logmx >= 10 && g.logmx <= 12 && g.logmy >= 10 && g.logmy <= 12;
     bool batched = split && p->pipeline && pipe_len && cap >= 2 && p->Ny % g.rb == 0;
-    if (batched) {                    // the tensor map of a batch must be encodable BEFORE anything is enqueued
-        CUtensorMap probe;
-        batched = encode_ws_tmap(&probe, B, p->Ny, g.mx, g.logwc, g.rb, cap < n ? cap : n);
-    }
-    if (split && (rc = build_asm_tables(p, g, zs, n, tab, resc)) != CWO_OK) return rc;
+    // the tensor maps of a full batch and of the remainder batch, encoded BEFORE anything is enqueued
+    CUtensorMap batch_map[2];
+    const int nb_full = cap < n ? cap : n, nb_rem = n % nb_full;
+    if (batched)
+        batched = encode_ws_tmap(&batch_map[0], B, p->Ny, g.mx, g.logwc, g.rb, nb_full) &&
+                  (nb_rem == 0 || encode_ws_tmap(&batch_map[1], B, p->Ny, g.mx, g.logwc, g.rb, nb_rem));
+    // the band limit and the offset are cwo_asm's (cwo.h): the band depends on |z|, and a batch shares one PassParams
+    if (split && (rc = build_asm_tables(p, g, zs, n, tab, resc, false)) != CWO_OK) return rc;
     PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, out_mode, nullptr, nullptr};
     if ((rc = pass_row_fwd(p, g, io, A)) != CWO_OK) return rc;
     PassParams pp; col_params(p, g, pp);
@@ -804,15 +811,14 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
             const int nb = n - k0 < cap ? n - k0 : cap;
             col_params(p, g, pp);
             pp.in = A; pp.out = B;
-            fill_asm_mid(p, g, zs[k0], true, poly, tab + (size_t)k0 * tab_stride, pp);
+            fill_asm_mid(p, g, zs[k0], true, poly, tab + (size_t)k0 * tab_stride, pp, false);
             pp.n_planes = nb; pp.tiles_per_plane = g.mx / g.wc; pp.in_plane_stride = 0; pp.out_plane_stride = f;
             pp.tab_plane_stride = tab_stride; pp.plane_resc = resc + k0;
             if ((rc = launch(p, g.logmy, COL_MIDINV, 0, MID_ASM_SPLIT, nb * (g.mx / g.wc), pp)) != CWO_OK) return rc;
             PassParams rp; row_params(p, g, rp);
             rp.in = B; rp.out = (float2*)out + (size_t)k0 * out_plane; rp.out_mode = out_mode; rp.out_scale = scale;
             rp.n_planes = nb; rp.tiles_per_plane = p->Ny / g.rb; rp.in_plane_stride = f; rp.out_plane_stride = out_plane;
-            rp.use_tmap = encode_ws_tmap(&rp.tmap, B, p->Ny, g.mx, g.logwc, g.rb, nb) ? 1 : 0;
-            if (!rp.use_tmap) return fail_cuda(p, cudaErrorUnknown);    // cannot happen: same shape as the probe
+            rp.tmap = batch_map[nb == nb_full ? 0 : 1]; rp.use_tmap = 1;
             if ((rc = launch(p, g.logmx, ROW_INV, 0, MID_NONE, nb * (p->Ny / g.rb), rp)) != CWO_OK) return rc;
             k0 += nb;
         }
@@ -821,7 +827,7 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     for (int k = 0; k < n; ++k) {
         col_params(p, g, pp);
         pp.in = A; pp.out = B;
-        fill_asm_mid(p, g, zs[k], split, poly, tab + (size_t)k * tab_stride, pp);
+        fill_asm_mid(p, g, zs[k], split, poly, tab + (size_t)k * tab_stride, pp, false);
         if ((rc = launch(p, g.logmy, COL_MIDINV, 0, split ? MID_ASM_SPLIT : MID_ASM_F64, g.mx / g.wc, pp)) != CWO_OK)
             return rc;
         io.out = (float2*)out + (size_t)k * out_plane;
@@ -914,7 +920,7 @@ extern "C" int cwo_gs(cwo_plan_t p, const float* amp_src, const float* amp_dst, 
     }
     // The ASM tables hold one z at a time; they are rebuilt before each propagation (tiny kernel).
     auto prop = [&](double zz, int set, const PropIO& io) -> int {
-        if (method == CWO_GS_ASM && split) { int r = build_asm_tables(p, geo, &zz, 1, p->asm_tab, nullptr); if (r != CWO_OK) return r; }
+        if (method == CWO_GS_ASM && split) { int r = build_asm_tables(p, geo, &zz, 1, p->asm_tab, nullptr, false); if (r != CWO_OK) return r; }
         return run_passes(p, method, zz, set, split, poly, io, ws);
     };
     // steps 1-2: G = amp_dst exp(i phi0); p = phasor(P(-z)[G]); the store already forms amp_src * p

@@ -143,7 +143,9 @@ struct AsmPlane { double c0, ax, ay, kz, ox, oy; };        // kz = z/lambda (-> 
 constexpr int ASM_PLANE_BATCH = 128;                      // planes per launch (passed by value)
 struct AsmPlaneBatch { AsmPlane p[ASM_PLANE_BATCH]; };
 cudaError_t build_asm_phase_tables(float* tab, float* resc, const AsmPlaneBatch& planes, int n_planes, int mx, int my,
-                                   cudaStream_t s);    // resc (may be null): z/lambda of every plane
+                                   cudaStream_t s, bool early);    // resc (may be null): z/lambda of every plane;
+                                                                   // early: tab is plan-owned (may be written before the
+                                                                   // preceding kernel of the stream has finished)
 // t[i] = scale (-1)^(alt i) exp(i 2 pi (c0 + c1 m + c2 m^2)), m = i - n/2, i < n; up to 4 tables per launch
 struct QuadTab { float2* out; int n; int alt; double c0, c1, c2, scale; };
 struct QuadTabBatch { QuadTab t[4]; };

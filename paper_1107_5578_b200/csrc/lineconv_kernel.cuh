@@ -236,7 +236,7 @@ __global__ void __launch_bounds__(Tile<LOGN>::T, Tile<LOGN>::MINB) lineconv_kern
 #pragma unroll 1
             for (int e = 0; e < 16; ++e) {
                 const float2 y = mine[e * C::T];
-                out[base + e * Q] = atan2f(y.y, y.x);
+                out[base + e * Q] = (y.x == 0.0f && y.y == 0.0f) ? 0.0f : atan2f(y.y, y.x);   // phasor(0) = 1 (cwo.h)
             }
             __syncthreads();
         }

@@ -420,7 +420,8 @@ pass_kernel(const __grid_constant__ PassParams P) {
                 if (row >= P.rows) continue;
                 const size_t a = (size_t)row * P.pitch + (s ? u[1] : u[0]) + e * Q;
                 const float2 x = mine[i * C::T];          // the sample is conj(x)
-                reinterpret_cast<float*>(P.out)[a] = atan2f(-x.y, x.x);
+                // phasor(0) = 1 (cwo.h): an exactly zero sample has phase 0, whatever the signs of its zeros
+                reinterpret_cast<float*>(P.out)[a] = (x.x == 0.0f && x.y == 0.0f) ? 0.0f : atan2f(-x.y, x.x);
             }
         }
     } else {

@@ -136,21 +136,24 @@ __global__ void asm_phase_kernel(float* tab, float* resc, const __grid_constant_
         c -= rint(c);
         t[i] = (float)c;
     }
-    // Launched with programmatic stream serialization: the table depends on nothing earlier in the stream (its
-    // previous reader finished before the preceding kernel let this one start), so it is computed while that
-    // kernel drains; completing only after it keeps the stream's order for everything that follows.
+    // Launched with programmatic stream serialization when the table is the plan's own: it depends on nothing earlier
+    // in the stream (its previous reader finished before the preceding kernel let this one start), so it is computed
+    // while that kernel drains; completing only after it keeps the stream's order for everything that follows.
     asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
+// early: the destination is memory that no kernel still running in the stream can be reading (the plan's own table);
+// otherwise (tables inside the caller's workspace, which the previous call's last kernel may still read) the kernel is
+// launched as an ordinary, fully ordered one and its griddepcontrol.wait is a no-op.
 cudaError_t build_asm_phase_tables(float* tab, float* resc, const AsmPlaneBatch& planes, int n_planes, int mx, int my,
-                                   cudaStream_t s) {
+                                   cudaStream_t s, bool early) {
     dim3 grid((mx + my + 255) / 256 > 64 ? 64 : (mx + my + 255) / 256, n_planes);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = 0; cfg.stream = s;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
+    cfg.attrs = at; cfg.numAttrs = early ? 1 : 0;
     return cudaLaunchKernelEx(&cfg, asm_phase_kernel, tab, resc, planes, mx, my);
 }
 

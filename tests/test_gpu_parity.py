@@ -474,6 +474,44 @@ def test_stack_batching_edges(api, oracle):
     assert api.lib().cwo_propagate_stack(plan._h, _dev(u1).data_ptr(), arr, 1, out.data_ptr()) == api.CWO_EWORKSPACE
 
 
+@pytest.mark.parametrize("n", [256, 1024])
+def test_stack_calls_back_to_back_on_one_workspace(api, oracle, n):
+    """Two stack calls with different plane counts enqueued back to back on ONE workspace sized for the first: the
+    second call's phase tables land where the first call's planes in flight were (the tables sit behind the planes),
+    so its table kernel must not start writing before the first call's last kernel has finished reading (it is an
+    ordinary, fully ordered launch when the tables live in the workspace).  Also a larger workspace than 64 planes' worth:
+    the batch is clamped to 64."""
+    cfg = W.CONFIGS["c4"].scaled(n)
+    u1 = W.make_field(cfg)
+    za, zb = [0.001, 0.004, -0.002], [0.002 * (k + 1) for k in range(7)]
+    f = 8 * n * n
+    plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+    plan.set_workspace(torch.empty(plan.workspace_bytes(api.CWO_OP_STACK, len(za)) + 4096 * len(zb), dtype=torch.uint8, device="cuda"))
+    d1 = _dev(u1)
+    oa = torch.empty((len(za), n, n), dtype=torch.complex64, device="cuda")
+    ob = torch.empty((len(zb), n, n), dtype=torch.complex64, device="cuda")
+    plan.bind_stream()
+    for rep in range(3):
+        oa.zero_(); ob.zero_()
+        assert api.lib().cwo_propagate_stack(plan._h, d1.data_ptr(), (api.ctypes.c_double * len(za))(*za), len(za), oa.data_ptr()) == 0
+        assert api.lib().cwo_propagate_stack(plan._h, d1.data_ptr(), (api.ctypes.c_double * len(zb))(*zb), len(zb), ob.data_ptr()) == 0
+        torch.cuda.synchronize()
+        for k in (0, len(za) - 1):
+            _assert_parity(oa[k].cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, za[k]), "first call, plane %d" % k)
+        for k in (0, len(zb) - 1):
+            _assert_parity(ob[k].cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, zb[k]), "second call, plane %d" % k)
+    if n == 1024:     # a workspace for 80 planes in flight: batches of at most 64 (70 planes = 64 + 6)
+        zs = [0.0005 * (k + 1) for k in range(70)]
+        plan = api.cwo_plan(n, n, cfg.pitch, cfg.lam)
+        plan.set_workspace(torch.empty(81 * f + 4 * 70 * (2 * n + 1) + 256, dtype=torch.uint8, device="cuda"))
+        out = torch.empty((len(zs), n, n), dtype=torch.complex64, device="cuda")
+        plan.bind_stream()
+        assert api.lib().cwo_propagate_stack(plan._h, d1.data_ptr(), (api.ctypes.c_double * len(zs))(*zs), len(zs), out.data_ptr()) == 0
+        torch.cuda.synchronize()
+        for k in (0, 63, 64, 69):
+            _assert_parity(out[k].cpu().numpy(), oracle.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, zs[k]), "plane %d of 70" % k)
+
+
 def test_back_to_back_calls_on_a_side_stream(api, oracle):
     """Programmatic dependent launch keeps stream order: alternating ASM / Fresnel calls with changing z, enqueued
     back to back on a non-default stream without synchronising, each read its predecessor's output."""
@@ -495,6 +533,30 @@ def test_back_to_back_calls_on_a_side_stream(api, oracle):
 
 
 # ---------------------------------------------------------------- randomised sweep -------------------------------
+
+
+def test_workspace_is_recorded_on_every_stream_it_is_used_on(api, oracle):
+    """The binding's workspace is a torch tensor: when it is regrown, the old block goes back to the caching allocator,
+    which may only reuse it once the kernels enqueued on EVERY stream the plan ran on are done.  The plan records the
+    workspace on each stream it is bound to (Plan.bind_stream), not on whatever stream is current when it regrows."""
+    u1 = _rand((512, 512), 71)
+    px, lam, z = 4e-6, 633e-9, 0.01
+    plan = api.cwo_plan(512, 512, px, lam)
+    d1 = _dev(u1); d2 = torch.empty_like(d1); d3 = torch.empty_like(d1)
+    api.cwo_asm(plan, d1, d2, z)                          # workspace allocated and used under the default stream
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    ws0 = plan._ws
+    with torch.cuda.stream(side):
+        api.cwo_asm(plan, d1, d2, -z)                     # the same block, now used on the side stream
+        assert side.cuda_stream in plan._ws_streams
+    api.cwo_fresnel_conv(plan, d1, d3, z)                 # regrows under the default stream while `side` may still run
+    assert plan._ws is not ws0 and torch.cuda.current_stream().cuda_stream in plan._ws_streams
+    assert side.cuda_stream not in plan._ws_streams       # the new block has not been used there
+    torch.cuda.synchronize()
+    _assert_parity(d2.cpu().numpy(), oracle.asm(u1, px, px, lam, -z), "asm on the side stream")
+    _assert_parity(d3.cpu().numpy(), oracle.fresnel_conv(u1, px, px, lam, z), "fresnel after the regrowth")
+
 
 @pytest.mark.parametrize("seed", range(16))
 def test_random_shapes_and_parameters(api, oracle, seed):
@@ -656,6 +718,93 @@ def test_asm_band_limited_fp64_path_and_option_off(api, oracle):
     api.cwo_asm(plan, d1, d2, 0.01)
     torch.cuda.synchronize()
     _assert_parity(d2.cpu().numpy(), oracle.asm(u1, 4e-6, 4e-6, lam, 0.01), "option off")
+
+
+@pytest.mark.parametrize("n,pipeline", [(256, 1), (1024, 1), (1024, 0)])
+def test_band_limit_and_offset_are_cwo_asm_only(api, oracle, n, pipeline):
+    """include/cwo.h: CWO_OPT_ASM_BAND_LIMIT and cwo_plan_set_offset change cwo_asm only.  With both set, the stack
+    (one launch pair per batch at 1024, plane by plane otherwise) and GS with the ASM propagator must give exactly what
+    they give without them -- at distances where the band of Eq.(18) would cut most of the grid and differs per plane."""
+    px, lam = 4e-6, 633e-9
+    zb = n * px * px / lam                                 # band edge = Nyquist / 2 at 1.0 zb, Nyquist / 6 at 3 zb
+    zs = [0.7 * zb, 3.0 * zb, -1.5 * zb, 2.2 * zb, 0.4 * zb]
+    u1 = _rand((n, n), 61)
+    outs = []
+    for band in (0, 1):
+        plan = api.cwo_plan(n, n, px, lam)
+        plan.set_option(api.CWO_OPT_PIPELINE, pipeline)
+        if band:
+            plan.set_option(api.CWO_OPT_ASM_BAND_LIMIT, 1)
+            plan.set_offset(13.4 * px, -7.7 * px)
+        out = torch.empty((len(zs), n, n), dtype=torch.complex64, device="cuda")
+        api.cwo_propagate_stack(plan, _dev(u1), zs, out)
+        torch.cuda.synchronize()
+        outs.append(out.cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
+    for k in (0, 1, 4):
+        _assert_parity(outs[1][k], oracle.asm(u1, px, px, lam, zs[k]), "stack plane %d with the band option set" % k)
+    amp_src, amp_dst, phi0 = W.gs_inputs((n, n), 9)
+    phases = []
+    for band in (0, 1):
+        plan = api.cwo_plan(n, n, px, lam)
+        plan.set_option(api.CWO_OPT_PIPELINE, pipeline)
+        plan.set_option(api.CWO_OPT_GS_METHOD, api.CWO_GS_ASM)
+        if band:
+            plan.set_option(api.CWO_OPT_ASM_BAND_LIMIT, 1)
+            plan.set_offset(13.4 * px, -7.7 * px)
+        ph = _dev(phi0.astype(np.float32))
+        api.cwo_gs(plan, _dev(amp_src), _dev(amp_dst), 3.0 * zb, 2, ph)
+        torch.cuda.synchronize()
+        phases.append(ph.cpu().numpy())
+    assert np.array_equal(phases[0], phases[1])
+
+
+@pytest.mark.parametrize("shape", [(64, 64), (256, 512), (1024, 1024), (4096, 4096)])
+def test_asm_pad2x_with_band_limit(api, oracle, shape):
+    """Zero expansion and the band limit together (the band-limited method of Eq.(18) as its authors use it: on the 2N grid):
+    the oracle's band-limited ASM on the field expanded with zeros, cropped.  4096: the prefetching padded column kernel."""
+    ny, nx = shape
+    px, lam = 4e-6, 633e-9
+    z = 2 * max(nx, ny) * px * px / lam * 1.5              # band edge = Nyquist / 3 on the expanded grid
+    u1 = _rand(shape, 63)
+    big = np.zeros((2 * ny, 2 * nx), dtype=np.complex64); big[:ny, :nx] = u1
+    cases = ((z, 0.0, 0.0), (-z, 21.3 * px, -9.6 * px)) if nx < 4096 else ((z, 21.3 * px, -9.6 * px),)
+    for zz, ox, oy in cases:
+        ref = oracle.asm_shifted(big, px, px, lam, zz, ox, oy)[:ny, :nx]
+        plan = api.cwo_plan(nx, ny, px, lam)
+        plan.set_option(api.CWO_OPT_ASM_PAD2X, 1)
+        plan.set_option(api.CWO_OPT_ASM_BAND_LIMIT, 1)
+        plan.set_offset(ox, oy)
+        d1 = _dev(u1); d2 = torch.empty_like(d1)
+        api.cwo_asm(plan, d1, d2, zz)
+        torch.cuda.synchronize()
+        _assert_parity(d2.cpu().numpy(), ref, "pad2x + band limit %s z=%g O=(%g,%g)" % (shape, zz, ox, oy))
+
+
+@pytest.mark.parametrize("method", [0, 1])
+def test_gs_with_zeros_in_the_target_amplitude(api, oracle, method):
+    """A target image with a black region (amp_dst == 0 there), 1024^2 (the packed TMA row store of the phasor x amplitude
+    mode): kinoform and one-iteration restart against the oracle; and an all-black target, where every propagated field
+    is exactly zero and phasor(0) = 1 (cwo.h) must give phase 0 everywhere, not NaN."""
+    n = 1024
+    cfg = W.CONFIGS["c5"]
+    z = cfg.zs[0] * n / 8192
+    amp_src, amp_dst, phi0 = W.gs_inputs((n, n), 11)
+    amp_dst = amp_dst.copy(); amp_dst[: n // 2, :] = 0.0; amp_dst[:, 100:164] = 0.0
+    th = _gs_gpu(api, method, amp_src, amp_dst, phi0, cfg.pitch, cfg.lam, z, 0)
+    p = oracle.gs_init(method, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z)
+    assert _phasor_rel_l2(th, p) <= REL_L2
+    p, G = oracle.gs_iter(method, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z, want_G=True)
+    phi_t = np.angle(G).astype(np.float32)
+    th = _gs_gpu(api, method, amp_src, amp_dst, phi_t, cfg.pitch, cfg.lam, z, 1)
+    pr = oracle.gs_init(method, amp_dst, phi_t, cfg.pitch, cfg.pitch, cfg.lam, z)
+    pr = oracle.gs_iter(method, amp_src, amp_dst, pr, cfg.pitch, cfg.pitch, cfg.lam, z)
+    assert _phasor_rel_l2(th, pr) <= REL_L2
+    black = np.zeros_like(amp_dst)
+    for iters in (0, 2):
+        th = _gs_gpu(api, method, amp_src, black, phi0, cfg.pitch, cfg.lam, z, iters)
+        assert np.all(th == 0.0), "all-black target, iters=%d" % iters
+        assert np.all(oracle.gs(method, amp_src, black, phi0, cfg.pitch, cfg.pitch, cfg.lam, z, iters) == 0.0)
 
 
 # ---------------------------------------------------------------- intensity stack (SURVEY 8(f) f4) --------------------
