@@ -16,8 +16,10 @@
  *              plan's stream and return (they may be captured into a CUDA graph); results are valid
  *              once the caller has synchronised that stream.  No host<->device copies.  Host arrays
  *              (zs) are read before return.
- *   Aliasing   u2 == u1 (exact in-place, as the paper's c.Diffract) is allowed.
- *              Partial overlap, or overlap with the workspace, is the caller's error.
+ *   Aliasing   u2 == u1 (exact in-place, as the paper's c.Diffract) is allowed; so is out == in for
+ *              cwo_scale255.  Any other overlap of an output with an input (stack: out with u1; cwo_gs: phase_out
+ *              with an amplitude; cwo_pls_cgh: out with pts), and any overlap of a field with the workspace, returns
+ *              CWO_EINVAL (a check of the pointer ranges; nothing is enqueued).
  *   Errors     int return, CWO_OK == 0, negative on failure.  Nothing is enqueued when a call
  *              returns CWO_EINVAL / CWO_EWORKSPACE / CWO_EUNSUPPORTED.  No exceptions, no
  *              global state; use one plan per host thread at a time, on the device it was made on.

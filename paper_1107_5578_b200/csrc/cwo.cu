@@ -576,10 +576,26 @@ static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, b
 
 static bool aligned16(const void* q) { return q && !((uintptr_t)q & 15); }
 
+// Aliasing rules of cwo.h, checked on the pointer ranges alone (no kernel work): an output may coincide EXACTLY with the
+// input it replaces (in place); any other overlap between an output and an input, or between a field and the
+// workspace, is refused with CWO_EINVAL.
+static bool overlaps(const void* a, size_t na, const void* b, size_t nb) {
+    const uintptr_t x = (uintptr_t)a, y = (uintptr_t)b;
+    return x < y + nb && y < x + na;
+}
+static bool partial_overlap(const void* in, const void* out, size_t n) { return in != out && overlaps(in, n, out, n); }
+static bool touches_ws(cwo_plan_t p, const void* q, size_t n) { return p->ws && overlaps(q, n, p->ws, p->ws_bytes); }
+// u1 -> u2, both complex Nx x Ny fields
+static bool fields_alias_badly(cwo_plan_t p, const void* u1, const void* u2) {
+    const size_t fb = sizeof(float2) * (size_t)p->Nx * p->Ny;
+    return partial_overlap(u1, u2, fb) || touches_ws(p, u1, fb) || touches_ws(p, u2, fb);
+}
+
 extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || !asm_sizes_ok(p)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_ASM, 0)) return CWO_EWORKSPACE;
+    if (fields_alias_badly(p, u1, u2)) return CWO_EINVAL;
     const bool pad2x = p->asm_pad2x != 0;
     const Geometry g = geometry(p, CWO_GS_ASM, pad2x);
     const bool split = asm_split_ok(p, &z, 1), poly = split && asm_poly_ok(p, &z, 1);
@@ -624,6 +640,7 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_sizes_ok(p)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL, 0)) return CWO_EWORKSPACE;
+    if (fields_alias_badly(p, u1, u2)) return CWO_EINVAL;
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0);
     if (rc != CWO_OK) return rc;
     if (fresnel_separable(p) && separable_gather(p)) {
@@ -674,6 +691,7 @@ extern "C" int cwo_fresnel_fourier(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_separable(p)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL_FOURIER, 0)) return CWO_EWORKSPACE;
+    if (fields_alias_badly(p, u1, u2)) return CWO_EINVAL;
     // Eq.(8): pre = (-1)^j exp(i pi x1^2/(lambda z)); Eq.(9): post = (-1)^j exp(i pi x2^2/(lambda z)) [x c on the x axis],
     // x2 = m lambda|z|/(N p) (reading R17)
     double cc, cm; fresnel_coef(p, z, &cc, &cm);
@@ -706,6 +724,7 @@ extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_separable(p)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_FRESNEL_SHIFTED, 0)) return CWO_EWORKSPACE;
+    if (fields_alias_badly(p, u1, u2)) return CWO_EINVAL;
     const double p1x = p->p1x > 0.0 ? p->p1x : p->px, p1y = p->p1y > 0.0 ? p->p1y : p->py;
     // spectra of h = exp(i pi S m^2) with the coefficient folded in (Eq.(13), Eq.(11))
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0, p1x, p1y);
@@ -752,6 +771,7 @@ enum { KIND_MINMAX = 8, KIND_SCALE = 9, KIND_PLS = 10 };
 
 extern "C" int cwo_scale255(cwo_plan_t p, const float* in, float* out, size_t n) {
     if (!p || !aligned16(in) || !aligned16(out) || n == 0) return CWO_EINVAL;
+    if (partial_overlap(in, out, sizeof(float) * n)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     DeviceInfo* d = device_info();
     if (!d) return CWO_EINVAL;
@@ -764,6 +784,7 @@ extern "C" int cwo_scale255(cwo_plan_t p, const float* in, float* out, size_t n)
 
 extern "C" int cwo_pls_cgh(cwo_plan_t p, const double* pts, int n, float* out) {
     if (!p || !aligned16(pts) || !aligned16(out) || n <= 0) return CWO_EINVAL;
+    if (overlaps(pts, sizeof(double) * 4 * (size_t)n, out, sizeof(float) * (size_t)p->Nx * p->Ny)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     return launch_tagged(p, KIND_PLS, [&] {
         return launch_pls_cgh(pts, n, out, p->Nx, p->Ny, p->px, p->py, p->lambda, p->stream); });
@@ -776,6 +797,10 @@ extern "C" int cwo_propagate_stack(cwo_plan_t p, const cwo_c64* u1, const double
     const Geometry g = geometry(p, CWO_GS_ASM);
     const size_t f = (size_t)p->Nx * p->Ny, fb = sizeof(float2) * f, tb = stack_table_bytes(p, n);
     if (!p->ws || p->ws_bytes < 2 * fb + tb) return CWO_EWORKSPACE;               // the minimum: one plane in flight
+    {
+        const size_t ob = (p->stack_intensity ? fb / 2 : fb) * (size_t)n;
+        if (overlaps(u1, fb, out, ob) || touches_ws(p, u1, fb) || touches_ws(p, out, ob)) return CWO_EINVAL;
+    }
     int cap = (int)((p->ws_bytes - tb) / fb) - 1;                                  // planes in flight
     if (cap > STACK_BATCH) cap = STACK_BATCH;                                      // the measured and tested batch size
     float2* A = (float2*)p->ws;       // FFT2[u1] in column-tile order, computed once (S9)
@@ -904,6 +929,12 @@ extern "C" int cwo_gs(cwo_plan_t p, const float* amp_src, const float* amp_dst, 
     if (method == CWO_GS_ASM ? !asm_sizes_ok(p) : (!fresnel_sizes_ok(p) || z == 0.0)) return CWO_EINVAL;
     if (check_call(p) != CWO_OK) return CWO_EINVAL;
     if (!p->ws || p->ws_bytes < cwo_plan_workspace_bytes(p, CWO_OP_GS, 0)) return CWO_EWORKSPACE;
+    {   // the two amplitudes are only read (they may coincide); phase_out is written
+        const size_t rb = sizeof(float) * (size_t)p->Nx * p->Ny;
+        if (overlaps(amp_src, rb, phase_out, rb) || overlaps(amp_dst, rb, phase_out, rb) || touches_ws(p, amp_src, rb) ||
+            touches_ws(p, amp_dst, rb) || touches_ws(p, phase_out, rb))
+            return CWO_EINVAL;
+    }
     if (method == CWO_GS_FRESNEL && fresnel_separable(p)) return gs_fresnel_separable(p, amp_src, amp_dst, z, iters, phase_out);
     const size_t f = (size_t)p->Nx * p->Ny;
     float2* g = (float2*)p->ws;          // the constrained field between propagations (8 B/px)

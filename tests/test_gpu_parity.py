@@ -399,6 +399,44 @@ def test_error_codes(api):
     assert plan.launch_count >= 2
 
 
+def test_overlapping_buffers_are_refused(api):
+    """include/cwo.h, Aliasing: exact in-place is allowed; partial overlap of an output with an input, or of a field with
+    the workspace, returns CWO_EINVAL before anything is enqueued (launch count unchanged)."""
+    n = 64
+    fb = 8 * n * n
+    L = api.lib()
+    plan = api.cwo_plan(n, n, 1e-5, 633e-9)
+    pool = torch.zeros(8 * n * n, dtype=torch.complex64, device="cuda")       # room for fields and a workspace side by side
+    base = pool.data_ptr()
+    plan.set_workspace(pool.view(torch.uint8)[4 * fb:])                        # workspace = second half of the pool
+    plan.bind_stream()
+    u1, u2 = base, base + fb
+    assert L.cwo_asm(plan._h, u1, u2, 0.1) == api.CWO_OK                       # disjoint neighbours
+    assert L.cwo_asm(plan._h, u1, u1, 0.1) == api.CWO_OK                       # exactly in place
+    count = plan.launch_count
+    for call in (L.cwo_asm, L.cwo_fresnel_conv):
+        assert call(plan._h, u1, u1 + 16, 0.1) == api.CWO_EINVAL               # shifted by two samples
+        assert call(plan._h, u1 + fb // 2, u1, 0.1) == api.CWO_EINVAL          # half a field apart
+        assert call(plan._h, u1, base + 4 * fb, 0.1) == api.CWO_EINVAL         # u2 is the start of the workspace
+        assert call(plan._h, base + 4 * fb - 16, u1, 0.1) == api.CWO_EINVAL    # u1 runs into the workspace
+    zs = (api.ctypes.c_double * 2)(0.1, 0.2)
+    assert L.cwo_propagate_stack(plan._h, u1, zs, 2, u1) == api.CWO_EINVAL     # the stack is never in place
+    assert L.cwo_propagate_stack(plan._h, u1 + fb, zs, 2, u1) == api.CWO_EINVAL   # plane 1 of out = u1
+    assert L.cwo_propagate_stack(plan._h, u1, zs, 2, base + 3 * fb) == api.CWO_EINVAL   # plane 1 of out = workspace
+    plan.set_option(api.CWO_OPT_GS_METHOD, api.CWO_GS_ASM)
+    rb = 4 * n * n
+    a, b, ph = base, base + rb, base + 2 * rb
+    assert L.cwo_gs(plan._h, a, a, 0.1, 0, ph) == api.CWO_OK                   # the two amplitudes may coincide
+    assert L.cwo_gs(plan._h, a, b, 0.1, 1, b) == api.CWO_EINVAL                # phase_out = amp_dst
+    assert L.cwo_gs(plan._h, a, b, 0.1, 1, a + 16) == api.CWO_EINVAL
+    assert L.cwo_scale255(plan._h, a, a, n * n) == api.CWO_OK
+    count = plan.launch_count
+    assert L.cwo_scale255(plan._h, a, a + 16, n * n) == api.CWO_EINVAL
+    assert L.cwo_pls_cgh(plan._h, a, 4, a) == api.CWO_EINVAL                   # the hologram over its own point list
+    assert plan.launch_count == count
+    torch.cuda.synchronize()
+
+
 def test_host_pipeline_matches_oracle(api, oracle):
     """api.HostPipeline (pinned host buffers, copies overlapped over three streams): every step's result is
     that step's propagation -- more steps than device buffers, so slots are reused."""
