@@ -12,7 +12,11 @@ inverse row pass) over one 4096 x 4096 complex64 field of BASELINE.json config c
              u2 inside the timed region
   roofline   the dominant kernel (c3: the fused column pass): algorithmic bytes (or nominal flops) per launch / its
              average duration from CUDA events recorded by the library (include/cwo_debug.h timing mode)
-  cpu_baseline  the fp64 oracle as it stands on the host cores (reported baseline, not the target)
+  cpu_baseline  the fp64 oracle as it stands on the host cores (reported baseline, not the target): c3 on all threads
+             and on one thread, the CPU model, and one propagation of every other BASELINE config
+  extra      (default run, N = 1 only) the other sizes the throughput target names -- asm8192, fresnel4096, fresnel8192,
+             c4, c5 -- each timed briefly after the headline: ms per call against its target, effective GB/s, the
+             dominant kernel's roofline fraction, clocks.  --no-extra skips them (profiling runs).
 
 --impl reference times the oracle itself (this tier has no installable reference implementation).
 N > 1: the path does not shard (replicas only) -- every rank propagates its own field.
@@ -134,13 +138,100 @@ def _oracle_time_props(cfg, n_props: int, size: int):
     return time.perf_counter() - t0, threads
 
 
-def cpu_baseline(cfg, budget_s: float = 20.0):
-    """The oracle as it stands, on a bounded sample: whole 4096^2 propagations while they fit the budget."""
+def _cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def _mem_available_gb():
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable"):
+                return float(line.split()[1]) / 1e6
+    except Exception:
+        pass
+    return 0.0
+
+
+_C5_INPUTS = {}
+
+
+def _gs_inputs_c5(W):
+    """c5's amplitudes and start phase (7 s of host work at 8192^2): drawn once per process."""
+    if "v" not in _C5_INPUTS:
+        _C5_INPUTS["v"] = W.gs_inputs_c5(W.CONFIGS["c5"])
+    return _C5_INPUTS["v"]
+
+
+def cpu_baseline_per_config(budget_s: float = 60.0):
+    """the oracle's time for ONE propagation of each BASELINE config (c4: one plane; c5: one Fresnel
+    propagation and one GS iteration), all host threads.  The c5 entries (three fp64 FFTs of 16384^2 per propagation,
+    ~9 GB) run only if their estimate fits the remaining budget and the host has the memory; otherwise they say so."""
+    from oracle import oracle as O
+    from paper_1107_5578_b200 import workloads as W
+    threads = O.max_threads()
+    O.set_threads(threads)
+    out, t_begin = {}, time.perf_counter()
+
+    def timed(f):
+        t0 = time.perf_counter(); f(); return time.perf_counter() - t0
+    for name in ("c1", "c2", "c4"):
+        cfg = W.CONFIGS[name]
+        u1 = W.make_field(cfg)
+        f = O.asm if cfg.op != "fresnel" else O.fresnel_conv
+        key = name if name != "c4" else "c4_one_plane"
+        out[key] = {"what": "%s %dx%d, one propagation" % ("Fresnel convolution" if f is O.fresnel_conv else "ASM", cfg.N, cfg.N),
+                    "seconds": timed(lambda: f(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0])), "threads": threads}
+    c5 = W.CONFIGS["c5"]
+    # one c5 propagation = three 2-D FFTs of (2 * 8192)^2 against three of (2 * 1024)^2 for c2
+    est = out["c2"]["seconds"] * (16384.0 ** 2 * 28) / (2048.0 ** 2 * 22)
+    for key, mult in (("c5_fresnel_propagation", 1.0), ("c5_gs_iteration", 2.0)):
+        left = budget_s - (time.perf_counter() - t_begin)
+        if est * mult > left or _mem_available_gb() < 40.0:
+            out[key] = {"skipped": "estimated %.0f s against %.0f s of budget left, %.0f GB of host memory available"
+                                   % (est * mult, left, _mem_available_gb())}
+            continue
+        if key == "c5_fresnel_propagation":
+            u1 = W.field_c3(W.Config("c5f", "fresnel", c5.N, c5.lam, c5.pitch, c5.zs, index=c5.index + 100))
+            sec = timed(lambda: O.fresnel_conv(u1, c5.pitch, c5.pitch, c5.lam, c5.zs[0]))
+            what = "Fresnel convolution 8192x8192 (transforms of 16384x16384), one propagation"
+            est = sec
+        else:
+            a_src, a_dst, _ = _gs_inputs_c5(W)
+            pz = W.random_phasor(c5)
+            sec = timed(lambda: O.gs_iter(0, a_src, a_dst, pz, c5.pitch, c5.pitch, c5.lam, c5.zs[0]))
+            what = "one Gerchberg-Saxton iteration at 8192x8192 (two Fresnel propagations + constraints)"
+        out[key] = {"what": what, "seconds": sec, "threads": threads}
+    return out
+
+
+def cpu_baseline(cfg, budget_s: float = 20.0, per_config: bool = True):
+    """The oracle as it stands, on a bounded sample: whole 4096^2 propagations while they fit the budget; then (SURVEY.md
+    8(d)) the same propagation on ONE thread and one propagation of each of the other configs."""
+    from oracle import oracle as O
     t1, threads = _oracle_time_props(cfg, 1, cfg.N)
     n = int(max(1, min(8, budget_s // max(t1, 1e-3))))
     t, _ = _oracle_time_props(cfg, n, cfg.N)
-    return {"value": n / t, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": "%d full %dx%d fp64 oracle propagation(s), %d OpenMP threads, %.2f s" % (n, cfg.N, cfg.N, threads, t)}
+    out = {"value": n / t, "unit": UNIT, "cores": threads, "kind": "oracle", "cpu_model": _cpu_model(),
+           "sample": "%d full %dx%d fp64 oracle propagation(s), %d OpenMP threads, %.2f s" % (n, cfg.N, cfg.N, threads, t)}
+    if per_config:
+        from paper_1107_5578_b200 import workloads as W
+        u1 = W.make_field(cfg)
+        O.set_threads(1)
+        t0 = time.perf_counter()
+        O.asm(u1, cfg.pitch, cfg.pitch, cfg.lam, cfg.zs[0])
+        ts = time.perf_counter() - t0
+        O.set_threads(threads)
+        out["one_thread"] = {"value": 1.0 / ts, "unit": UNIT, "cores": 1,
+                             "sample": "1 full %dx%d fp64 oracle propagation on one thread, %.2f s" % (cfg.N, cfg.N, ts)}
+        out["per_config"] = cpu_baseline_per_config()
+        out["per_config"]["c3"] = {"what": "ASM %dx%d, one propagation" % (cfg.N, cfg.N), "seconds": t / n, "threads": threads}
+    return out
 
 
 def run_reference(args):
@@ -185,10 +276,12 @@ WORKLOADS = {"c1": ("asm", 256), "c3": ("asm", 4096), "asm8192": ("asm", 8192), 
              "pls2048": ("pls", 2048), "gs_asm2048": ("gs_asm", 2048)}
 
 
-def make_workload(name, rank, torch, api, W):
-    """Device-resident inputs, the step function and the algorithmic byte counts of a workload."""
+def make_workload(name, rank, torch, api, W, nbuf=3):
+    """Device-resident inputs, the step function and the algorithmic byte counts of a workload.
+    nbuf: field pairs the steps rotate over (the `extra` legs use one: a single 4096^2 / 8192^2 step already touches
+    403 MB / 1.6 GB, more than the 126 MB L2)."""
     op, N = WORKLOADS[name]
-    NBUF = 3
+    NBUF = nbuf
     n2 = float(N) * N
     pad2x = op == "asm_pad"                                  # SURVEY 8(f) f1: cwo_asm on the zero-expanded grid
     if pad2x:
@@ -290,8 +383,8 @@ def make_workload(name, rank, torch, api, W):
                                                            N, N, 2 * N, 2 * N, base.lam * 1e9, base.pitch * 1e6,
                                                            "{" + ",".join("%.4g" % z for z in zs) + "}"))
         ws = (24 if (op == "asm" and not pad2x) else 32) * n2   # u1 + u2 + workspace touched per step
-        l2 = ("working set %.0f MB per step, rotating over 3 field pairs (%s the 126 MB L2); no flush"
-              % (ws / 1e6, "larger than" if ws > 126e6 else "FITS in"))
+        l2 = ("working set %.0f MB per step, rotating over %d field pair%s (%s the 126 MB L2); no flush"
+              % (ws / 1e6, NBUF, "s" if NBUF > 1 else "", "larger than" if ws > 126e6 else "FITS in"))
         # nominal flops of one line-convolution launch: N lines x (4 N-point FFTs at 5 n log2 n + ~30 flops per sample for
         # the modulation, the spectrum multiply and the recombination)
         kf = {5: N * (20.0 * N * np.log2(N) + 30.0 * N)}
@@ -367,7 +460,7 @@ def make_workload(name, rank, torch, api, W):
                     l2="34 MB field + 34 MB workspace (L2-resident); no flush",
                     metric="propagations/sec inside cwo_gs (ASM propagator, 41 per call)")
     cfg = W.CONFIGS["c5"]
-    a_src, a_dst, phi0 = W.gs_inputs_c5(cfg)
+    a_src, a_dst, phi0 = _gs_inputs_c5(W)
     d_src, d_dst = torch.from_numpy(a_src).cuda(), torch.from_numpy(a_dst).cuda()
     d_phi0 = torch.from_numpy(phi0).cuda()
     d_phi = torch.empty_like(d_phi0)
@@ -399,6 +492,91 @@ def make_workload(name, rank, torch, api, W):
                      "20 iterations (41 propagations per call)",
                 l2="537 MB field + 1074 MB workspace per propagation (>> 126 MB L2); no flush",
                 metric="propagations/sec inside cwo_gs (c5, 41 per call); effective HBM GB/s for 168 N^2 bytes per iteration")
+
+
+KIND_NAMES = {0: "pass_R (row FFT)", 1: "pass_R' (row IFFT)", 2: "pass_C0 (column FFT)",
+              3: "pass_C (fused column FFT*H*IFFT)", 4: "pass_C' (H * column IFFT)",
+              5: "line convolution pass (FFT*C*IFFT per line, separable Fresnel)", 6: "transpose",
+              7: "line transform pass (pre * FFT * post per line, Fourier-form Fresnel)", 10: "point-light-source CGH (Eq.(23))"}
+KIND_KEYS = {0: "pass_R", 1: "pass_Rinv", 2: "pass_C0", 3: "pass_C", 4: "pass_Cmidinv", 5: "lineconv", 6: "transpose",
+             7: "linefft", 10: "pls"}
+
+
+def _roofline(wl, tm, workload):
+    """The roofline object of the dominant kernel from the library-recorded per-launch times `tm` ([(tag, ms), ...])."""
+    per_kind = {}
+    for tag, t_ms in tm:
+        per_kind.setdefault(tag & 15, []).append(t_ms)
+    names = KIND_NAMES
+    passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
+    dom_kind = max(per_kind, key=lambda k: np.sum(per_kind[k]))
+    dom_ms = float(np.mean(per_kind[dom_kind]))
+    peak, peak_src = _peak()
+    tot = sum(float(np.sum(v)) for v in per_kind.values())
+    alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves (DESIGN.md 6)
+    hbm_gbs = alg_bytes / (dom_ms * 1e-3) / 1e9
+    traffic = _ncu_traffic(workload, KIND_KEYS.get(dom_kind, "-"))
+    common = {"kernel": names[dom_kind], "traffic": traffic,
+              "traffic_source": "profiles/traffic.csv (committed ncu --set full capture; not measured by this run)" if traffic else None,
+              "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms, "pass_ms": passes,
+              "step_share": float(np.sum(per_kind[dom_kind])) / tot,
+              "hbm_gbs": hbm_gbs, "hbm_frac": hbm_gbs / peak, "hbm_peak": peak, "hbm_peak_source": peak_src}
+    if dom_kind in wl.get("kind_flops", {}):
+        # the line-convolution passes are bound by the fp32 pipes, not by HBM (DESIGN.md 6): nominal flops per launch
+        # over the live duration against 148 SMs x 128 lanes x 2 x 1965 MHz
+        fl = wl["kind_flops"][dom_kind]
+        ach = fl / (dom_ms * 1e-3) / 1e12
+        return dict(common, bound="alu", achieved=ach, peak=FP32_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / FP32_PEAK_TFLOPS,
+                    peak_source="148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
+                    nominal_flops_per_launch=fl)
+    return dict(common, bound="hbm", achieved=hbm_gbs, peak=peak, unit="GB/s", frac=hbm_gbs / peak, peak_source=peak_src)
+
+
+# the other sizes north_star's target names (SURVEY.md 8(d) table: time at 60 % of 8 TB/s for the algorithmic bytes), timed
+# briefly after the headline so that the driver's one JSON line carries them: (workload, timed steps, target ms per call)
+EXTRA_WORKLOADS = (("asm8192", 30, 0.671), ("fresnel4096", 40, 0.280), ("fresnel8192", 15, 1.118), ("c4", 6, 1.818),
+                   ("c5", 2, 48.0))
+
+
+def time_extra(name, steps, target_ms, local, torch, api, W):
+    """One extra workload, device-resident, CUDA events on the launching stream: a compact record for the `extra` object."""
+    wl = make_workload(name, 0, torch, api, W, nbuf=1)
+    plan, step = wl["plan"], wl["step"]
+    stream = torch.cuda.current_stream()
+    sampler = ClockSampler(local)
+    sampler.start()
+    for i in range(3):
+        step(i)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(steps):
+        step(i)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    plan.set_timing(True)
+    for i in range(6 if wl["props_per_step"] == 1 else 1):
+        step(i)
+    tm = plan.timings(65536)
+    plan.set_timing(False)
+    t_end, i = time.time() + 1.5, 0
+    while len(sampler.rows) < 4 and time.time() < t_end and sampler.proc is not None:
+        step(i); i += 1
+        torch.cuda.synchronize()
+    clocks = sampler.stop()
+    r = _roofline(wl, tm, name)
+    peak, _ = _peak()
+    eff = wl["bytes_per_step"] / (ms * 1e-3) / 1e9
+    rec = {"workload": wl["desc"], "steps": steps, "warmup": 3, "ms_per_call": ms, "target_ms_per_call": target_ms,
+           "value": wl["props_per_step"] / (ms * 1e-3), "unit": "propagations/s" if name != "c4" else "planes/s",
+           "bytes_per_call": int(wl["bytes_per_step"]), "effective_gbs": eff, "pct_of_8TBs": 100.0 * eff / NOMINAL_HBM_GBS,
+           "pct_of_measured_copy": 100.0 * eff / peak,
+           "roofline": {k: r[k] for k in ("kernel", "bound", "achieved", "peak", "unit", "frac", "kernel_ms", "step_share")},
+           "clocks": clocks}
+    del wl, plan, step
+    torch.cuda.empty_cache()
+    return rec
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -500,37 +678,7 @@ def run_cuda(args):
                 torch.cuda.synchronize()
         torch.cuda.synchronize()
     clocks = sampler.stop() if rank == 0 else None
-    per_kind = {}
-    for tag, t_ms in tm:
-        per_kind.setdefault(tag & 15, []).append(t_ms)
-    names = {0: "pass_R (row FFT)", 1: "pass_R' (row IFFT)", 2: "pass_C0 (column FFT)",
-             3: "pass_C (fused column FFT*H*IFFT)", 4: "pass_C' (H * column IFFT)",
-             5: "line convolution pass (FFT*C*IFFT per line, separable Fresnel)", 6: "transpose",
-             7: "line transform pass (pre * FFT * post per line, Fourier-form Fresnel)", 10: "point-light-source CGH (Eq.(23))"}
-    passes = {names[k]: float(np.mean(v)) for k, v in per_kind.items() if k in names}
-    dom_kind = max(per_kind, key=lambda k: np.sum(per_kind[k]))
-    dom_ms = float(np.mean(per_kind[dom_kind]))
-    peak, peak_src = _peak()
-    tot = sum(float(np.sum(v)) for v in per_kind.values())
-    alg_bytes = wl["kind_bytes"][dom_kind]         # algorithmic bytes one launch of that pass moves
-    hbm_gbs = alg_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = _ncu_traffic(args.workload, {0: "pass_R", 1: "pass_Rinv", 2: "pass_C0", 3: "pass_C", 4: "pass_Cmidinv", 5: "lineconv", 6: "transpose", 7: "linefft", 10: "pls"}.get(dom_kind, "-"))
-    common = {"kernel": names[dom_kind], "traffic": traffic,
-              "traffic_source": "profiles/traffic.csv (committed ncu --set full capture; not measured by this run)" if traffic else None,
-              "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": dom_ms, "pass_ms": passes,
-              "step_share": float(np.sum(per_kind[dom_kind])) / tot,
-              "hbm_gbs": hbm_gbs, "hbm_frac": hbm_gbs / peak, "hbm_peak": peak, "hbm_peak_source": peak_src}
-    if dom_kind in wl.get("kind_flops", {}):
-        # the line-convolution passes are bound by the fp32 pipes, not by HBM: nominal flops per launch
-        # over the live duration against 148 SMs x 128 lanes x 2 x 1965 MHz
-        fl = wl["kind_flops"][dom_kind]
-        ach = fl / (dom_ms * 1e-3) / 1e12
-        roofline = dict(common, bound="alu", achieved=ach, peak=FP32_PEAK_TFLOPS, unit="TFLOP/s", frac=ach / FP32_PEAK_TFLOPS,
-                        peak_source="148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks)",
-                        nominal_flops_per_launch=fl)
-    else:
-        roofline = dict(common, bound="hbm", achieved=hbm_gbs, peak=peak, unit="GB/s", frac=hbm_gbs / peak,
-                        peak_source=peak_src)
+    roofline = _roofline(wl, tm, args.workload)
 
     # ---- end to end: host (pinned) buffers, H2D + propagate + D2H every step -----------------------
     e2e_step, h2d, d2h = wl["e2e"]()
@@ -556,6 +704,7 @@ def run_cuda(args):
            "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
 
     if rank == 0:
+        peak, _ = _peak()
         ms_step = ms / args.steps
         eff = wl["bytes_per_step"] / (ms_step * 1e-3) / 1e9
         line = {"metric": METRIC if args.workload == "c3" else wl["metric"], "value": value, "unit": UNIT, "n_gpus": world,
@@ -573,8 +722,18 @@ def run_cuda(args):
             line["ms_per_step_cuda_graph"] = graph_ms       # the step is launch-bound through the Python binding
         if args.fresnel_2d or args.no_pipeline:
             line["not_a_benchmark"] = "fresnel_2d=%d no_pipeline=%d" % (int(args.fresnel_2d), int(args.no_pipeline))
+        if world == 1 and not args.no_extra and args.workload == "c3":
+            # the headline's buffers are no longer needed: release them before the 8192^2 workloads allocate theirs
+            del wl, plan, step, e2e_step
+            torch.cuda.empty_cache()
+            line["extra"] = {}
+            for name, k, target in EXTRA_WORKLOADS:
+                try:
+                    line["extra"][name] = time_extra(name, k, target, local, torch, api, W)
+                except Exception as ex:       # the headline must still be printed
+                    line["extra"][name] = {"error": repr(ex)}
         if world == 1 and not args.no_cpu_baseline and args.workload == "c3":
-            line["cpu_baseline"] = cpu_baseline(W.CONFIGS["c3"])
+            line["cpu_baseline"] = cpu_baseline(W.CONFIGS["c3"], per_config=not args.no_extra)
         print(json.dumps(line), flush=True)
     if use_dist:
         dist.destroy_process_group()
@@ -587,6 +746,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip the `extra` legs (asm8192, fresnel4096, fresnel8192, c4, c5 timed briefly after c3) and the "
+                         "per-config / one-thread oracle timings (profiling runs)")
     ap.add_argument("--no-pipeline", action="store_true",
                     help="CWO_OPT_PIPELINE = 0: one CTA per tile everywhere (comparison runs only)")
     ap.add_argument("--fresnel-2d", action="store_true",
