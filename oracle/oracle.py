@@ -173,6 +173,13 @@ def stack_intensity(u1, px, py, lam, zs):
     return out
 
 
+def intensity(u):
+    """Intensity of a complex amplitude, Eq.(20): I(m, n) = Re(u)^2 + Im(u)^2, in fp64 (the paper's c.Intensity()
+    applied to one diffracted plane, Listing 1)."""
+    u = _z(u)
+    return u.real * u.real + u.imag * u.imag
+
+
 def asm_shifted(u1, px, py, lam, z, ox=0.0, oy=0.0):
     """Shifted (band-limited) angular spectrum method, Eq.(18)-(19) P:L213-229; (ox, oy) = destination offset [m]."""
     u1 = _z(u1); u2 = np.empty_like(u1)

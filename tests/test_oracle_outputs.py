@@ -50,3 +50,19 @@ def test_pls_superposition_and_depth(oracle):
     one = oracle.pls_cgh(ny, nx, p, p, LAM, [0.0], [0.0], [0.1], [1.0])
     ref = cf.pls_term(repr(LAM), "0.1", repr(7 * p), repr(-3 * p))
     assert abs(one[16 - 3, 16 + 7] - ref) < 1e-9
+
+
+def test_intensity_is_re2_plus_im2(oracle):
+    # Eq.(20): exact small integers (3-4-5, 5-12-13), unit phasors, |c u|^2 = |c|^2 |u|^2, Parseval against the oracle's own
+    # FFT, and the C oracle's stack intensity of one plane (written independently in cwo_oracle.c)
+    u = np.array([[3 + 4j, -5 + 12j], [0j, -1j]])
+    assert np.array_equal(oracle.intensity(u), np.array([[25.0, 169.0], [0.0, 1.0]]))
+    r = np.random.default_rng(3)
+    th = r.uniform(0, 2 * np.pi, (8, 16))
+    assert np.allclose(oracle.intensity(np.exp(1j * th)), 1.0, rtol=0, atol=1e-15)
+    v = r.standard_normal((8, 16)) + 1j * r.standard_normal((8, 16))
+    assert np.allclose(oracle.intensity((2 - 1j) * v), 5.0 * oracle.intensity(v), rtol=1e-14)
+    assert np.isclose(oracle.intensity(oracle.fft2d(v)).sum(), v.size * oracle.intensity(v).sum(), rtol=1e-13)
+    px, lam, z = 4e-6, LAM, 0.003
+    assert np.allclose(oracle.intensity(oracle.asm(v, px, px, lam, z)), oracle.stack_intensity(v, px, px, lam, [z])[0],
+                       rtol=1e-13, atol=0)
