@@ -68,11 +68,16 @@ enum {
     CWO_OPT_STACK_INTENSITY = 6, /* value 1: cwo_propagate_stack writes the INTENSITY |u|^2 of every plane (Eq.(20),
                                P:L254-256; the quantity the paper's 3-D example renders) as float [n][Ny][Nx]
                                instead of the complex amplitude: half the output bytes.  Default 0. */
-    CWO_OPT_ASM_BAND_LIMIT = 7 /* value 1: cwo_asm multiplies the transfer function by the two Rect band limits of
+    CWO_OPT_ASM_BAND_LIMIT = 7, /* value 1: cwo_asm multiplies the transfer function by the two Rect band limits of
                                Eq.(18)-(19) for the on-axis case: bins with |fx| > 1/(lambda
                                sqrt((2 dfx z)^2 + 1)) (same in y) are zeroed, which removes the aliased part of H at
                                long distances.  Default 0.  cwo_propagate_stack and cwo_gs ignore this option and the
                                offset of cwo_plan_set_offset: they always apply the plain H of Eq.(16). */
+    CWO_OPT_OUT_INTENSITY = 8 /* value 1: cwo_asm, cwo_fresnel_conv, cwo_fresnel_fourier and cwo_fresnel_shifted write the
+                               INTENSITY |u2|^2 (Eq.(20); the paper's Diffract -> Intensity of Listing 1,
+                               P:L245-252) as float [Ny][Nx] through the u2 pointer (4*Nx*Ny bytes) instead of the complex
+                               amplitude: the conversion happens in the call's last store, there is no extra pass.
+                               u2 == u1 stays allowed.  Default 0.  (The stack has CWO_OPT_STACK_INTENSITY.) */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
 

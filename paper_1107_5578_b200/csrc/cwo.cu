@@ -26,7 +26,7 @@ struct cwo_plan_s {
     cudaStream_t stream;
     void* ws;
     size_t ws_bytes;
-    int gs_method, pipeline, asm_pad2x, stack_intensity, band_limit, fresnel_2d;
+    int gs_method, pipeline, asm_pad2x, stack_intensity, band_limit, fresnel_2d, out_intensity;
     int fresnel_gather;             // include/cwo_debug.h: -1 auto (by field size), 0 transposing form, 1 gathering form
     int last_cuda_error;
     long long launches;
@@ -238,6 +238,10 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
         case CWO_OPT_ASM_BAND_LIMIT:
             if (!flag) return CWO_EINVAL;
             p->band_limit = value;
+            return CWO_OK;
+        case CWO_OPT_OUT_INTENSITY:
+            if (!flag) return CWO_EINVAL;
+            p->out_intensity = value;
             return CWO_OK;
     }
     return CWO_EINVAL;
@@ -588,7 +592,8 @@ static bool touches_ws(cwo_plan_t p, const void* q, size_t n) { return p->ws && 
 // u1 -> u2, both complex Nx x Ny fields
 static bool fields_alias_badly(cwo_plan_t p, const void* u1, const void* u2) {
     const size_t fb = sizeof(float2) * (size_t)p->Nx * p->Ny;
-    return partial_overlap(u1, u2, fb) || touches_ws(p, u1, fb) || touches_ws(p, u2, fb);
+    const size_t ob = p->out_intensity ? fb / 2 : fb;                  // CWO_OPT_OUT_INTENSITY: u2 holds floats
+    return (u1 != u2 && overlaps(u1, fb, u2, ob)) || touches_ws(p, u1, fb) || touches_ws(p, u2, ob);
 }
 
 extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
@@ -602,7 +607,7 @@ extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     int rc;
     const bool band = p->band_limit != 0;
     if (split && (rc = build_asm_tables(p, g, &z, 1, p->asm_tab, nullptr, band)) != CWO_OK) return rc;
-    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
+    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, p->out_intensity ? OUT_INTENSITY : OUT_COMPLEX, u2, nullptr};
     return run_passes(p, CWO_GS_ASM, z, 0, split, poly, io, (float2*)p->ws, pad2x, band);
 }
 
@@ -635,6 +640,11 @@ static int transpose_c64(cwo_plan_t p, const float2* in, float2* out, int rows, 
 static int transpose_f32(cwo_plan_t p, const float* in, float* out, int rows, int cols) {
     return launch_tagged(p, KIND_TRANSPOSE, [&] { return launch_transpose_f32(in, out, rows, cols, p->stream); });
 }
+// the last transposition of a separable call: complex u2, or |u2|^2 as floats with CWO_OPT_OUT_INTENSITY
+static int transpose_out(cwo_plan_t p, const float2* in, void* u2, int rows, int cols) {
+    if (!p->out_intensity) return transpose_c64(p, in, (float2*)u2, rows, cols);
+    return launch_tagged(p, KIND_TRANSPOSE, [&] { return launch_transpose_abs2(in, (float*)u2, rows, cols, p->stream); });
+}
 
 extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     if (!p || !aligned16(u1) || !aligned16(u2) || !isfinite(z) || z == 0.0 || !fresnel_sizes_ok(p)) return CWO_EINVAL;
@@ -643,7 +653,8 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
     if (fields_alias_badly(p, u1, u2)) return CWO_EINVAL;
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0);
     if (rc != CWO_OK) return rc;
-    if (fresnel_separable(p) && separable_gather(p)) {
+    // (the intensity output is formed by the last transposition: the gathering form has none)
+    if (fresnel_separable(p) && separable_gather(p) && !p->out_intensity) {
         // y first (lines = columns of u1, gathered; result in the transposed layout [Nx][Ny]), then x (lines = columns
         // of that, gathered; result row-major [Ny][Nx])
         float2* w0 = (float2*)p->ws;
@@ -667,9 +678,9 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
         memset(&cp, 0, sizeof(cp));
         cp.in = w1; cp.out = w1; cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][1];
         if ((rc = conv_pass(p, 1, 0, cp)) != CWO_OK) return rc;                     // columns, in place
-        return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);                      // u2 = w1^T
+        return transpose_out(p, w1, u2, p->Nx, p->Ny);                               // u2 = w1^T (or |w1^T|^2)
     }
-    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, OUT_COMPLEX, u2, nullptr};
+    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, p->out_intensity ? OUT_INTENSITY : OUT_COMPLEX, u2, nullptr};
     return run_passes(p, CWO_GS_FRESNEL, z, 0, false, false, io, (float2*)p->ws);
 }
 
@@ -717,7 +728,7 @@ extern "C" int cwo_fresnel_fourier(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     lp.tw = p->tw[p->logny]; lp.n_lines = p->Nx;
     rc = launch_tagged(p, p->logny * 16 + KIND_LINEFFT, [&] { return kLineFft[p->logny](p->stream, lp); });   // columns, in place
     if (rc != CWO_OK) return rc;
-    return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);
+    return transpose_out(p, w1, u2, p->Nx, p->Ny);
 }
 
 extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
@@ -739,7 +750,7 @@ extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     b.t[2] = QuadTab{p->quad[1][0], p->Ny, 0, 0.0, -p->py * p->off_y / lz, p->py * (p->py - p1y) / (2.0 * lz), 1.0};
     b.t[3] = QuadTab{p->quad[1][1], p->Ny, 0, p->off_y * p->off_y / (2.0 * lz), p1y * p->off_y / lz, p1y * (p1y - p->py) / (2.0 * lz), 1.0};
     if ((rc = build_quad(p, b)) != CWO_OK) return rc;
-    if (separable_gather(p)) {
+    if (separable_gather(p) && !p->out_intensity) {
         float2* w0 = (float2*)p->ws;
         ConvParams cp; memset(&cp, 0, sizeof(cp));
         cp.in = (const float2*)u1; cp.gather = 1; cp.in_stride = p->Nx; cp.out = w0;
@@ -762,7 +773,7 @@ extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     cp.in = w1; cp.out = w1; cp.tab[0] = (const ulonglong2*)p->chirp_pairs[0][1];
     cp.pre = p->quad[1][0]; cp.post = p->quad[1][1];
     if ((rc = conv_pass(p, 1, 4, cp)) != CWO_OK) return rc;
-    return transpose_c64(p, w1, (float2*)u2, p->Nx, p->Ny);
+    return transpose_out(p, w1, u2, p->Nx, p->Ny);
 }
 
 // ---- output conversions (outputs.cu) ----------------------------------------------------------------------------

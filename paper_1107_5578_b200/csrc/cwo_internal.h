@@ -153,6 +153,7 @@ cudaError_t build_quad_phase_tables(const QuadTabBatch& b, int n_tabs, cudaStrea
 // out[c][r] = in[r][c] (transpose.cu); rows, cols multiples of 32
 cudaError_t launch_transpose_c64(const float2* in, float2* out, int rows, int cols, cudaStream_t s);
 cudaError_t launch_transpose_f32(const float* in, float* out, int rows, int cols, cudaStream_t s);
+cudaError_t launch_transpose_abs2(const float2* in, float* out, int rows, int cols, cudaStream_t s);   // out[c][r] = |in[r][c]|^2
 
 // outputs.cu: Scale (Eq.(21)) and the point-light-source CGH (Eq.(23))
 cudaError_t launch_minmax(const float* in, size_t n, unsigned* mm, int n_sm, cudaStream_t s);     // mm: {min, max} encoded

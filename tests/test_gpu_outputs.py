@@ -148,3 +148,72 @@ def test_new_calls_capture_into_a_cuda_graph_and_replay(api, oracle):
         got = holo.cpu().numpy().astype(np.float64)
         assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= REL_L2
         assert np.abs(holo8.cpu().numpy() - oracle.scale255(got)).max() <= 255 * 4e-6
+
+
+# ---------------------------------------------------------------- intensity output of one propagation -----------------
+
+def _rand_field(shape, seed):
+    r = np.random.default_rng(seed)
+    return (r.standard_normal(shape) + 1j * r.standard_normal(shape)).astype(np.complex64)
+
+
+def _assert_intensity(got, ref, what):
+    got = got.astype(np.float64)
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    mx = np.max(np.abs(got - ref)) / np.max(ref)
+    # |u|^2 doubles the relative error of u: bars 2 x (2e-5, 1e-4), as for the intensity stack
+    assert rel <= 2 * REL_L2 and mx <= 2 * MAX_ABS, "%s: rel-L2 %.3e max/peak %.3e" % (what, rel, mx)
+
+
+@pytest.mark.parametrize("case", [
+    ("asm", (64, 64)), ("asm", (256, 512)), ("asm", (1024, 1024)), ("asm", (64, 4096)), ("asm", (64, 8192)), ("asm", (32, 16384)),
+    ("asm", (2048, 2048)), ("asm_pad2x", (256, 256)), ("asm_pad2x", (1024, 1024)), ("asm_pad2x", (64, 4096)),
+    ("fresnel", (64, 64)), ("fresnel", (128, 32)), ("fresnel", (256, 512)), ("fresnel", (1024, 1024)), ("fresnel", (4096, 256)),
+    ("fourier", (256, 512)), ("fourier", (1024, 1024)), ("shifted", (512, 256)), ("shifted", (1024, 1024))],
+    ids=lambda c: "%s-%dx%d" % (c[0], c[1][0], c[1][1]))
+def test_intensity_output_of_single_propagations(api, oracle, case):
+    """CWO_OPT_OUT_INTENSITY (the paper's Listing 1: Diffract -> Intensity): float |u2|^2 from the last store of cwo_asm
+    (circular and zero-expanded; scalar, lane-pair, pipelined and one-row tiles), cwo_fresnel_conv (three-pass form below
+    256, separable form above), cwo_fresnel_fourier and cwo_fresnel_shifted, against oracle.intensity of the oracle's
+    propagation, out of place and in place; and the complex output again once the option is switched off."""
+    op, shape = case
+    ny, nx = shape
+    px, py, lam = 4e-6, 5e-6, 633e-9
+    u1 = _rand_field(shape, 17 + nx % 13)
+    z = max(nx, ny) * px * px / lam * 0.35
+    plan = api.cwo_plan(nx, ny, px, lam)
+    plan.set_pitch_xy(px, py)
+    if op == "asm":
+        call, ref = api.cwo_asm, oracle.asm(u1, px, py, lam, z)
+    elif op == "asm_pad2x":
+        plan.set_option(api.CWO_OPT_ASM_PAD2X, 1)
+        call, ref = api.cwo_asm, oracle.asm_pad2x(u1, px, py, lam, z)
+    elif op == "fresnel":
+        call, ref = api.cwo_fresnel_conv, oracle.fresnel_conv(u1, px, py, lam, z)
+    elif op == "fourier":
+        call, ref = api.cwo_fresnel_fourier, oracle.fresnel_fourier(u1, px, py, lam, z)
+    else:
+        p1, off = (1.3 * px, 0.8 * py), (11.5 * px, -20.25 * py)
+        plan.set_dst_pitch_xy(*p1); plan.set_offset(*off)
+        call, ref = api.cwo_fresnel_shifted, oracle.fresnel_shifted(u1, (px, py), p1, lam, z, (0.0, 0.0), off)
+    plan.set_option(api.CWO_OPT_OUT_INTENSITY, 1)
+    d1 = torch.from_numpy(u1).cuda()
+    out = torch.full((ny, nx), -1.0, dtype=torch.float32, device="cuda")
+    call(plan, d1, out, z)
+    torch.cuda.synchronize()
+    assert torch.equal(d1.cpu(), torch.from_numpy(u1))                    # the input is untouched
+    _assert_intensity(out.cpu().numpy(), oracle.intensity(ref), "%s %s" % (op, shape))
+    # in place: the intensity occupies the first half of u1's bytes
+    with pytest.raises(TypeError):
+        call(plan, d1, d1, z)                                             # the binding wants a float32 tensor for u2
+    inplace = d1.view(torch.float32).view(-1)[: nx * ny].view(ny, nx)
+    call(plan, d1, inplace, z)
+    torch.cuda.synchronize()
+    assert torch.equal(inplace, out)
+    # option off again: complex output at the usual bar
+    plan.set_option(api.CWO_OPT_OUT_INTENSITY, 0)
+    d1 = torch.from_numpy(u1).cuda(); d2 = torch.empty_like(d1)
+    call(plan, d1, d2, z)
+    torch.cuda.synchronize()
+    got = d2.cpu().numpy().astype(np.complex128)
+    assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= REL_L2
