@@ -180,6 +180,30 @@ def intensity(u):
     return u.real * u.real + u.imag * u.imag
 
 
+def amplitude(u):
+    """|u| = sqrt(re^2 + im^2): the "amplitude" real field of section 5, the square root of Eq.(20)."""
+    return np.sqrt(intensity(u))
+
+
+def re(u):
+    """Real part of Eq.(24) P:L473-476 (the paper's Re(), conversion 1 P:L491)."""
+    return _z(u).real.copy()
+
+
+def im(u):
+    """Imaginary part of Eq.(24) P:L473-476."""
+    return _z(u).imag.copy()
+
+
+def phase(u):
+    """Argument of the complex amplitude, Eq.(25) P:L480-483 read as the four-quadrant atan2(im, re) in [-pi, pi] (the
+    paper's Phase(), conversion 2 P:L497); 0 where u == 0 (phasor(0) = 1, as in the GS loop)."""
+    u = _z(u)
+    th = np.arctan2(u.imag, u.real)
+    th[(u.real == 0) & (u.imag == 0)] = 0.0
+    return th
+
+
 def asm_shifted(u1, px, py, lam, z, ox=0.0, oy=0.0):
     """Shifted (band-limited) angular spectrum method, Eq.(18)-(19) P:L213-229; (ox, oy) = destination offset [m]."""
     u1 = _z(u1); u2 = np.empty_like(u1)

@@ -66,3 +66,22 @@ def test_intensity_is_re2_plus_im2(oracle):
     px, lam, z = 4e-6, LAM, 0.003
     assert np.allclose(oracle.intensity(oracle.asm(v, px, px, lam, z)), oracle.stack_intensity(v, px, px, lam, [z])[0],
                        rtol=1e-13, atol=0)
+
+
+def test_real_field_conversions_of_section_5(oracle):
+    # exact cases (3-4-5 triangle, the axes), and the paper's own round trips: Complex(a, b) of conversion 5 rebuilds u from
+    # amplitude and phase, conversion 6 from the real and imaginary parts
+    u = np.array([[3 + 4j, -3 + 4j, -3 - 4j], [1 + 0j, 1j, -1 + 0j], [-1j, 0j, 2 - 2j]])
+    assert np.array_equal(oracle.amplitude(u)[0], [5.0, 5.0, 5.0])
+    assert np.array_equal(oracle.re(u)[0], [3.0, -3.0, -3.0]) and np.array_equal(oracle.im(u)[0], [4.0, 4.0, -4.0])
+    th = oracle.phase(u)
+    assert np.allclose(th[1], [0.0, np.pi / 2, np.pi], atol=1e-15) and np.isclose(th[2, 0], -np.pi / 2)
+    assert th[2, 1] == 0.0 and np.isclose(th[2, 2], -np.pi / 4)
+    assert np.isclose(th[0, 0], np.arctan(4.0 / 3.0)) and np.isclose(th[0, 1], np.pi - np.arctan(4.0 / 3.0))   # quadrants
+    assert np.isclose(th[0, 2], -np.pi + np.arctan(4.0 / 3.0))
+    r = np.random.default_rng(5)
+    v = r.standard_normal((16, 8)) + 1j * r.standard_normal((16, 8))
+    assert np.allclose(oracle.amplitude(v) ** 2, oracle.intensity(v), rtol=1e-14)
+    assert np.allclose(oracle.amplitude(v) * np.exp(1j * oracle.phase(v)), v, rtol=1e-13)
+    assert np.array_equal(oracle.re(v) + 1j * oracle.im(v), v)
+    assert oracle.phase(v).min() >= -np.pi and oracle.phase(v).max() <= np.pi
