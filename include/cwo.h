@@ -73,13 +73,20 @@ enum {
                                sqrt((2 dfx z)^2 + 1)) (same in y) are zeroed, which removes the aliased part of H at
                                long distances.  Default 0.  cwo_propagate_stack and cwo_gs ignore this option and the
                                offset of cwo_plan_set_offset: they always apply the plain H of Eq.(16). */
-    CWO_OPT_OUT_INTENSITY = 8 /* value 1: cwo_asm, cwo_fresnel_conv, cwo_fresnel_fourier and cwo_fresnel_shifted write the
-                               INTENSITY |u2|^2 (Eq.(20); the paper's Diffract -> Intensity of Listing 1,
+    CWO_OPT_OUT_REAL = 8     /* value CWO_OUT_INTENSITY .. CWO_OUT_PHASE: cwo_asm, cwo_fresnel_conv, cwo_fresnel_fourier and
+                               cwo_fresnel_shifted write a REAL field of u2 (section 5: the paper's Intensity(),
+                               Amp, Re(), Im, Phase() applied to the diffracted plane, e.g. Diffract -> Intensity of Listing 1,
                                P:L245-252) as float [Ny][Nx] through the u2 pointer (4*Nx*Ny bytes) instead of the complex
                                amplitude: the conversion happens in the call's last store, there is no extra pass.
-                               u2 == u1 stays allowed.  Default 0.  (The stack has CWO_OPT_STACK_INTENSITY.) */
+                               u2 == u1 stays allowed.  Default CWO_OUT_COMPLEX.  (The stack has CWO_OPT_STACK_INTENSITY.) */
 };
 enum { CWO_GS_FRESNEL = 0, CWO_GS_ASM = 1 };
+enum { CWO_OUT_COMPLEX = 0,
+       CWO_OUT_INTENSITY = 1,   /* |u2|^2, Eq.(20) */
+       CWO_OUT_AMPLITUDE = 2,   /* |u2| */
+       CWO_OUT_RE = 3,          /* real part, Eq.(24) */
+       CWO_OUT_IM = 4,          /* imaginary part */
+       CWO_OUT_PHASE = 5 };     /* atan2(im, re) in [-pi, pi], Eq.(25); 0 where u2 == 0 */
 
 /* Plane parameters (SetPitch / SetWaveLength / Create).  pitch_x = pitch_y = pitch
  * [m], lambda [m].  Frequency sampling is 1/(M*pitch) with M the transform size.

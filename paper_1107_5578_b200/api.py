@@ -30,7 +30,8 @@ CWO_OPT_PIPELINE = 3
 CWO_OPT_ASM_PAD2X = 5
 CWO_OPT_STACK_INTENSITY = 6
 CWO_OPT_ASM_BAND_LIMIT = 7
-CWO_OPT_OUT_INTENSITY = 8
+CWO_OPT_OUT_REAL = 8
+CWO_OUT_COMPLEX, CWO_OUT_INTENSITY, CWO_OUT_AMPLITUDE, CWO_OUT_RE, CWO_OUT_IM, CWO_OUT_PHASE = 0, 1, 2, 3, 4, 5
 CWO_GS_FRESNEL, CWO_GS_ASM = 0, 1
 
 # include/cwo.h (the product boundary) and include/cwo_debug.h (measurement hooks of the harness)
@@ -104,7 +105,7 @@ class Plan:
         self._ws = None
         self._ws_streams = set()      # streams (handles) the current workspace tensor has been recorded on
         self.stack_intensity = False
-        self.out_intensity = False
+        self.out_real = False         # CWO_OPT_OUT_REAL set: u2 of the single-propagation calls is float32
         rc = lib().cwo_plan(self.Nx, self.Ny, float(pitch), float(lam), ctypes.byref(self._h))
         if rc != CWO_OK:
             raise CwoError(rc, "cwo_plan")
@@ -120,8 +121,8 @@ class Plan:
         self._check(lib().cwo_plan_set_option(self._h, int(key), int(value)), "cwo_plan_set_option")
         if key == CWO_OPT_STACK_INTENSITY:
             self.stack_intensity = bool(value)
-        if key == CWO_OPT_OUT_INTENSITY:
-            self.out_intensity = bool(value)
+        if key == CWO_OPT_OUT_REAL:
+            self.out_real = bool(value)
 
     def set_offset(self, ox: float, oy: float) -> None:
         self._check(lib().cwo_plan_set_offset(self._h, float(ox), float(oy)), "cwo_plan_set_offset")
@@ -205,28 +206,28 @@ def cwo_plan(Nx: int, Ny: int, pitch: float, lam: float) -> Plan:
 
 def cwo_asm(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
     s = (plan.Ny, plan.Nx)
-    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_intensity else torch.complex64, s, "u2")
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_real else torch.complex64, s, "u2")
     plan.ensure_workspace(CWO_OP_ASM); plan.bind_stream()
     plan._check(lib().cwo_asm(plan._h, a, b, float(z)), "cwo_asm")
 
 
 def cwo_fresnel_conv(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
     s = (plan.Ny, plan.Nx)
-    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_intensity else torch.complex64, s, "u2")
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_real else torch.complex64, s, "u2")
     plan.ensure_workspace(CWO_OP_FRESNEL); plan.bind_stream()
     plan._check(lib().cwo_fresnel_conv(plan._h, a, b, float(z)), "cwo_fresnel_conv")
 
 
 def cwo_fresnel_fourier(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
     s = (plan.Ny, plan.Nx)
-    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_intensity else torch.complex64, s, "u2")
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_real else torch.complex64, s, "u2")
     plan.ensure_workspace(CWO_OP_FRESNEL_FOURIER); plan.bind_stream()
     plan._check(lib().cwo_fresnel_fourier(plan._h, a, b, float(z)), "cwo_fresnel_fourier")
 
 
 def cwo_fresnel_shifted(plan: Plan, u1: torch.Tensor, u2: torch.Tensor, z: float) -> None:
     s = (plan.Ny, plan.Nx)
-    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_intensity else torch.complex64, s, "u2")
+    a, b = _field(u1, torch.complex64, s, "u1"), _field(u2, torch.float32 if plan.out_real else torch.complex64, s, "u2")
     plan.ensure_workspace(CWO_OP_FRESNEL_SHIFTED); plan.bind_stream()
     plan._check(lib().cwo_fresnel_shifted(plan._h, a, b, float(z)), "cwo_fresnel_shifted")
 

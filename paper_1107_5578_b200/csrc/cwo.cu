@@ -26,7 +26,7 @@ struct cwo_plan_s {
     cudaStream_t stream;
     void* ws;
     size_t ws_bytes;
-    int gs_method, pipeline, asm_pad2x, stack_intensity, band_limit, fresnel_2d, out_intensity;
+    int gs_method, pipeline, asm_pad2x, stack_intensity, band_limit, fresnel_2d, out_real;   // out_real: CWO_OPT_OUT_REAL value (0 complex, 1..5)
     int fresnel_gather;             // include/cwo_debug.h: -1 auto (by field size), 0 transposing form, 1 gathering form
     int last_cuda_error;
     long long launches;
@@ -239,9 +239,9 @@ extern "C" int cwo_plan_set_option(cwo_plan_t p, int key, int value) {
             if (!flag) return CWO_EINVAL;
             p->band_limit = value;
             return CWO_OK;
-        case CWO_OPT_OUT_INTENSITY:
-            if (!flag) return CWO_EINVAL;
-            p->out_intensity = value;
+        case CWO_OPT_OUT_REAL:
+            if (value < CWO_OUT_COMPLEX || value > CWO_OUT_PHASE) return CWO_EINVAL;
+            p->out_real = value;
             return CWO_OK;
     }
     return CWO_EINVAL;
@@ -354,6 +354,7 @@ static Geometry geometry(cwo_plan_t p, int method, bool pad2x = false) {
 struct PropIO {
     int in_mode; const float2* in; const float* in_amp; const float* in_phase;
     int out_mode; void* out; const float* out_amp;
+    int real_mode;            // OUT_INTENSITY: RealMode (0 = |u|^2); omitted initialisers leave it 0
 };
 
 static int check_call(cwo_plan_t p) {
@@ -544,6 +545,7 @@ static int pass_row_fwd(cwo_plan_t p, const Geometry& g, const PropIO& io, float
 static int pass_row_inv(cwo_plan_t p, const Geometry& g, const PropIO& io, const float2* ws, float scale) {
     PassParams pp; row_params(p, g, pp);
     pp.in = ws; pp.out = (float2*)io.out; pp.out_mode = io.out_mode; pp.out_amp = io.out_amp; pp.out_scale = scale;
+    pp.real_mode = io.real_mode;
     if (row_fold(p, g, io.out_mode == OUT_COMPLEX) && encode_ws_tmap(&pp.tmap, ws, p->Ny, g.mx, g.logwc, 1)) {
         pp.use_fold = 1;
         return launch(p, g.logmx, ROW_INV, g.pad, MID_NONE, p->Ny, pp);
@@ -578,6 +580,12 @@ static int run_passes(cwo_plan_t p, int method, double z, int set, bool split, b
     return pass_row_inv(p, g, io, ws, scale);
 }
 
+// CWO_OPT_OUT_REAL value -> RealMode of the stores
+static int real_mode_of(cwo_plan_t p) { return p->out_real == CWO_OUT_PHASE ? REAL_PHASE : p->out_real > 0 ? p->out_real - 1 : 0; }
+// output mode of the inverse row pass of the two-dimensional forms (the phase has its own store mode: GS uses it)
+static int out_mode_of(cwo_plan_t p) {
+    return !p->out_real ? OUT_COMPLEX : p->out_real == CWO_OUT_PHASE ? OUT_PHASE : OUT_INTENSITY;
+}
 static bool aligned16(const void* q) { return q && !((uintptr_t)q & 15); }
 
 // Aliasing rules of cwo.h, checked on the pointer ranges alone (no kernel work): an output may coincide EXACTLY with the
@@ -592,7 +600,7 @@ static bool touches_ws(cwo_plan_t p, const void* q, size_t n) { return p->ws && 
 // u1 -> u2, both complex Nx x Ny fields
 static bool fields_alias_badly(cwo_plan_t p, const void* u1, const void* u2) {
     const size_t fb = sizeof(float2) * (size_t)p->Nx * p->Ny;
-    const size_t ob = p->out_intensity ? fb / 2 : fb;                  // CWO_OPT_OUT_INTENSITY: u2 holds floats
+    const size_t ob = p->out_real ? fb / 2 : fb;                       // CWO_OPT_OUT_REAL: u2 holds floats
     return (u1 != u2 && overlaps(u1, fb, u2, ob)) || touches_ws(p, u1, fb) || touches_ws(p, u2, ob);
 }
 
@@ -607,7 +615,7 @@ extern "C" int cwo_asm(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
     int rc;
     const bool band = p->band_limit != 0;
     if (split && (rc = build_asm_tables(p, g, &z, 1, p->asm_tab, nullptr, band)) != CWO_OK) return rc;
-    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, p->out_intensity ? OUT_INTENSITY : OUT_COMPLEX, u2, nullptr};
+    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, out_mode_of(p), u2, nullptr, real_mode_of(p)};
     return run_passes(p, CWO_GS_ASM, z, 0, split, poly, io, (float2*)p->ws, pad2x, band);
 }
 
@@ -640,10 +648,11 @@ static int transpose_c64(cwo_plan_t p, const float2* in, float2* out, int rows, 
 static int transpose_f32(cwo_plan_t p, const float* in, float* out, int rows, int cols) {
     return launch_tagged(p, KIND_TRANSPOSE, [&] { return launch_transpose_f32(in, out, rows, cols, p->stream); });
 }
-// the last transposition of a separable call: complex u2, or |u2|^2 as floats with CWO_OPT_OUT_INTENSITY
+// the last transposition of a separable call: complex u2, or a real field of it with CWO_OPT_OUT_REAL
 static int transpose_out(cwo_plan_t p, const float2* in, void* u2, int rows, int cols) {
-    if (!p->out_intensity) return transpose_c64(p, in, (float2*)u2, rows, cols);
-    return launch_tagged(p, KIND_TRANSPOSE, [&] { return launch_transpose_abs2(in, (float*)u2, rows, cols, p->stream); });
+    if (!p->out_real) return transpose_c64(p, in, (float2*)u2, rows, cols);
+    return launch_tagged(p, KIND_TRANSPOSE, [&] {
+        return launch_transpose_real(in, (float*)u2, rows, cols, real_mode_of(p), p->stream); });
 }
 
 extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, double z) {
@@ -654,7 +663,7 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
     int rc = build_fresnel_tables(p, geometry(p, CWO_GS_FRESNEL), z, 0);
     if (rc != CWO_OK) return rc;
     // (the intensity output is formed by the last transposition: the gathering form has none)
-    if (fresnel_separable(p) && separable_gather(p) && !p->out_intensity) {
+    if (fresnel_separable(p) && separable_gather(p) && !p->out_real) {
         // y first (lines = columns of u1, gathered; result in the transposed layout [Nx][Ny]), then x (lines = columns
         // of that, gathered; result row-major [Ny][Nx])
         float2* w0 = (float2*)p->ws;
@@ -680,7 +689,7 @@ extern "C" int cwo_fresnel_conv(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2, do
         if ((rc = conv_pass(p, 1, 0, cp)) != CWO_OK) return rc;                     // columns, in place
         return transpose_out(p, w1, u2, p->Nx, p->Ny);                               // u2 = w1^T (or |w1^T|^2)
     }
-    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, p->out_intensity ? OUT_INTENSITY : OUT_COMPLEX, u2, nullptr};
+    PropIO io = {IN_COMPLEX, (const float2*)u1, nullptr, nullptr, out_mode_of(p), u2, nullptr, real_mode_of(p)};
     return run_passes(p, CWO_GS_FRESNEL, z, 0, false, false, io, (float2*)p->ws);
 }
 
@@ -750,7 +759,7 @@ extern "C" int cwo_fresnel_shifted(cwo_plan_t p, const cwo_c64* u1, cwo_c64* u2,
     b.t[2] = QuadTab{p->quad[1][0], p->Ny, 0, 0.0, -p->py * p->off_y / lz, p->py * (p->py - p1y) / (2.0 * lz), 1.0};
     b.t[3] = QuadTab{p->quad[1][1], p->Ny, 0, p->off_y * p->off_y / (2.0 * lz), p1y * p->off_y / lz, p1y * (p1y - p->py) / (2.0 * lz), 1.0};
     if ((rc = build_quad(p, b)) != CWO_OK) return rc;
-    if (separable_gather(p) && !p->out_intensity) {
+    if (separable_gather(p) && !p->out_real) {
         float2* w0 = (float2*)p->ws;
         ConvParams cp; memset(&cp, 0, sizeof(cp));
         cp.in = (const float2*)u1; cp.gather = 1; cp.in_stride = p->Nx; cp.out = w0;

@@ -10,6 +10,20 @@ namespace cwo {
 
 enum InMode { IN_COMPLEX = 0, IN_AMP_PHASE = 1 };
 enum OutMode { OUT_COMPLEX = 0, OUT_PHASOR_AMP = 1, OUT_PHASE = 2, OUT_INTENSITY = 3 };
+// the real fields of section 5 an OUT_INTENSITY store can write; REAL_PHASE only in the transposing store
+enum RealMode { REAL_ABS2 = 0, REAL_ABS = 1, REAL_RE = 2, REAL_IM = 3, REAL_PHASE = 4 };
+#ifdef __CUDACC__
+// real field of the sample (re - i mim) * sc, i.e. of the conjugate of (re, mim) as the inverse passes hold it
+__device__ __forceinline__ float real_field(float re, float mim, float sc, int mode) {
+    switch (mode) {
+        case REAL_ABS: return sqrtf(re * re + mim * mim) * sc;
+        case REAL_RE: return re * sc;
+        case REAL_IM: return -mim * sc;
+        case REAL_PHASE: return (re == 0.0f && mim == 0.0f) ? 0.0f : atan2f(-mim, re);     // Eq.(25); phasor(0) = 1
+        default: return (re * re + mim * mim) * (sc * sc);                                   // Eq.(20)
+    }
+}
+#endif
 enum MidMode { MID_NONE = 0, MID_TABLES = 1, MID_ASM_SPLIT = 2, MID_ASM_F64 = 3 };
 
 struct PassParams {
@@ -39,6 +53,7 @@ struct PassParams {
     int use_pipe;             // 1: use the pipelined form where it exists (CWO_OPT_PIPELINE)
     const float2* tw;         // forward twiddles exp(-i 2 pi m/n), m < n
     float out_scale;          // ROW_INV store
+    int real_mode;            // OUT_INTENSITY store: which real field (RealMode; 0 = |u|^2)
     // Mid (transfer function / impulse-response spectrum, S2/S5/S7); lane = x bin, point = y bin
     double z, inv_lam2, df_lane, df_point;   // MID_ASM_F64
     int n_lane_bins;                          // Mx (signed-bin map of the lane index)
@@ -153,7 +168,7 @@ cudaError_t build_quad_phase_tables(const QuadTabBatch& b, int n_tabs, cudaStrea
 // out[c][r] = in[r][c] (transpose.cu); rows, cols multiples of 32
 cudaError_t launch_transpose_c64(const float2* in, float2* out, int rows, int cols, cudaStream_t s);
 cudaError_t launch_transpose_f32(const float* in, float* out, int rows, int cols, cudaStream_t s);
-cudaError_t launch_transpose_abs2(const float2* in, float* out, int rows, int cols, cudaStream_t s);   // out[c][r] = |in[r][c]|^2
+cudaError_t launch_transpose_real(const float2* in, float* out, int rows, int cols, int real_mode, cudaStream_t s);   // out[c][r] = real field of in[r][c]
 
 // outputs.cu: Scale (Eq.(21)) and the point-light-source CGH (Eq.(23))
 cudaError_t launch_minmax(const float* in, size_t n, unsigned* mm, int n_sm, cudaStream_t s);     // mm: {min, max} encoded

@@ -401,8 +401,13 @@ pass_kernel(const __grid_constant__ PassParams P) {
                 const int row = lane0 + (C::PAIR ? s : 0);
                 if (row >= P.rows) continue;
                 const size_t base = (size_t)row * P.pitch + u[s];
+                if (P.real_mode == REAL_ABS2) {
 #pragma unroll
-                for (int e = 0; e < NE; ++e) outf[base + e * Q] = (v[s][e].x * v[s][e].x + v[s][e].y * v[s][e].y) * sc2;
+                    for (int e = 0; e < NE; ++e) outf[base + e * Q] = (v[s][e].x * v[s][e].x + v[s][e].y * v[s][e].y) * sc2;
+                } else {                                        // |u|, Re u, Im u (section 5); the sample is conj(v)
+#pragma unroll
+                    for (int e = 0; e < NE; ++e) outf[base + e * Q] = real_field(v[s][e].x, v[s][e].y, P.out_scale, P.real_mode);
+                }
             }
         } else {
             // OUT_PHASE, Eq.(25) P:L482 as atan2, by a rolled loop over the thread's samples staged through its own

@@ -440,8 +440,13 @@ pipe_kernel(const __grid_constant__ PassParams P) {
                         pk_split(pv.r[e], ar, br); pk_split(pv.i[e], ai, bi);
                         const float2 m = cmul(make_float2(br, bi), e < 8 ? tq[e] : cmul_mi(tq[e - 8]));
                         const float2 lo = make_float2(ar + m.x, ai + m.y), hi = make_float2(ar - m.x, ai - m.y);
-                        y[e * QH] = (lo.x * lo.x + lo.y * lo.y) * (sc * sc);
-                        y[H + e * QH] = (hi.x * hi.x + hi.y * hi.y) * (sc * sc);
+                        if (P.real_mode == REAL_ABS2) {
+                            y[e * QH] = (lo.x * lo.x + lo.y * lo.y) * (sc * sc);
+                            y[H + e * QH] = (hi.x * hi.x + hi.y * hi.y) * (sc * sc);
+                        } else {
+                            y[e * QH] = real_field(lo.x, lo.y, sc, P.real_mode);
+                            y[H + e * QH] = real_field(hi.x, hi.y, sc, P.real_mode);
+                        }
                     }
                 } else if constexpr (IOM == OUT_PHASOR_AMP) {
                     // GS constraints (S10; Listing 8 lines 11-13 / 15-16): keep u/|u| (1 where u == 0), impose the amplitude
@@ -568,7 +573,9 @@ pipe_kernel(const __grid_constant__ PassParams P) {
                 for (int s = 0; s < 2; ++s)
 #pragma unroll
                     for (int e = 0; e < NE; ++e)
-                        smf[(w0 + s) * RS * 2 + us + e * Q] = (v[s][e].x * v[s][e].x + v[s][e].y * v[s][e].y) * (sc * sc);
+                        smf[(w0 + s) * RS * 2 + us + e * Q] =
+                            P.real_mode == REAL_ABS2 ? (v[s][e].x * v[s][e].x + v[s][e].y * v[s][e].y) * (sc * sc)
+                                                     : real_field(v[s][e].x, v[s][e].y, sc, P.real_mode);
             } else {
 #pragma unroll
                 for (int s = 0; s < 2; ++s)

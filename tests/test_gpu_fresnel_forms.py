@@ -176,7 +176,10 @@ def test_shifted_and_gs_in_both_forms(api, oracle, mode):
         p = oracle.gs_init(0, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, z)
         for _ in range(iters):
             p = oracle.gs_iter(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, z)
-        assert _phasor_rel_l2(ph.cpu().numpy(), p) <= REL_L2 * (1 + 2 * iters), "gs mode %d iters %d" % (mode, iters)
+        val = _phasor_rel_l2(ph.cpu().numpy(), p)
+        print("MEASURED gs 512x1024 mode %d iters %d: phasor rel-L2 %.3e" % (mode, iters, val))
+        # measured on the B200: 1.1e-6 (kinoform), 5.9e-6 (two iterations): the propagation bar itself holds
+        assert val <= REL_L2, "gs mode %d iters %d" % (mode, iters)
 
 
 @pytest.mark.parametrize("seed", range(10))

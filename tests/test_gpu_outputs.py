@@ -171,11 +171,12 @@ def _assert_intensity(got, ref, what):
     ("fresnel", (64, 64)), ("fresnel", (128, 32)), ("fresnel", (256, 512)), ("fresnel", (1024, 1024)), ("fresnel", (4096, 256)),
     ("fourier", (256, 512)), ("fourier", (1024, 1024)), ("shifted", (512, 256)), ("shifted", (1024, 1024))],
     ids=lambda c: "%s-%dx%d" % (c[0], c[1][0], c[1][1]))
-def test_intensity_output_of_single_propagations(api, oracle, case):
-    """CWO_OPT_OUT_INTENSITY (the paper's Listing 1: Diffract -> Intensity): float |u2|^2 from the last store of cwo_asm
-    (circular and zero-expanded; scalar, lane-pair, pipelined and one-row tiles), cwo_fresnel_conv (three-pass form below
-    256, separable form above), cwo_fresnel_fourier and cwo_fresnel_shifted, against oracle.intensity of the oracle's
-    propagation, out of place and in place; and the complex output again once the option is switched off."""
+def test_real_field_output_of_single_propagations(api, oracle, case):
+    """CWO_OPT_OUT_REAL (the paper's Listing 1: Diffract -> Intensity; section 5: Amp, Re(), Im, Phase()): a float field of
+    u2 from the last store of cwo_asm (circular and zero-expanded; scalar, lane-pair, pipelined and one-row tiles),
+    cwo_fresnel_conv (three-pass form below 256, separable form above), cwo_fresnel_fourier and cwo_fresnel_shifted, against
+    the oracle's conversion of the oracle's propagation; the intensity also in place; and the complex output again once the
+    option is switched off."""
     op, shape = case
     ny, nx = shape
     px, py, lam = 4e-6, 5e-6, 633e-9
@@ -196,24 +197,46 @@ def test_intensity_output_of_single_propagations(api, oracle, case):
         p1, off = (1.3 * px, 0.8 * py), (11.5 * px, -20.25 * py)
         plan.set_dst_pitch_xy(*p1); plan.set_offset(*off)
         call, ref = api.cwo_fresnel_shifted, oracle.fresnel_shifted(u1, (px, py), p1, lam, z, (0.0, 0.0), off)
-    plan.set_option(api.CWO_OPT_OUT_INTENSITY, 1)
     d1 = torch.from_numpy(u1).cuda()
-    out = torch.full((ny, nx), -1.0, dtype=torch.float32, device="cuda")
-    call(plan, d1, out, z)
-    torch.cuda.synchronize()
+    peak = np.abs(ref).max()
+    outs = {}
+    for mode, conv in ((api.CWO_OUT_INTENSITY, oracle.intensity), (api.CWO_OUT_AMPLITUDE, oracle.amplitude),
+                       (api.CWO_OUT_RE, oracle.re), (api.CWO_OUT_IM, oracle.im), (api.CWO_OUT_PHASE, oracle.phase)):
+        plan.set_option(api.CWO_OPT_OUT_REAL, mode)
+        out = torch.full((ny, nx), -7.0, dtype=torch.float32, device="cuda")
+        call(plan, d1, out, z)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().astype(np.float64)
+        outs[mode] = out
+        want = conv(ref)
+        what = "%s %s mode %d" % (op, shape, mode)
+        if mode == api.CWO_OUT_INTENSITY:
+            _assert_intensity(got, want, what)
+        elif mode == api.CWO_OUT_PHASE:
+            # the phase is ill-conditioned where |u2| is small (an error e moves it by e/|u2|): compare the phasors, weighted
+            # by the amplitude, at the propagation bars; and the range of Eq.(25)
+            assert got.min() >= -np.pi - 1e-6 and got.max() <= np.pi + 1e-6
+            d = np.abs(ref) * np.abs(np.exp(1j * got) - np.exp(1j * want))
+            assert np.linalg.norm(d) / np.linalg.norm(ref) <= REL_L2 and d.max() <= MAX_ABS * peak, what
+        else:
+            # |u|, Re, Im carry the error of u itself: the propagation bars, relative to the field's norm and peak
+            d = np.abs(got - want)
+            assert np.linalg.norm(d) / np.linalg.norm(ref) <= REL_L2 and d.max() <= MAX_ABS * peak, what
     assert torch.equal(d1.cpu(), torch.from_numpy(u1))                    # the input is untouched
-    _assert_intensity(out.cpu().numpy(), oracle.intensity(ref), "%s %s" % (op, shape))
-    # in place: the intensity occupies the first half of u1's bytes
+    # in place: the real field occupies the first half of u1's bytes
+    plan.set_option(api.CWO_OPT_OUT_REAL, api.CWO_OUT_INTENSITY)
     with pytest.raises(TypeError):
         call(plan, d1, d1, z)                                             # the binding wants a float32 tensor for u2
     inplace = d1.view(torch.float32).view(-1)[: nx * ny].view(ny, nx)
     call(plan, d1, inplace, z)
     torch.cuda.synchronize()
-    assert torch.equal(inplace, out)
+    assert torch.equal(inplace, outs[api.CWO_OUT_INTENSITY])
     # option off again: complex output at the usual bar
-    plan.set_option(api.CWO_OPT_OUT_INTENSITY, 0)
+    plan.set_option(api.CWO_OPT_OUT_REAL, api.CWO_OUT_COMPLEX)
     d1 = torch.from_numpy(u1).cuda(); d2 = torch.empty_like(d1)
     call(plan, d1, d2, z)
     torch.cuda.synchronize()
     got = d2.cpu().numpy().astype(np.complex128)
     assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= REL_L2
+    with pytest.raises(api.CwoError):
+        plan.set_option(api.CWO_OPT_OUT_REAL, 6)

@@ -172,7 +172,12 @@ def test_fresnel_2048_and_4096(api, oracle):
         got = _gpu_fresnel(api, u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024)
         if n == 2048:
             _assert_parity(got, oracle.fresnel_conv(u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024), "fresnel 2048")
-        else:       # sampled outputs: direct sum of Eq.(1) per point
+        else:
+            # the whole field against the oracle's Eq.(5) pipeline (three fp64 FFTs of 8192^2) ...
+            oracle.set_threads(oracle.max_threads())
+            _assert_parity(got, oracle.fresnel_conv(u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024), "fresnel 4096, full field")
+            oracle.set_threads(min(8, oracle.max_threads()))
+            # ... and sampled outputs against the direct sum of Eq.(1) per point (independent of the oracle's FFT)
             r = np.random.default_rng(1)
             ms = r.integers(0, n, 24); ns = r.integers(0, n, 24)
             ref = oracle.fresnel_points(u1, 8e-6, 8e-6, 532e-9, 0.2 * n / 1024, ms, ns)
@@ -276,7 +281,7 @@ def test_gs_kinoform_and_restart_parity(api, oracle, method, n):
 
 
 @pytest.mark.parametrize("method", [0, 1])
-@pytest.mark.parametrize("shape", [(2048, 2048), (4096, 64), (64, 4096), (8192, 64), (64, 8192)])
+@pytest.mark.parametrize("shape", [(2048, 2048), (4096, 4096), (4096, 64), (64, 4096), (8192, 64), (64, 8192)])
 def test_gs_restart_parity_long_transforms(api, oracle, method, shape):
     """The GS load / store modes (amp * exp(i phi) load, phasor x amplitude store, atan2 store) on the tile shapes of
     the 4096- .. 16384-point transforms, full field: kinoform (iters = 0) and one-iteration restart from the
@@ -911,4 +916,6 @@ def test_calls_capture_into_a_cuda_graph_and_replay(api, oracle):
         p = oracle.gs_init(0, amp_dst, phi0, cfg.pitch, cfg.pitch, cfg.lam, 0.02)
         for _ in range(2):
             p = oracle.gs_iter(0, amp_src, amp_dst, p, cfg.pitch, cfg.pitch, cfg.lam, 0.02)
-        assert _phasor_rel_l2(d_phi.cpu().numpy(), p) <= 5 * REL_L2     # two iterations: drift allowance
+        val = _phasor_rel_l2(d_phi.cpu().numpy(), p)
+        print("MEASURED graph gs two iterations: phasor rel-L2 %.3e" % val)
+        assert val <= REL_L2         # two iterations; measured 3.6e-6 on the B200 (SURVEY G5 allowed a drift of 5x)
